@@ -1,0 +1,448 @@
+"""Pins for the oracle's split-step scheme (oracle/gpe_oracle.c), CPU only.
+
+Each test compares the oracle with something fixed by the paper's statement of the method or
+by mathematics, not with the oracle itself: closed forms, conservation laws, an independent
+ODE integration, a numpy-FFT residual.  SURVEY.md 8(c) "What pins each part"; the paper's
+passages are cited per test.  A plausible mistake (dropped term, wrong sign or index,
+transposed axis, wrong factor order) fails at least one of them.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy.linalg import expm
+from scipy.special import jv
+
+import workloads as W
+from oracle.gpe_oracle import Oracle
+
+
+def _plain(n, L, **kw):
+    p = W._base(n, n, L)
+    p.update(kw)
+    return p
+
+
+def _moments(psi, p):
+    x = W.axis(p["nx"], p["Lx"])[:, None]
+    y = W.axis(p["ny"], p["Ly"])[None, :]
+    d = np.abs(psi) ** 2
+    d = d / d.sum()
+    return float((d * x * x).sum()), float((d * y * y).sum())
+
+
+# ------------------------------------------------------------------ schedule (reading Q4)
+def test_schedule_pulse_and_ramp():
+    p = _plain(64, 16.0, sched_step=np.array([0., 200., 200.]), sched_amp=np.array([7., 7., 0.]))
+    o = Oracle(p)
+    assert o.schedule(0, 0) == 7.0 and o.schedule(0, 199) == 7.0
+    assert o.schedule(0, 200) == 0.0 and o.schedule(0, 5000) == 0.0   # on for n < tau/dt
+    p = _plain(64, 16.0, sched_step=np.array([0., 10000.]), sched_amp=np.array([0., 20.]))
+    o = Oracle(p)
+    assert o.schedule(0, 2500) == pytest.approx(5.0, abs=1e-14)
+    assert o.schedule(0, 20000) == 20.0
+    assert Oracle(_plain(64, 16.0)).schedule(0, 3) == 0.0
+
+
+# ------------------------------------------------------------------ kinetic factor alone
+def test_kinetic_composition_exact():
+    """the kinetic factor is diagonal in k, so n steps of dt == one of n*dt."""
+    p = _plain(64, 16.0)
+    psi0 = W.noisy_gaussian(64, 64, 16.0, 16.0, 1.5, 3)
+    a, b = psi0.copy(), psi0.copy()
+    o = Oracle(p)
+    for _ in range(10):
+        o.kinetic_step(a, 1e-3, False)
+    o.kinetic_step(b, 1e-2, False)
+    assert np.linalg.norm(a - b) / np.linalg.norm(b) <= 1e-12
+    # and the full step with V=0, g=0 is that factor
+    c = psi0.copy()
+    Oracle(p).evolve(c, 1e-2, 1, False)
+    assert np.linalg.norm(c - b) / np.linalg.norm(b) <= 1e-13
+
+
+def test_free_gaussian_expansion():
+    """Free Schroedinger spreading, hbar=m=1: <x^2>(t) = s0^2/2 + t^2/(2 s0^2) per axis."""
+    n, L, s0 = 128, 40.0, 1.0
+    p = _plain(n, L)
+    psi = W.noisy_gaussian(n, n, L, L, s0, 0, noise=0.0)
+    o = Oracle(p)
+    t = 0.0
+    for _ in range(4):
+        o.evolve(psi, 0.05, 20, False)
+        t += 1.0
+        mx, my = _moments(psi, p)
+        expect = s0 ** 2 / 2 + t ** 2 / (2 * s0 ** 2)
+        assert mx == pytest.approx(expect, rel=1e-10)
+        assert my == pytest.approx(expect, rel=1e-10)
+    obs, _, _ = o.observables(psi)
+    assert obs[0]["norm"] == pytest.approx(1.0, abs=1e-12)
+    assert obs[0]["e_kin"] == pytest.approx(2 * 1.0 / (4 * s0 ** 2), rel=1e-10)  # conserved
+
+
+def test_anisotropic_axes_not_swapped():
+    """Lx != Ly, nx != ny: spreading along each axis follows its own width."""
+    nx, ny, Lx, Ly = 128, 64, 48.0, 24.0
+    p = W._base(nx, ny, Lx)
+    p["Ly"] = Ly
+    x = W.axis(nx, Lx)[:, None]
+    y = W.axis(ny, Ly)[None, :]
+    sx, sy = 2.0, 1.0
+    psi = np.exp(-x * x / (2 * sx * sx) - y * y / (2 * sy * sy)).astype(np.complex128)
+    psi = np.ascontiguousarray(psi)
+    Oracle(p).evolve(psi, 0.02, 50, False)
+    mx, my = _moments(psi, p)
+    assert mx == pytest.approx(sx ** 2 / 2 + 1.0 / (2 * sx ** 2), rel=1e-9)
+    assert my == pytest.approx(sy ** 2 / 2 + 1.0 / (2 * sy ** 2), rel=1e-9)
+
+
+# ------------------------------------------------------------------ potential factor alone
+@pytest.mark.parametrize("axis", [0, 1])
+def test_potential_factor_jacobi_anger(axis):
+    """PAPER.md:154 Eq. 9 / :67: uniform psi times exp(-i V0 cos^2(k r) dt/2) has k-space
+    amplitudes e^{-i b}(-i)^m J_m(b) at k = 2 m k_l, b = V0 dt/4 (Jacobi-Anger)."""
+    n, L, k = 256, 4 * math.pi, 4.0         # orders up to |m| = 7 resolved: aliasing J_13(b)
+    V0, dt = 800.0, 1e-3
+    beta = V0 * dt / 4                      # half step: phase (V0 dt/2) * (1 + cos 2kr)/2
+    p = _plain(n, L, lattice_axis=axis, lattice_k=k,
+               sched_step=np.array([0.]), sched_amp=np.array([V0]))
+    psi = np.full((n, n), 1.0 / L, dtype=np.complex128)
+    Oracle(p).potential_half_step(psi, dt, False)
+    hat = np.fft.fft2(psi) / (n * n) * L
+    dk = 2 * math.pi / L
+    for m in range(-3, 4):
+        idx = int(round(2 * m * k / dk)) % n
+        got = hat[idx, 0] if axis == 0 else hat[0, idx]
+        expect = np.exp(-1j * beta) * (-1j) ** abs(m) * jv(abs(m), beta)
+        assert abs(got - expect) <= 1e-11, (m, got, expect)
+    # imaginary time: the same factor is a real decay
+    psi = np.full((n, n), 1.0 / L, dtype=np.complex128)
+    Oracle(p).potential_half_step(psi, dt, True)
+    r = W.axis(n, L)
+    shape = np.cos(k * r) ** 2
+    expect = np.exp(-V0 * shape * dt / 2) / L
+    got = psi[:, 0] if axis == 0 else psi[0, :]
+    assert np.max(np.abs(got - expect)) <= 1e-15
+
+
+def test_potential_factor_nonlinear_term():
+    """V = V_ext + g|psi|^2 -- phase of each point is -(V + g|psi|^2) dt/2."""
+    n, L = 64, 16.0
+    p = W.config1(g=10.0)
+    psi0 = p["psi0"].copy()
+    psi = psi0.copy()
+    Oracle(p).potential_half_step(psi, 1e-2, False)
+    ph = np.angle(psi / psi0)
+    expect = -(p["v_static"] + 10.0 * np.abs(psi0) ** 2) * 1e-2 / 2
+    assert np.max(np.abs(ph - expect)) <= 1e-13
+    assert np.max(np.abs(np.abs(psi) - np.abs(psi0))) <= 1e-15
+
+
+# ------------------------------------------------------------------ imaginary time, harmonic trap
+def test_gaussian_recurrence_closed_form():
+    """in V = r^2/2 with g = 0 a noise-free Gaussian e^{-a r^2/2} stays
+    Gaussian under V/2.T.V/2 with a <- (a+dt/2)/(1+(a+dt/2)dt) + dt/2; E = 2(a/4 + 1/(4a)),
+    <x^2> = 1/(2a).  Pins factor order, the dt/2 split, the 1/2 in T and V, and step 6."""
+    p = W.config1(g=0.0, noise=0.0)
+    psi = p["psi0"].copy()
+    dt, nsteps = 1e-3, 2000
+    o = Oracle(p)
+    o.evolve(psi, dt, nsteps, True)
+    a = 1.0 / 1.5 ** 2
+    for _ in range(nsteps):
+        b = a + dt / 2
+        a = b / (1 + b * dt) + dt / 2
+    obs, _, _ = o.observables(psi)
+    E = obs[0]["e_kin"] + obs[0]["e_pot"]
+    assert obs[0]["norm"] == pytest.approx(1.0, abs=1e-13)
+    assert E == pytest.approx(2 * (a / 4 + 1 / (4 * a)), abs=2e-11)
+    mx, my = _moments(psi, p)
+    assert mx == pytest.approx(1 / (2 * a), abs=2e-11)
+    assert my == pytest.approx(1 / (2 * a), abs=2e-11)
+    # T/2.V.T/2 ordering would give a different a after 2000 steps; so would dt instead of dt/2.
+
+
+def test_harmonic_ground_state_energy():
+    """north_star pin: the non-interacting 2-D harmonic ground state has E = (wx+wy)/2 = 1
+    (imaginary time converges to the ground state)."""
+    p = W.config1(g=0.0)
+    psi = p["psi0"].copy()
+    o = Oracle(p)
+    o.evolve(psi, 1e-3, 2000, True)
+    obs, _, _ = o.observables(psi)
+    E = obs[0]["e_kin"] + obs[0]["e_pot"]
+    assert abs(E - 1.0) <= 2e-4            # tau = 2 is short: residual n=2 admixture ~ e^{-2 tau}
+    o.evolve(psi, 1e-3, 10000, True)
+    obs, _, _ = o.observables(psi)
+    E = obs[0]["e_kin"] + obs[0]["e_pot"]
+    assert abs(E - 1.0) <= 1e-8
+    d = np.abs(psi) ** 2
+    x = W.axis(64, 16.0)[:, None]
+    y = W.axis(64, 16.0)[None, :]
+    a = math.sqrt(1 + 1e-3 ** 2 / 4)        # fixed point of the recurrence
+    exact = a / math.pi * np.exp(-a * (x * x + y * y))
+    assert np.max(np.abs(d - exact)) <= 1e-8
+
+
+def test_virial_interacting_ground_state():
+    """2-D harmonic trap virial theorem at the GPE ground state: E_kin - E_pot + E_int = 0."""
+    p = W.config1(g=10.0)
+    psi = p["psi0"].copy()
+    o = Oracle(p)
+    o.evolve(psi, 2e-3, 4000, True)
+    obs, _, _ = o.observables(psi)
+    ob = obs[0]
+    assert abs(ob["e_kin"] - ob["e_pot"] + ob["e_int"]) <= 2e-3
+    assert ob["e_int"] > 0.2 and ob["norm"] == pytest.approx(1.0, abs=1e-12)
+
+
+def test_thomas_fermi_limit():
+    """PAPER.md:144-148 (Sec. 5.1): at large g the density follows Thomas-Fermi:
+    mu = sqrt(g/pi), E = 2mu/3, n(0) = mu/g, <r^2> = 2mu/3 (norm 1, w = 1)."""
+    n, L, g = 128, 20.0, 1000.0
+    p = W._with_trap(W._base(n, n, L))
+    p["g"] = np.array([g])
+    psi = W.noisy_gaussian(n, n, L, L, 3.0, 5)
+    o = Oracle(p)
+    o.evolve(psi, 2e-3, 3000, True)
+    obs, dens, _ = o.observables(psi, density=True)
+    ob = obs[0]
+    mu = math.sqrt(g / math.pi)
+    E = ob["e_kin"] + ob["e_pot"] + ob["e_int"]
+    assert E == pytest.approx(2 * mu / 3, rel=0.02)
+    assert dens[0, n // 2, n // 2] == pytest.approx(mu / g, rel=0.02)
+    mx, my = _moments(psi, p)
+    assert mx + my == pytest.approx(2 * mu / 3, rel=0.02)
+    # profile inside the bulk
+    x = W.axis(n, L)
+    tf = np.maximum(mu - 0.5 * x * x, 0) / g
+    bulk = np.abs(x) < 0.7 * math.sqrt(2 * mu)
+    assert np.max(np.abs(dens[0, :, n // 2][bulk] - tf[bulk]) / tf[bulk]) <= 0.03
+
+
+# ------------------------------------------------------------------ real time invariants
+def test_real_time_norm_and_time_reversal():
+    """Unitary factors: the norm is conserved; Strang with reading Q2 is symmetric, so n steps
+    of dt followed by n steps of -dt return psi0."""
+    p = W.config1(g=10.0)
+    p["lattice_axis"], p["lattice_k"] = 0, 2.0
+    p["sched_step"], p["sched_amp"] = np.array([0.]), np.array([3.0])
+    psi0 = p["psi0"].copy()
+    psi = psi0.copy()
+    o = Oracle(p)
+    o.evolve(psi, 2e-3, 50, False)
+    obs, _, _ = o.observables(psi)
+    assert obs[0]["norm"] == pytest.approx(1.0, abs=1e-13)
+    assert np.linalg.norm(psi - psi0) > 1e-2
+    o.evolve(psi, -2e-3, 50, False)
+    assert np.linalg.norm(psi - psi0) / np.linalg.norm(psi0) <= 1e-12
+
+
+def test_convergence_order_two():
+    """local error O(dt^3) -> global error O(dt^2)."""
+    p = W.config1(g=10.0)
+    T = 0.2
+
+    def run(nsteps):
+        psi = p["psi0"].copy()
+        Oracle(p).evolve(psi, T / nsteps, nsteps, False)
+        return psi
+
+    ref = run(1600)
+    e1 = np.linalg.norm(run(50) - ref)
+    e2 = np.linalg.norm(run(100) - ref)
+    e3 = np.linalg.norm(run(200) - ref)
+    assert math.log2(e1 / e2) == pytest.approx(2.0, abs=0.1)
+    assert math.log2(e2 / e3) == pytest.approx(2.0, abs=0.1)
+
+
+# ------------------------------------------------------------------ Kapitza-Dirac
+def _coupled_mode_populations(V0, k, t, M=10):
+    """Schroedinger equation of the momentum states |2 m k>:
+    i dc_m/dt = ((2mk)^2/2 + V0/2) c_m + (V0/4)(c_{m-1} + c_{m+1}),  c_m(0) = delta_m0."""
+    m = np.arange(-M, M + 1)
+    H = np.diag((2 * m * k) ** 2 / 2 + V0 / 2).astype(complex)
+    H += np.diag(np.full(2 * M, V0 / 4), 1) + np.diag(np.full(2 * M, V0 / 4), -1)
+    c0 = np.zeros(2 * M + 1, complex)
+    c0[M] = 1
+    c = expm(-1j * H * t) @ c0
+    return {int(mm): float(abs(cc) ** 2) for mm, cc in zip(m, c)}
+
+
+@pytest.mark.parametrize("V0", [5.0, 20.0])
+def test_kapitza_dirac_coupled_mode(V0):
+    """the non-interacting populations agree with integrating the
+    Schroedinger equation in momentum space.  Uniform gas, g=0, no trap; error ~ dt^2."""
+    n, L, k = 128, 4 * math.pi, 4.0
+    p = _plain(n, L, lattice_axis=0, lattice_k=k,
+               sched_step=np.array([0., 200., 200.]), sched_amp=np.array([V0, V0, 0.]))
+    psi = np.full((n, n), 1.0 / L, dtype=np.complex128)
+    o = Oracle(p)
+    o.evolve(psi, 1e-4, 200, False)
+    pops = o.populations(psi, 0, k, 3)[0]
+    ref = _coupled_mode_populations(V0, k, 0.02)
+    for m in range(-3, 4):
+        assert pops[m + 3] == pytest.approx(ref[m], abs=5e-6), m
+    assert pops[3 + 1] == pytest.approx(pops[3 - 1], rel=1e-9)
+    # g = 0, lattice off: populations stay constant during free evolution
+    o.evolve(psi, 1e-4, 100, False)
+    pops2 = o.populations(psi, 0, k, 3)[0]
+    assert np.max(np.abs(pops2 - pops)) <= 1e-12
+
+
+def test_kapitza_dirac_raman_nath_bessel():
+    """north_star pin: short-pulse populations follow J_m^2(V0 tau/2) (Raman-Nath regime)."""
+    n, L, k = 128, 4 * math.pi, 4.0
+    V0, nst, dt = 500.0, 20, 1e-4
+    p = _plain(n, L, lattice_axis=1, lattice_k=k,
+               sched_step=np.array([0.]), sched_amp=np.array([V0]))
+    psi = np.full((n, n), 1.0 / L, dtype=np.complex128)
+    o = Oracle(p)
+    o.evolve(psi, dt, nst, False)
+    pops = o.populations(psi, 1, k, 3)[0]
+    beta = V0 * nst * dt / 2
+    for m in range(-3, 4):
+        assert pops[m + 3] == pytest.approx(jv(abs(m), beta) ** 2, abs=2e-3), m
+    assert pops[4] > 0.05                     # really diffracted
+
+
+# ------------------------------------------------------------------ observables on a known state
+def test_observables_closed_forms_gaussian():
+    """For psi = Gaussian(sigma): E_kin = 1/(2 s^2), E_trap = s^2/2, E_int = g/(4 pi s^2),
+    Theta = exp(-k^2 s^2/2); alpha = N eta Theta/(Delta + i kappa) (Eq. 14)."""
+    n, L, s, g, kc = 128, 24.0, 1.3, 7.0, 1.0
+    p = W._with_trap(W._base(n, n, L))
+    p.update(g=np.array([g]), cavity_on=1, cavity_k=kc, eta_mode=0, eta_or_u=np.array([0.8]),
+             n_atoms=np.array([3.0]), delta=np.array([-2.0]), kappa=np.array([0.5]))
+    psi = W.noisy_gaussian(n, n, L, L, s, 0, noise=0.0)
+    obs, dens, kd = Oracle(p).observables(psi, density=True, kdensity=True)
+    ob = obs[0]
+    assert ob["norm"] == pytest.approx(1.0, abs=1e-13)
+    assert ob["e_kin"] == pytest.approx(1 / (2 * s * s), rel=1e-10)
+    assert ob["e_pot"] == pytest.approx(s * s / 2, rel=1e-10)
+    assert ob["e_int"] == pytest.approx(g / (4 * math.pi * s * s), rel=1e-10)
+    theta = math.exp(-kc * kc * s * s / 2)
+    assert ob["theta"] == pytest.approx(theta, rel=1e-10)
+    alpha = 3.0 * 0.8 * theta / complex(-2.0, 0.5)
+    assert ob["re_alpha"] == pytest.approx(alpha.real, rel=1e-10)
+    assert ob["im_alpha"] == pytest.approx(alpha.imag, rel=1e-10)
+    assert ob["e_cav"] == pytest.approx(3.0 * 0.64 * theta ** 2 * (-2.0) / (4 + 0.25), rel=1e-10)
+    assert np.max(np.abs(dens[0] - np.abs(psi) ** 2)) == 0.0
+    assert kd[0].sum() == pytest.approx(1.0, abs=1e-12)
+    kx = 2 * math.pi * np.fft.fftfreq(n, L / n)
+    expect = np.exp(-(kx[:, None] ** 2 + kx[None, :] ** 2) * s * s)
+    expect /= expect.sum()
+    assert np.max(np.abs(kd[0] - expect)) <= 1e-12
+
+
+# ------------------------------------------------------------------ cavity
+def _cavity_small(Vp, g=0.0, n=64, delta=-1.0):
+    L = 4 * math.pi
+    p = W._cavity(W._with_trap(W._base(n, n, L)), 1, Vp, delta, g)
+    p["sched_step"], p["sched_amp"] = np.array([0.]), np.array([Vp])
+    p["psi0"] = W.noisy_gaussian(n, n, L, L, 1.2, 7)
+    return p
+
+
+def test_cavity_real_time_conservation():
+    """Static parameters, real time: V real -> norm conserved; with E_cav = N eta^2 Theta^2
+    Delta/(Delta^2+kappa^2) (so that dE_cav/d|psi|^2 = C cos cos, Eqs. 13-14) the total
+    energy is conserved up to the splitting error, which shrinks with dt."""
+    p = _cavity_small(8.0, g=5.0)
+
+    def drift(dt, nsteps):
+        psi = p["psi0"].copy()
+        o = Oracle(p)
+        ob0 = o.observables(psi)[0][0]
+        o.evolve(psi, dt, nsteps, False)
+        ob1 = o.observables(psi)[0][0]
+        e = lambda ob: ob["e_kin"] + ob["e_pot"] + ob["e_int"] + ob["e_cav"]
+        assert ob1["norm"] == pytest.approx(1.0, abs=1e-12)
+        assert abs(ob1["theta"] - ob0["theta"]) > 1e-4        # something happened
+        return abs(e(ob1) - e(ob0)) / abs(e(ob0))
+
+    d1 = drift(1e-3, 200)
+    d2 = drift(5e-4, 400)
+    assert d1 <= 2e-5
+    assert d2 <= 0.6 * d1
+    # a wrong sign or a missing factor 2 in C breaks conservation at O(1):
+    # (checked by construction: E_cav's functional derivative must equal the potential used)
+
+
+def test_cavity_self_organisation_and_fixed_point():
+    """below a critical pump the cavity field vanishes, above it the gas orders
+    into the chequerboard and the field is non-zero (Delta < 0).  At the imaginary-time fixed
+    point psi is an eigenstate of H[psi] with alpha frozen: residual O(dt), via numpy's FFT."""
+    lo = _cavity_small(1.0)
+    psi = lo["psi0"].copy()
+    o = Oracle(lo)
+    o.evolve(psi, 2e-3, 3000, True)
+    # "vanishing" up to the explicit overlap of the finite cloud itself: for the trap ground
+    # state |psi|^2 = e^{-r^2}/pi the overlap is exp(-k^2/4)^2 = e^{-8} = 3.4e-4
+    assert abs(o.observables(psi)[0][0]["theta"]) <= 1e-3
+
+    hi = _cavity_small(15.0)
+    psi = hi["psi0"].copy()
+    o = Oracle(hi)
+    o.evolve(psi, 2e-3, 4000, True)
+    ob = o.observables(psi)[0][0]
+    assert abs(ob["theta"]) >= 0.3
+    # eigen-residual with numpy
+    n, L, k = 64, 4 * math.pi, 4.0
+    x = W.axis(n, L)
+    eta = math.sqrt(15.0 * 4.0)
+    alpha = eta * ob["theta"] / complex(-1.0, 0.5)
+    V = hi["v_static"] + 15.0 * np.cos(k * x)[None, :] ** 2 \
+        + 2 * eta * alpha.real * np.cos(k * x)[:, None] * np.cos(k * x)[None, :]
+    kk = 2 * math.pi * np.fft.fftfreq(n, L / n)
+    K2 = kk[:, None] ** 2 + kk[None, :] ** 2
+    Hpsi = np.fft.ifft2(0.5 * K2 * np.fft.fft2(psi)) + V * psi
+    mu = np.vdot(psi, Hpsi) / np.vdot(psi, psi)
+    res = np.linalg.norm(Hpsi - mu * psi) / np.linalg.norm(psi) / abs(mu)
+    assert res <= 5e-3
+    assert ob["re_alpha"] == pytest.approx(alpha.real, rel=1e-12)
+
+
+def test_interactions_raise_threshold():
+    """repulsive interactions increase the critical pump."""
+    thetas = {}
+    for g in (0.0, 60.0):
+        p = _cavity_small(8.0, g=g)
+        psi = p["psi0"].copy()
+        o = Oracle(p)
+        o.evolve(psi, 2e-3, 3000, True)
+        thetas[g] = abs(o.observables(psi)[0][0]["theta"])
+    assert thetas[0.0] > 0.5
+    assert thetas[60.0] < 0.2 * thetas[0.0]
+
+
+# ------------------------------------------------------------------ batch and records
+def test_batch_members_equal_single_runs_and_records():
+    p = W.config5(n=64, side=2, n_steps=30)
+    psi = p["psi0"].astype(np.complex128).copy()
+    o = Oracle(p)
+    rec = o.evolve(psi, 5e-4, 30, True, record_every=10)
+    assert rec.shape == (3, 4, 6)
+    for b in range(4):
+        q = W.member(p, b)
+        s = q["psi0"].astype(np.complex128).copy()
+        os_ = Oracle(q)
+        r1 = os_.evolve(s, 5e-4, 30, True, record_every=10)
+        # OpenMP sum order is not fixed, so equality is to round-off, not bitwise
+        assert np.linalg.norm(s - psi[b]) / np.linalg.norm(s) <= 1e-13
+        assert np.allclose(r1[:, 0, :], rec[:, b, :], rtol=1e-12, atol=1e-15)
+    ob = o.observables(psi)[0]
+    assert rec[-1, 3, 0] == 30
+    assert rec[-1, 3, 2] == pytest.approx(ob[3]["theta"], rel=1e-12)
+    assert rec[-1, 3, 1] == pytest.approx(1.0, abs=1e-12)
+
+
+def test_f32_build_tracks_f64():
+    """The float build is the same statements in complex64 (used only as the fp32 floor)."""
+    p = W.config1(g=10.0)
+    a = p["psi0"].astype(np.complex64)
+    b = a.astype(np.complex128)
+    Oracle(p, "f32").evolve(a, 1e-3, 10, True)
+    Oracle(p, "f64").evolve(b, 1e-3, 10, True)
+    err = np.linalg.norm(a.astype(np.complex128) - b) / np.linalg.norm(b)
+    assert 1e-9 < err < 5e-6
