@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused split-step hot path on B200, one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+Workload (config.workload): BASELINE.json configs[3] -- the 2048 x 2048 complex64 real-time run
+with the self-consistent cavity potential, pump ramp 0 -> 20 over 10000 steps, dt = 1e-4,
+g = 200, order parameter recorded every 100 steps -- the configuration the metric's target is
+quoted on ("at 2048 x 2048 complex64").  One bench "step" is one gpe_evolve call of `--inner`
+(default 200) split-step steps of the whole hot path (all SURVEY.md 8(a) rows: pass A, pass B,
+pass C with the fused norm/overlap reduction and the on-device scalar update, records).
+metric = split-step grid-point updates per second = nx*ny*inner*K*N / seconds.
+
+Single grid does not shard (replicas only): with --gpus N every rank
+evolves its own replica, no data-path collective, scaling "weak".
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the same config and metric,
+one split-step of the 2048^2 grid per bench step, on rank 0's host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "split-step grid-point updates/sec"
+UNIT = "updates/s"
+WORKLOAD = ("config4: 2048x2048 complex64, real time dt=1e-4, V_trap + V_p cos^2(4y) + "
+            "2 eta Re(alpha) cos(4x)cos(4y), pump ramp 0->20 over 10000 steps, g=200, "
+            "Delta=-1, kappa=0.5, u=4, record every 100")
+
+
+def _measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            d = json.load(open(path))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            try:
+                sm.append(float(r[1]))
+                mx = float(r[2])
+                for n, v in zip(names, r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def aggregate(local_ms: float, local_units: float, world: int, reduce_max=None, reduce_sum=None):
+    """Whole-job value from per-rank numbers: time = max over ranks, units = sum over ranks.
+    reduce_max / reduce_sum are the collectives (identity at world == 1); kept as a function so
+    the N > 1 logic is testable under gloo on CPU (tests/test_bench_host.py)."""
+    t = reduce_max(local_ms) if reduce_max else local_ms
+    u = reduce_sum(local_units) if reduce_sum else local_units
+    return u / (t * 1e-3), t
+
+
+def cpu_baseline(nx: int, budget_s: float = 15.0):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the bench
+    workload: whole split-steps of the same 2048^2 config-4 grid (complex128)."""
+    import workloads as W
+    from oracle.gpe_oracle import Oracle
+    p = W.config4(n=nx)
+    psi = p["psi0"].copy()
+    o = Oracle(p)
+    t0 = time.perf_counter()
+    o.evolve(psi, 1e-4, 1, False)
+    t1 = time.perf_counter() - t0
+    n = max(2, min(40, int(budget_s / max(t1, 1e-3))))
+    t0 = time.perf_counter()
+    o.evolve(psi, 1e-4, n, False)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return {"value": nx * nx * n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n} whole split-steps of the {nx}x{nx} config-4 grid in complex128 "
+                      f"({dt:.1f} s, OpenMP over rows/columns/points)"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import workloads as W
+    from oracle.gpe_oracle import Oracle
+    nx = args.n
+    p = W.config4(n=nx)
+    psi = p["psi0"].copy()
+    o = Oracle(p)
+    for _ in range(args.warmup):
+        o.evolve(psi, 1e-4, 1, False)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.evolve(psi, 1e-4, 1, False, record_every=100)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    val = nx * nx * args.steps / dt
+    sample = f"1 split-step of the {nx}x{nx} config-4 grid per bench step, complex128 oracle"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": WORKLOAD, "nx": nx, "ny": nx, "inner_steps": 1},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import paper_2404_14401_b200 as G
+    import workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    nx = args.n
+    inner, K, Wm = args.inner, args.steps, args.warmup
+    p = W.config4(n=nx)
+    stream = torch.cuda.Stream()
+    plan = G.Plan(nx, nx, p["Lx"], p["Ly"], "c64", 1, stream=stream.cuda_stream)
+    with torch.cuda.stream(stream):
+        plan.set_potential(p)                      # separable trap: no 2-D potential array
+        psi0_host = torch.from_numpy(p["psi0"].astype(np.complex64)).pin_memory()
+        psi = psi0_host.to("cuda", non_blocking=True)
+        flush = torch.empty(384 * 1024 * 1024, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+    stream.synchronize()
+    P = nx * nx
+
+    def one_step(record=True):
+        return plan.evolve(psi, 1e-4, inner, "real", record_every=100 if record else 0)
+
+    # ---- device-resident timing --------------------------------------------------------
+    with torch.cuda.stream(stream):
+        for _ in range(Wm):
+            flush.fill_(1)
+            one_step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = []
+    with torch.cuda.stream(stream):
+        for _ in range(K):
+            flush.fill_(1)                         # L2 flushed between timed evolve calls
+            e0 = torch.cuda.Event(enable_timing=True)
+            e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            one_step()
+            e1.record(stream)
+            evs.append((e0, e1))
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    local_ms = sum(a.elapsed_time(b) for a, b in evs)
+    launches = K * (1 + 3 * inner)
+
+    def rmax(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def rsum(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    value, tot_ms = aggregate(local_ms, float(P) * inner * K, world, rmax, rsum)
+
+    # ---- end to end: host buffers, copies inside the timed region -----------------------
+    h_out = torch.empty_like(psi0_host).pin_memory()
+    nrec = max(1, inner // 100)
+    h_rec = torch.empty((nrec, 1, G.GPE_NREC), dtype=torch.float64).pin_memory()
+    plan.step = 0
+    barrier()
+    t0 = time.perf_counter()
+    with torch.cuda.stream(stream):
+        for _ in range(K):
+            psi.copy_(psi0_host, non_blocking=True)
+            plan.step = 0
+            rec = one_step()
+            h_out.copy_(psi, non_blocking=True)
+            h_rec.copy_(rec[:nrec], non_blocking=True)
+            stream.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    barrier()
+    e2e_value, _ = aggregate(e2e_ms, float(P) * inner * K, world, rmax, rsum)
+    h2d = psi0_host.numel() * psi0_host.element_size()
+    d2h = h2d + h_rec.numel() * 8
+
+    # ---- per-pass device times (CUDA events inside the library, on the plan's stream) ----
+    roof = None
+    extra = {}
+    if rank == 0:
+        peak, how = _measured_peaks()
+        with torch.cuda.stream(stream):
+            flush.fill_(1)
+        ms = G.gpe_profile_passes(plan.plan, psi.data_ptr(), 1e-4, 300, G.GPE_REAL_TIME)
+        names = ("pass A k_row_fwd (potential half-step + FFT_y)",
+                 "pass B k_col (FFT_x + kinetic + IFFT_x)",
+                 "pass C k_row_inv (IFFT_y + potential half-step + reductions)")
+        dom = max(range(3), key=lambda i: ms[i])
+        alg = 16.0 * P                              # each pass reads 8 B/pt and writes 8 B/pt (c64)
+        ach = alg / (ms[dom] * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": names[dom], "achieved": ach, "peak": peak, "unit": "GB/s",
+                "frac": ach / peak, "traffic": None, "peak_source": how,
+                "algorithmic_bytes_per_launch": alg, "launch_ms": ms[dom]}
+        step_ms = tot_ms / (K * inner)
+        step_alg = 48.0 * P
+        extra = {"pass_ms": {"A": ms[0], "B": ms[1], "C": ms[2]},
+                 "roofline_step": {"bound": "hbm", "achieved": step_alg / (step_ms * 1e-3) / 1e9,
+                                   "peak": peak, "unit": "GB/s",
+                                   "frac": step_alg / (step_ms * 1e-3) / 1e9 / peak,
+                                   "algorithmic_bytes_per_step": step_alg, "us_per_split_step": step_ms * 1e3}}
+    plan.close()
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(nx)
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+                "ms_per_step": tot_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": {"workload": WORKLOAD, "nx": nx, "ny": nx, "batch_per_gpu": 1, "inner_steps": inner,
+                           "parallelism": f"replicas x{world} (single grid does not shard)",
+                           "l2": "L2 flushed (384 MB write) between timed evolve calls; inside a call the "
+                                 "32 MiB wavefunction is re-read every pass, as the iteration requires"},
+                "clocks": clocks,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
+        line.update(extra)
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--inner", type=int, default=200, help="split-step steps per bench step")
+    ap.add_argument("--n", type=int, default=2048, help="grid side (the metric is quoted at 2048)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = max(args.warmup, 3) if os.environ.get("GPE_BENCH_STRICT", "1") == "1" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,190 @@
+/*
+ * gpe.h -- C ABI of libgpe: symmetric split-step Fourier propagation of the 2-D
+ * Gross-Pitaevskii equation on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes is the method of arXiv 2404.14401 (TorchGPE), cited below as
+ * PAPER.md:<line> (the copy under /root/reference), in the readings listed in DESIGN.md:
+ *
+ *   i d(psi)/dt = [ -1/2 nabla^2 + V_ext(r,t,psi) + g |psi|^2 ] psi          (Eq. 1)
+ *
+ * hbar = m = 1 (oscillator units).  One step of size dt is the Strang
+ * splitting V/2 . T . V/2 (Eqs. 2-4; order of factors: DESIGN.md reading Q1):
+ *   psi <- psi * exp(-s (V_n + g|psi|^2) dt/2)        s = i (real time), s = 1 (imaginary time)
+ *   psi <- IFFT2[ exp(-s (kx^2+ky^2) dt/2) * FFT2[psi] ]
+ *   psi <- psi * exp(-s (V_n + g|psi|^2) dt/2)        |psi|^2 recomputed
+ *   imaginary time: psi <- psi / sqrt(sum |psi|^2 dx dy) after every step
+ * with V_n(x,y) = V_static(x,y) + A_n cos^2(k_l r_axis) + C_n cos(k_c x) cos(k_c y)
+ * (PAPER.md:154 Eq. 9, :175-179 Eqs. 11, 13), A_n a piecewise-linear schedule sampled at the
+ * start of step n, and the self-consistent cavity coefficient recomputed once per step from
+ * the current density (Eq. 14):
+ *   Theta_n = sum cos(k_c x) cos(k_c y) |psi_n|^2 dx dy
+ *   alpha_n = N_at eta_n Theta_n / (Delta + i kappa),  C_n = 2 eta_n Re(alpha_n),
+ *   eta_n = eta (eta_mode 0) or sqrt(|A_n| u) (eta_mode 1; eta = sqrt(V0 U0) in Eq. 13).
+ * V_c (Eq. 12) and the dispersive shift (Eq. 15) are not applied (reading Q6).
+ *
+ * Grid: x_i = -Lx/2 + i Lx/nx, i = 0..nx-1 (periodic), likewise y_j; psi is stored
+ * [batch][nx][ny], y fastest, interleaved (re, im); integrals are sums times dx dy.
+ * FFT convention: forward unnormalised with exp(-i(kx x + ky y)), inverse with 1/(nx ny).
+ *
+ * All pointers named *_dev / marked DEVICE are CUDA device pointers on the current device;
+ * all others are host pointers.  Nothing here takes or returns a torch / C++ type.
+ * Every call returns a gpe_status and never throws; gpe_last_error() gives the text of the
+ * last failure on that plan.  The library has no CPU fallback: without a CUDA device every
+ * compute call returns GPE_ECUDA.
+ */
+#ifndef GPE_H
+#define GPE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define GPE_API __attribute__((visibility("default")))
+#else
+#define GPE_API
+#endif
+
+typedef struct gpe_plan gpe_plan; /* opaque; owns tables, workspace and the device scalar block */
+
+typedef enum { GPE_C64 = 0, GPE_C128 = 1 } gpe_dtype;     /* complex64 / complex128 */
+typedef enum { GPE_REAL_TIME = 0, GPE_IMAG_TIME = 1 } gpe_mode;
+typedef enum {
+    GPE_OK = 0,
+    GPE_EINVAL = 1,       /* bad argument (NULL, non-finite, misaligned, wrong size) */
+    GPE_EUNSUPPORTED = 2, /* nx or ny not a power of two in [64, 2048] */
+    GPE_ENOMEM = 3,       /* host or device allocation failed */
+    GPE_ECUDA = 4,        /* a CUDA runtime call failed (text in gpe_last_error) */
+    GPE_ESTATE = 5,       /* call order: gpe_evolve / gpe_observables before gpe_set_potential */
+    GPE_ENONFINITE = 6    /* the device saw a non-finite norm during an earlier gpe_evolve */
+} gpe_status;
+
+#define GPE_NREC 6 /* doubles per record: {step, norm, theta, re_alpha, im_alpha, A} */
+
+/*
+ * gpe_plan_create -- the discretised problem of Eq. 1: an nx x ny periodic grid
+ * over the box [-Lx/2, Lx/2) x [-Ly/2, Ly/2), `batch` independent wavefunctions (parameter
+ * sweeps, north_star (4)).  nx, ny powers of two in [64, 2048] (the paper benchmarks powers of
+ * two), else GPE_EUNSUPPORTED; Lx, Ly > 0 and finite, batch >= 1, else GPE_EINVAL.
+ * Allocates the twiddle / wavenumber tables and the per-member device scalars on the current
+ * device.  *out is set only on GPE_OK and is released with gpe_plan_destroy.
+ */
+GPE_API gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly, gpe_dtype dtype,
+                           int batch);
+
+/* All work of the plan is enqueued on this cudaStream_t (default: the legacy stream 0). */
+GPE_API gpe_status gpe_plan_set_stream(gpe_plan *p, void *cuda_stream);
+
+/* Frees everything the plan owns (synchronises its stream first).  NULL is a no-op. */
+GPE_API gpe_status gpe_plan_destroy(gpe_plan *p);
+
+/*
+ * gpe_potential_desc -- V_ext of Eq. 1 in the fixed form used by the paper's examples
+ * (PAPER.md:154 Eq. 9; :170-186 Eqs. 10, 11, 13, 14) plus the contact coupling g.
+ * "real" below is float for GPE_C64 and double for GPE_C128.
+ */
+typedef struct {
+    const void *v_static;     /* DEVICE real [nx][ny] (or [batch][nx][ny]); NULL = none          */
+    int v_static_batched;     /* 0: one array shared by all members; 1: one per member           */
+    const double *vx, *vy;    /* HOST, optional separable static part vx[i] + vy[j]; NULL = none
+                                 (added to v_static if both are given)                           */
+    const double *g;          /* HOST [batch] contact coupling, norm-1 convention; NULL = 0      */
+    int lattice_axis;         /* -1 none; 0: A cos^2(k_l x); 1: A cos^2(k_l y)   (Eqs. 9, 11)    */
+    double lattice_k;
+    int sched_len;            /* knots of the piecewise-linear amplitude A(step); 0 = A == 0     */
+    const double *sched_step; /* HOST [sched_len], non-decreasing, in units of steps. A_n is
+                                 interpolated on the segment starting at the LAST knot with
+                                 step <= n; constant before the first and after the last knot   */
+    const double *sched_amp;  /* HOST [sched_len], or [batch][sched_len] if sched_batched        */
+    int sched_batched;
+    int cavity_on;            /* adds C_n cos(k_c x) cos(k_c y)                  (Eqs. 13, 14)   */
+    double cavity_k;
+    int eta_mode;             /* 0: eta given; 1: eta_n = sqrt(|A_n| u)                          */
+    const double *eta_or_u;   /* HOST [batch] (required if cavity_on)                            */
+    const double *n_atoms;    /* HOST [batch] N_at of Eq. 14; NULL = 1                           */
+    const double *delta;      /* HOST [batch] cavity detuning Delta (required if cavity_on)      */
+    const double *kappa;      /* HOST [batch] cavity decay kappa  (required if cavity_on)        */
+} gpe_potential_desc;
+
+/*
+ * gpe_set_potential -- copies everything it needs (the caller may free all arrays on return;
+ * the device array v_static is copied device-to-device on the plan's stream).  May be called
+ * again at any time between gpe_evolve calls.  GPE_EINVAL on inconsistent fields.
+ */
+GPE_API gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d);
+
+/*
+ * gpe_evolve -- n_steps split-step steps (see the top of this file) in place on
+ * psi: DEVICE [batch][nx][ny] complex of the plan's dtype, 16-byte aligned, caller-owned.
+ * dt: time step; must be finite and non-zero, and > 0 for GPE_IMAG_TIME.
+ * The plan keeps a step counter n (time origin of the schedule, A_n = A(n)); it starts at 0,
+ * advances by n_steps per call and is read / set with gpe_get_step / gpe_set_step.
+ * record_every > 0: after every step whose new counter value is a multiple of record_every,
+ * GPE_NREC doubles per member are written to
+ * records: DEVICE [n_rec][batch][GPE_NREC] = {step, norm, Theta, Re alpha, Im alpha, A}, evaluated on
+ * the wavefunction after that step (after the renormalisation in imaginary time), with
+ * n_rec = floor((n0+n_steps)/record_every) - floor(n0/record_every).  record_every = 0: none.
+ * The call only ENQUEUES work on the plan's stream: no host synchronisation, no host round
+ * trip of the per-step scalars (norm, Theta, alpha live in device memory; north_star (3)).
+ * GPE_ESTATE before gpe_set_potential; GPE_EINVAL on bad arguments; GPE_ECUDA on launch errors.
+ */
+GPE_API gpe_status gpe_evolve(gpe_plan *p, void *psi_dev, double dt, long n_steps, gpe_mode mode,
+                      long record_every, double *records_dev);
+
+/*
+ * gpe_observables -- norm, energies and cavity quantities of psi:
+ *   norm  = sum |psi|^2 dx dy
+ *   e_kin = 1/2 sum (kx^2+ky^2)|psi^|^2 / sum |psi^|^2 * norm
+ *   e_pot = sum (V_static + A_n cos^2) |psi|^2 dx dy          (n = the plan's step counter)
+ *   e_int = g/2 sum |psi|^4 dx dy
+ *   e_cav = N_at eta_n^2 Theta^2 Delta / (Delta^2 + kappa^2)  (its functional derivative is
+ *           the interference potential of Eq. 13)
+ *   theta, re_alpha, im_alpha as in Eq. 14.
+ * out_host: HOST [batch].  density_dev (DEVICE real [batch][nx][ny], or NULL): |psi|^2.
+ * kdensity_dev (DEVICE real [batch][nx][ny], or NULL): |psi^|^2 / sum |psi^|^2 in FFT order
+ * ("directly from the wave-function amplitude in reciprocal space").
+ * Synchronises the plan's stream (it returns host values).  psi is not modified.
+ * Returns GPE_ENONFINITE if an earlier gpe_evolve on this plan produced a non-finite norm.
+ */
+typedef struct {
+    double norm, e_kin, e_pot, e_int, e_cav, theta, re_alpha, im_alpha;
+} gpe_obs;
+GPE_API gpe_status gpe_observables(gpe_plan *p, const void *psi_dev, gpe_obs *out_host, void *density_dev,
+                           void *kdensity_dev);
+
+/*
+ * gpe_populations -- momentum-order populations after a lattice pulse:
+ *   out_host[b][m + m_max] = sum over |k_axis - 2 m k_l| < k_l (all k on the other axis)
+ *                            of |psi^|^2 / sum |psi^|^2,   m = -m_max .. m_max
+ * axis: 0 (x) or 1 (y).  out_host: HOST [batch][2 m_max + 1].  Synchronises the stream.
+ */
+GPE_API gpe_status gpe_populations(gpe_plan *p, const void *psi_dev, int axis, double k_l, int m_max,
+                           double *out_host);
+
+/*
+ * gpe_profile_passes -- measurement aid for the roofline report: runs n_steps
+ * steps exactly as gpe_evolve does (psi evolves, the step counter advances, no records), with
+ * CUDA events on the plan's stream around ONE of the three fused passes per step (round-robin),
+ * and returns the mean device time per launch in milliseconds:
+ * ms_out_host[0] = pass A (potential half-step + FFT along y), [1] = pass B (FFT along x, kinetic
+ * factor, inverse FFT along x), [2] = pass C (inverse FFT along y, potential half-step, fused
+ * norm / overlap reduction and scalar update).  3 <= n_steps <= 30000.  Synchronises the stream.
+ */
+GPE_API gpe_status gpe_profile_passes(gpe_plan *p, void *psi_dev, double dt, long n_steps, gpe_mode mode,
+                              double *ms_out_host);
+
+/* Step counter n (schedule time origin); see gpe_evolve. */
+GPE_API gpe_status gpe_get_step(const gpe_plan *p, long *step);
+GPE_API gpe_status gpe_set_step(gpe_plan *p, long step);
+
+/* Text of the last error on this plan ("" if none).  p == NULL: text of the last
+ * gpe_plan_create failure on this thread.  The pointer stays valid until the next call. */
+GPE_API const char *gpe_last_error(const gpe_plan *p);
+
+/* Library build information: "libgpe <version> sm_100a". */
+GPE_API const char *gpe_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GPE_H */

@@ -1,0 +1,740 @@
+// gpe_api.cu -- the C ABI of include/gpe.h: plan, tables, launch sequencing, observables.
+// Host logic only, plus the small non-FFT kernels (prologue reduction, final rescale,
+// observables).  The FFT passes live in gpe_kernels.cuh (one TU per dtype and size).
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/gpe.h"
+#include "gpe_dispatch.h"
+#include "gpe_kernels.cuh"
+
+using namespace gpe;
+
+namespace {
+
+constexpr int kMaxCpm = 1024;   // partial-sum slots per member
+constexpr int kReduceCtas = 128;  // CTAs per member of the prologue reduction
+constexpr double kPi = 3.14159265358979323846;
+
+thread_local std::string g_create_error;
+
+}  // namespace
+
+struct gpe_plan {
+    int nx = 0, ny = 0, batch = 0;
+    double Lx = 0, Ly = 0;
+    gpe_dtype dtype = GPE_C64;
+    cudaStream_t stream = nullptr;
+    bool pot_set = false;
+    long step = 0;
+    std::string err;
+
+    // device tables (typed by dtype)
+    void *tw_x = nullptr, *tw_y = nullptr;
+    void *kin_x = nullptr, *kin_y = nullptr;
+    double kin_dt = 0.0;
+    int kin_mode = -1;
+    void *vx = nullptr, *vy = nullptr, *latx = nullptr, *laty = nullptr, *cavx = nullptr, *cavy = nullptr;
+    void *g = nullptr;
+    void *v2d = nullptr;
+    size_t v2d_elems = 0;
+    int flags = 0;
+
+    // device scalars
+    MemberState *st = nullptr;
+    double2 *partials = nullptr;
+    unsigned int *counters = nullptr;
+    int *nonfinite = nullptr;
+    double *d_sched_step = nullptr, *d_sched_amp = nullptr;
+    double *d_eta = nullptr, *d_natoms = nullptr, *d_delta = nullptr, *d_kappa = nullptr;
+
+    // host copies of the descriptor
+    int lattice_axis = -1, sched_len = 0, sched_batched = 0, cavity_on = 0, eta_mode = 0;
+    double lattice_k = 0, cavity_k = 0;
+    std::vector<double> h_sched_step, h_sched_amp, h_eta, h_natoms, h_delta, h_kappa, h_g;
+
+    // observables workspace
+    void *scratch = nullptr;     // complex [batch][nx][ny]
+    double *obs_dev = nullptr;   // [batch][8]
+    double *pop_dev = nullptr;
+    int pop_len = 0;
+    double *obsA_dev = nullptr;  // [batch]
+};
+
+namespace {
+
+size_t real_bytes(const gpe_plan *p) { return p->dtype == GPE_C64 ? 4 : 8; }
+
+gpe_status fail(gpe_plan *p, gpe_status s, const std::string &msg) {
+    if (p) p->err = msg; else g_create_error = msg;
+    return s;
+}
+gpe_status cuda_fail(gpe_plan *p, cudaError_t e, const char *what) {
+    return fail(p, GPE_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define GPE_CUDA(p, call)                                              \
+    do {                                                               \
+        cudaError_t e__ = (call);                                      \
+        if (e__ != cudaSuccess) return cuda_fail((p), e__, #call);     \
+    } while (0)
+
+bool pow2_in_range(int n) { return n >= 64 && n <= 2048 && (n & (n - 1)) == 0; }
+
+double coord(int i, int n, double L) { return -0.5 * L + (double)i * L / (double)n; }
+double wavenumber(int q, int n, double L) { return 2.0 * kPi * (double)(q < n / 2 ? q : q - n) / L; }
+
+// upload a double host vector as T (float/double) into a device buffer (allocating if needed)
+template <typename T>
+gpe_status upload_real(gpe_plan *p, void **dev, const std::vector<double> &h) {
+    if (!*dev) GPE_CUDA(p, cudaMalloc(dev, sizeof(T) * h.size()));
+    std::vector<T> t(h.size());
+    for (size_t i = 0; i < h.size(); ++i) t[i] = (T)h[i];
+    GPE_CUDA(p, cudaMemcpyAsync(*dev, t.data(), sizeof(T) * t.size(), cudaMemcpyHostToDevice, p->stream));
+    GPE_CUDA(p, cudaStreamSynchronize(p->stream));
+    return GPE_OK;
+}
+template <typename T>
+gpe_status upload_cplx(gpe_plan *p, void **dev, const std::vector<double> &re, const std::vector<double> &im) {
+    if (!*dev) GPE_CUDA(p, cudaMalloc(dev, 2 * sizeof(T) * re.size()));
+    std::vector<T> t(2 * re.size());
+    for (size_t i = 0; i < re.size(); ++i) { t[2 * i] = (T)re[i]; t[2 * i + 1] = (T)im[i]; }
+    GPE_CUDA(p, cudaMemcpyAsync(*dev, t.data(), sizeof(T) * t.size(), cudaMemcpyHostToDevice, p->stream));
+    GPE_CUDA(p, cudaStreamSynchronize(p->stream));
+    return GPE_OK;
+}
+gpe_status upload_f64(gpe_plan *p, double **dev, const std::vector<double> &h) {
+    if (*dev) { cudaFree(*dev); *dev = nullptr; }
+    if (h.empty()) return GPE_OK;
+    GPE_CUDA(p, cudaMalloc((void **)dev, sizeof(double) * h.size()));
+    GPE_CUDA(p, cudaMemcpyAsync(*dev, h.data(), sizeof(double) * h.size(), cudaMemcpyHostToDevice, p->stream));
+    GPE_CUDA(p, cudaStreamSynchronize(p->stream));
+    return GPE_OK;
+}
+
+template <typename T> gpe_status make_twiddles(gpe_plan *p) {
+    for (int ax = 0; ax < 2; ++ax) {
+        int n = ax == 0 ? p->nx : p->ny;
+        std::vector<double> re(n), im(n);
+        for (int m = 0; m < n; ++m) {
+            double ang = -2.0 * kPi * (double)m / (double)n;
+            re[m] = cos(ang); im[m] = sin(ang);
+        }
+        gpe_status s = upload_cplx<T>(p, ax == 0 ? &p->tw_x : &p->tw_y, re, im);
+        if (s != GPE_OK) return s;
+    }
+    return GPE_OK;
+}
+
+// kinetic tables for (dt, mode) (row a3); 1/(nx ny) of the inverse transform folded into x
+template <typename T> gpe_status make_kinetic(gpe_plan *p, double dt, int mode) {
+    if (p->kin_mode == mode && p->kin_dt == dt) return GPE_OK;
+    if (p->kin_mode != mode) {  // element size changes between real (complex table) and imaginary
+        if (p->kin_x) { cudaFree(p->kin_x); p->kin_x = nullptr; }
+        if (p->kin_y) { cudaFree(p->kin_y); p->kin_y = nullptr; }
+    }
+    const double invP = 1.0 / ((double)p->nx * (double)p->ny);
+    for (int ax = 0; ax < 2; ++ax) {
+        int n = ax == 0 ? p->nx : p->ny;
+        double L = ax == 0 ? p->Lx : p->Ly;
+        double sc = ax == 0 ? invP : 1.0;
+        std::vector<double> re(n), im(n);
+        for (int q = 0; q < n; ++q) {
+            double k = wavenumber(q, n, L), w = k * k * dt * 0.5;
+            if (mode == GPE_IMAG_TIME) { re[q] = exp(-w) * sc; im[q] = 0.0; }
+            else {  // exp(-i w) - 1 = -2 sin^2(w/2) - i sin w  (see sincosm1_t in gpe_kernels.cuh)
+                double sh = sin(0.5 * w);
+                re[q] = -2.0 * sh * sh * sc; im[q] = -sin(w) * sc;
+            }
+        }
+        void **dev = ax == 0 ? &p->kin_x : &p->kin_y;
+        gpe_status s = mode == GPE_IMAG_TIME ? upload_real<T>(p, dev, re) : upload_cplx<T>(p, dev, re, im);
+        if (s != GPE_OK) return s;
+    }
+    p->kin_mode = mode;
+    p->kin_dt = dt;
+    return GPE_OK;
+}
+
+// ------------------------------------------------------------------ small kernels
+// Prologue of gpe_evolve: sums of the wavefunction as handed in by the caller (row a0 needs
+// Theta_0).  grid = (kReduceCtas, batch).
+template <typename T>
+__global__ void __launch_bounds__(256) k_reduce(const cx<T> *psi, int nx, int ny, const T *cavx,
+                                                const T *cavy, int cavity_on, FinalizeParams fin) {
+    __shared__ double red[64];
+    const int b = blockIdx.y;
+    const cx<T> *w = psi + (size_t)b * nx * ny;
+    double sn = 0.0, st = 0.0;
+    for (int i = blockIdx.x; i < nx; i += gridDim.x) {
+        double rn = 0.0, rt = 0.0;
+        for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+            cx<T> z = w[(size_t)i * ny + j];
+            double d = (double)z.x * (double)z.x + (double)z.y * (double)z.y;
+            rn += d;
+            if (cavity_on) rt += d * (double)cavy[j];
+        }
+        sn += rn;
+        if (cavity_on) st += rt * (double)cavx[i];
+    }
+    block_reduce_and_finalize(fin, b, blockIdx.x, sn, st, red);
+}
+
+// Epilogue of an imaginary-time gpe_evolve: apply the pending lazy scale (row a7).
+template <typename T>
+__global__ void __launch_bounds__(256) k_rescale(cx<T> *psi, size_t npts, MemberState *st) {
+    const int b = blockIdx.y;
+    const T s = (T)st[b].scale;
+    cx<T> *w = psi + (size_t)b * npts;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < npts; q += (size_t)gridDim.x * blockDim.x) {
+        cx<T> z = w[q];
+        z.x *= s; z.y *= s;
+        w[q] = z;
+    }
+}
+__global__ void k_reset_scale(MemberState *st, int batch) {
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < batch) st[b].scale = 1.0;
+}
+
+__device__ inline void block_atomic_add(double v, double *dst, double *red) {
+    v = warp_sum(v);
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) red[w] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0;
+        for (int i = 0; i < (int)((blockDim.x + 31) >> 5); ++i) a += red[i];
+        atomicAdd(dst, a);
+    }
+}
+
+// real-space observables: out[b][0..3] += {sum d, sum (Vs + A lat) d, sum d^2, sum cos cos d}
+template <typename T>
+__global__ void __launch_bounds__(256) k_obs_real(const cx<T> *psi, int nx, int ny, int flags, const T *v2d,
+                                                  const T *vx, const T *vy, const T *latx, const T *laty,
+                                                  const T *cavx, const T *cavy, const double *A, double *out,
+                                                  T *density) {
+    __shared__ double red[32];
+    const int b = blockIdx.y;
+    const size_t npts = (size_t)nx * ny;
+    const cx<T> *w = psi + (size_t)b * npts;
+    const T *v2 = (flags & F_HAS_V2D) ? v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * npts : 0) : nullptr;
+    const double Ab = A[b];
+    double sn = 0, sp = 0, s4 = 0, st = 0;
+    for (int i = blockIdx.x; i < nx; i += gridDim.x)
+        for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+            size_t q = (size_t)i * ny + j;
+            cx<T> z = w[q];
+            T dT = z.x * z.x + z.y * z.y;
+            if (density) density[(size_t)b * npts + q] = dT;
+            double d = (double)z.x * (double)z.x + (double)z.y * (double)z.y;
+            double V = 0.0;
+            if (flags & F_HAS_SEP) V += (double)vx[i] + (double)vy[j];
+            if (flags & F_LAT_X) V += Ab * (double)latx[i];
+            if (flags & F_LAT_Y) V += Ab * (double)laty[j];
+            if (v2) V += (double)v2[q];
+            sn += d; sp += V * d; s4 += d * d;
+            if (flags & F_CAVITY) st += (double)cavx[i] * (double)cavy[j] * d;
+        }
+    block_atomic_add(sn, out + b * 8 + 0, red);
+    block_atomic_add(sp, out + b * 8 + 1, red);
+    block_atomic_add(s4, out + b * 8 + 2, red);
+    block_atomic_add(st, out + b * 8 + 3, red);
+}
+
+// k-space sums: out[b][4] += sum |psi^|^2, out[b][5] += sum k^2 |psi^|^2
+template <typename T>
+__global__ void __launch_bounds__(256) k_obs_k(const cx<T> *hat, int nx, int ny, double Lx, double Ly, double *out) {
+    __shared__ double red[32];
+    const int b = blockIdx.y;
+    const cx<T> *w = hat + (size_t)b * nx * ny;
+    double s0 = 0, s2 = 0;
+    for (int i = blockIdx.x; i < nx; i += gridDim.x) {
+        double kx = 2.0 * kPi * (double)(i < nx / 2 ? i : i - nx) / Lx;
+        for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+            double ky = 2.0 * kPi * (double)(j < ny / 2 ? j : j - ny) / Ly;
+            cx<T> z = w[(size_t)i * ny + j];
+            double d = (double)z.x * (double)z.x + (double)z.y * (double)z.y;
+            s0 += d; s2 += (kx * kx + ky * ky) * d;
+        }
+    }
+    block_atomic_add(s0, out + b * 8 + 4, red);
+    block_atomic_add(s2, out + b * 8 + 5, red);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_kdensity(const cx<T> *hat, size_t npts, const double *out, T *kd) {
+    const int b = blockIdx.y;
+    const double inv = 1.0 / out[b * 8 + 4];
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < npts; q += (size_t)gridDim.x * blockDim.x) {
+        cx<T> z = hat[(size_t)b * npts + q];
+        kd[(size_t)b * npts + q] = (T)(((double)z.x * (double)z.x + (double)z.y * (double)z.y) * inv);
+    }
+}
+
+// momentum-order windows: pop[b][m + m_max] += |psi^|^2 for |k - 2 m k_l| < k_l
+template <typename T>
+__global__ void __launch_bounds__(256) k_populations(const cx<T> *hat, int nx, int ny, double Lx, double Ly, int axis,
+                                                     double k_l, int m_max, double *pop) {
+    extern __shared__ double spop[];
+    const int b = blockIdx.y, nm = 2 * m_max + 1;
+    for (int m = threadIdx.x; m < nm; m += blockDim.x) spop[m] = 0.0;
+    __syncthreads();
+    const cx<T> *w = hat + (size_t)b * nx * ny;
+    for (int i = blockIdx.x; i < nx; i += gridDim.x) {
+        double kx = 2.0 * kPi * (double)(i < nx / 2 ? i : i - nx) / Lx;
+        for (int j = threadIdx.x; j < ny; j += blockDim.x) {
+            double ky = 2.0 * kPi * (double)(j < ny / 2 ? j : j - ny) / Ly;
+            double k = axis == 0 ? kx : ky;
+            cx<T> z = w[(size_t)i * ny + j];
+            double d = (double)z.x * (double)z.x + (double)z.y * (double)z.y;
+            for (int m = -m_max; m <= m_max; ++m)
+                if (fabs(k - 2.0 * m * k_l) < k_l) atomicAdd(&spop[m + m_max], d);
+        }
+    }
+    __syncthreads();
+    for (int m = threadIdx.x; m < nm; m += blockDim.x) atomicAdd(&pop[(size_t)b * nm + m], spop[m]);
+}
+
+// ------------------------------------------------------------------ typed implementations
+template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src, void *dst) {
+    StepArgs<T, cx<T>> a;
+    memset(&a, 0, sizeof(a));
+    a.src = (const cx<T> *)src;
+    a.dst = (cx<T> *)dst;
+    a.nx = p->nx; a.ny = p->ny; a.batch = p->batch; a.flags = p->flags;
+    a.v2d = (const T *)p->v2d;
+    a.vx = (const T *)p->vx; a.vy = (const T *)p->vy;
+    a.latx = (const T *)p->latx; a.laty = (const T *)p->laty;
+    a.cavx = (const T *)p->cavx; a.cavy = (const T *)p->cavy;
+    a.g = (const T *)p->g;
+    a.tw_x = (const cx<T> *)p->tw_x; a.tw_y = (const cx<T> *)p->tw_y;
+    a.kin_xc = (const cx<T> *)p->kin_x; a.kin_yc = (const cx<T> *)p->kin_y;
+    a.kin_xr = (const T *)p->kin_x; a.kin_yr = (const T *)p->kin_y;
+    a.inv_p = (T)(1.0 / ((double)p->nx * (double)p->ny));
+    FinalizeParams &f = a.fin;
+    f.st = p->st; f.partials = p->partials; f.counters = p->counters; f.nonfinite = p->nonfinite;
+    f.sched_len = p->sched_len; f.sched_step = p->d_sched_step; f.sched_amp = p->d_sched_amp;
+    f.sched_batched = p->sched_batched;
+    f.cavity_on = p->cavity_on; f.eta_mode = p->eta_mode;
+    f.eta_or_u = p->d_eta; f.n_atoms = p->d_natoms; f.delta = p->d_delta; f.kappa = p->d_kappa;
+    f.dxdy = (p->Lx / p->nx) * (p->Ly / p->ny);
+    f.batch = p->batch;
+    return a;
+}
+
+// per-pass timing (gpe_profile_passes): events bracket ONE pass per step, round-robin, so the
+// host stays ahead of the device and no launch gap is measured.
+struct PassProfile {
+    std::vector<cudaEvent_t> e0, e1;
+    std::vector<int> which;
+};
+
+template <typename T>
+gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode mode, long record_every,
+                       double *records, PassProfile *prof = nullptr) {
+    const bool imag = mode == GPE_IMAG_TIME;
+    gpe_status s = make_kinetic<T>(p, dt, (int)mode);
+    if (s != GPE_OK) return s;
+    const Ops<T> *oy = get_ops<T>(p->ny), *ox = get_ops<T>(p->nx);
+    StepArgs<T, cx<T>> a = base_args<T>(p, psi, psi);
+    a.half_dt = (T)(0.5 * dt);
+    // prologue: Theta_0, A_0, C_0 from the wavefunction as given (row a0)
+    {
+        FinalizeParams f = a.fin;
+        f.cpm = kReduceCtas < p->nx ? kReduceCtas : p->nx;
+        f.normalise = 0; f.advance = 0; f.step0 = p->step;
+        f.record_every = 0; f.records = nullptr;
+        dim3 grid(f.cpm, p->batch);
+        k_reduce<T><<<grid, 256, 0, p->stream>>>((const cx<T> *)psi, p->nx, p->ny, (const T *)p->cavx,
+                                                 (const T *)p->cavy, p->cavity_on, f);
+        GPE_CUDA(p, cudaGetLastError());
+    }
+    a.fin.cpm = p->nx / oy->rows_per_cta;
+    a.fin.normalise = imag ? 1 : 0;
+    a.fin.advance = 1;
+    a.fin.record_every = records ? record_every : 0;
+    a.fin.rec_first = record_every > 0 ? p->step / record_every : 0;
+    a.fin.records = records;
+    for (long n = 0; n < n_steps; ++n) {
+        const int w = prof ? (int)(n % 3) : -1;
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        if (prof) {
+            GPE_CUDA(p, cudaEventCreate(&e0));
+            GPE_CUDA(p, cudaEventCreate(&e1));
+            prof->e0.push_back(e0); prof->e1.push_back(e1); prof->which.push_back(w);
+        }
+        if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, p->stream));
+        GPE_CUDA(p, oy->row_fwd(a, imag, p->stream));
+        if (w == 0) GPE_CUDA(p, cudaEventRecord(e1, p->stream));
+        if (w == 1) GPE_CUDA(p, cudaEventRecord(e0, p->stream));
+        GPE_CUDA(p, ox->col(a, imag, 0, p->stream));
+        if (w == 1) GPE_CUDA(p, cudaEventRecord(e1, p->stream));
+        if (w == 2) GPE_CUDA(p, cudaEventRecord(e0, p->stream));
+        GPE_CUDA(p, oy->row_inv(a, imag, p->stream));
+        if (w == 2) GPE_CUDA(p, cudaEventRecord(e1, p->stream));
+    }
+    if (imag) {
+        dim3 grid(256, p->batch);
+        k_rescale<T><<<grid, 256, 0, p->stream>>>((cx<T> *)psi, (size_t)p->nx * p->ny, p->st);
+        GPE_CUDA(p, cudaGetLastError());
+        k_reset_scale<<<(p->batch + 127) / 128, 128, 0, p->stream>>>(p->st, p->batch);
+        GPE_CUDA(p, cudaGetLastError());
+    }
+    p->step += n_steps;
+    return GPE_OK;
+}
+
+gpe_status ensure_scratch(gpe_plan *p) {
+    if (!p->scratch)
+        GPE_CUDA(p, cudaMalloc(&p->scratch, 2 * real_bytes(p) * (size_t)p->batch * p->nx * p->ny));
+    return GPE_OK;
+}
+
+// psi^ of every member into the plan's scratch buffer (natural FFT order)
+template <typename T> gpe_status fft_to_scratch(gpe_plan *p, const void *psi) {
+    gpe_status s = ensure_scratch(p);
+    if (s != GPE_OK) return s;
+    const Ops<T> *oy = get_ops<T>(p->ny), *ox = get_ops<T>(p->nx);
+    StepArgs<T, cx<T>> a = base_args<T>(p, psi, p->scratch);
+    a.flags |= F_NO_POT;
+    GPE_CUDA(p, oy->row_fwd(a, false, p->stream));
+    a.src = (const cx<T> *)p->scratch;
+    GPE_CUDA(p, ox->col(a, false, 1, p->stream));
+    return GPE_OK;
+}
+
+double host_schedule(const gpe_plan *p, int b, double n) {
+    if (p->sched_len <= 0) return 0.0;
+    const double *amp = p->h_sched_amp.data() + (p->sched_batched ? (size_t)b * p->sched_len : 0);
+    const double *st = p->h_sched_step.data();
+    int L = p->sched_len;
+    if (n < st[0]) return amp[0];
+    int i = 0;
+    for (int q = 0; q < L; ++q)
+        if (st[q] <= n) i = q;
+    if (i == L - 1) return amp[L - 1];
+    double t = (n - st[i]) / (st[i + 1] - st[i]);
+    return amp[i] + t * (amp[i + 1] - amp[i]);
+}
+
+template <typename T>
+gpe_status observables_impl(gpe_plan *p, const void *psi, gpe_obs *out, void *density, void *kdensity) {
+    const int B = p->batch;
+    const size_t npts = (size_t)p->nx * p->ny;
+    if (!p->obs_dev) GPE_CUDA(p, cudaMalloc((void **)&p->obs_dev, sizeof(double) * 8 * B));
+    if (!p->obsA_dev) GPE_CUDA(p, cudaMalloc((void **)&p->obsA_dev, sizeof(double) * B));
+    std::vector<double> A(B);
+    for (int b = 0; b < B; ++b) A[b] = host_schedule(p, b, (double)p->step);
+    GPE_CUDA(p, cudaMemcpyAsync(p->obsA_dev, A.data(), sizeof(double) * B, cudaMemcpyHostToDevice, p->stream));
+    GPE_CUDA(p, cudaMemsetAsync(p->obs_dev, 0, sizeof(double) * 8 * B, p->stream));
+    dim3 grid(p->nx < 256 ? p->nx : 256, B);
+    k_obs_real<T><<<grid, 256, 0, p->stream>>>((const cx<T> *)psi, p->nx, p->ny, p->flags, (const T *)p->v2d,
+                                               (const T *)p->vx, (const T *)p->vy, (const T *)p->latx,
+                                               (const T *)p->laty, (const T *)p->cavx, (const T *)p->cavy,
+                                               p->obsA_dev, p->obs_dev, (T *)density);
+    GPE_CUDA(p, cudaGetLastError());
+    gpe_status s = fft_to_scratch<T>(p, psi);
+    if (s != GPE_OK) return s;
+    k_obs_k<T><<<grid, 256, 0, p->stream>>>((const cx<T> *)p->scratch, p->nx, p->ny, p->Lx, p->Ly, p->obs_dev);
+    GPE_CUDA(p, cudaGetLastError());
+    if (kdensity) {
+        dim3 g2(256, B);
+        k_kdensity<T><<<g2, 256, 0, p->stream>>>((const cx<T> *)p->scratch, npts, p->obs_dev, (T *)kdensity);
+        GPE_CUDA(p, cudaGetLastError());
+    }
+    std::vector<double> h(8 * B);
+    int nonfinite = 0;
+    GPE_CUDA(p, cudaMemcpyAsync(h.data(), p->obs_dev, sizeof(double) * 8 * B, cudaMemcpyDeviceToHost, p->stream));
+    GPE_CUDA(p, cudaMemcpyAsync(&nonfinite, p->nonfinite, sizeof(int), cudaMemcpyDeviceToHost, p->stream));
+    GPE_CUDA(p, cudaStreamSynchronize(p->stream));
+    const double dxdy = (p->Lx / p->nx) * (p->Ly / p->ny);
+    for (int b = 0; b < B; ++b) {
+        const double *r = &h[8 * b];
+        gpe_obs &o = out[b];
+        o.norm = r[0] * dxdy;
+        o.e_pot = r[1] * dxdy;
+        o.e_int = 0.5 * (p->h_g.empty() ? 0.0 : p->h_g[b]) * r[2] * dxdy;
+        o.theta = p->cavity_on ? r[3] * dxdy : 0.0;
+        o.e_kin = 0.5 * r[5] / r[4] * o.norm;
+        o.e_cav = 0.0; o.re_alpha = 0.0; o.im_alpha = 0.0;
+        if (p->cavity_on) {
+            double eta = p->eta_mode == 0 ? p->h_eta[b] : sqrt(fabs(A[b]) * p->h_eta[b]);
+            double D = p->h_delta[b], K = p->h_kappa[b], den = D * D + K * K;
+            double num = p->h_natoms[b] * eta * o.theta;
+            o.re_alpha = num * D / den;
+            o.im_alpha = -num * K / den;
+            o.e_cav = p->h_natoms[b] * eta * eta * o.theta * o.theta * D / den;
+        }
+    }
+    if (nonfinite) return fail(p, GPE_ENONFINITE, "a non-finite norm was seen during gpe_evolve");
+    return GPE_OK;
+}
+
+template <typename T>
+gpe_status populations_impl(gpe_plan *p, const void *psi, int axis, double k_l, int m_max, double *out) {
+    const int B = p->batch, nm = 2 * m_max + 1;
+    if (!p->obs_dev) GPE_CUDA(p, cudaMalloc((void **)&p->obs_dev, sizeof(double) * 8 * B));
+    if (p->pop_len < nm * B) {
+        if (p->pop_dev) cudaFree(p->pop_dev);
+        p->pop_dev = nullptr;
+        GPE_CUDA(p, cudaMalloc((void **)&p->pop_dev, sizeof(double) * nm * B));
+        p->pop_len = nm * B;
+    }
+    GPE_CUDA(p, cudaMemsetAsync(p->obs_dev, 0, sizeof(double) * 8 * B, p->stream));
+    GPE_CUDA(p, cudaMemsetAsync(p->pop_dev, 0, sizeof(double) * nm * B, p->stream));
+    gpe_status s = fft_to_scratch<T>(p, psi);
+    if (s != GPE_OK) return s;
+    dim3 grid(p->nx < 256 ? p->nx : 256, B);
+    k_obs_k<T><<<grid, 256, 0, p->stream>>>((const cx<T> *)p->scratch, p->nx, p->ny, p->Lx, p->Ly, p->obs_dev);
+    GPE_CUDA(p, cudaGetLastError());
+    k_populations<T><<<grid, 256, sizeof(double) * nm, p->stream>>>((const cx<T> *)p->scratch, p->nx, p->ny, p->Lx,
+                                                                   p->Ly, axis, k_l, m_max, p->pop_dev);
+    GPE_CUDA(p, cudaGetLastError());
+    std::vector<double> h(8 * B);
+    GPE_CUDA(p, cudaMemcpyAsync(h.data(), p->obs_dev, sizeof(double) * 8 * B, cudaMemcpyDeviceToHost, p->stream));
+    GPE_CUDA(p, cudaMemcpyAsync(out, p->pop_dev, sizeof(double) * nm * B, cudaMemcpyDeviceToHost, p->stream));
+    GPE_CUDA(p, cudaStreamSynchronize(p->stream));
+    for (int b = 0; b < B; ++b)
+        for (int m = 0; m < nm; ++m) out[(size_t)b * nm + m] /= h[8 * b + 4];
+    return GPE_OK;
+}
+
+template <typename T> gpe_status set_potential_impl(gpe_plan *p, const gpe_potential_desc *d) {
+    const int nx = p->nx, ny = p->ny, B = p->batch;
+    int flags = 0;
+    gpe_status s;
+    std::vector<double> hx(nx, 0.0), hy(ny, 0.0);
+    if (d->vx || d->vy) {
+        flags |= F_HAS_SEP;
+        if (d->vx) hx.assign(d->vx, d->vx + nx);
+        if (d->vy) hy.assign(d->vy, d->vy + ny);
+    }
+    if ((s = upload_real<T>(p, &p->vx, hx)) != GPE_OK) return s;
+    if ((s = upload_real<T>(p, &p->vy, hy)) != GPE_OK) return s;
+    std::vector<double> lx(nx, 0.0), ly(ny, 0.0), cxv(nx, 0.0), cyv(ny, 0.0);
+    if (d->lattice_axis == 0) {
+        flags |= F_LAT_X;
+        for (int i = 0; i < nx; ++i) { double c = cos(d->lattice_k * coord(i, nx, p->Lx)); lx[i] = c * c; }
+    } else if (d->lattice_axis == 1) {
+        flags |= F_LAT_Y;
+        for (int j = 0; j < ny; ++j) { double c = cos(d->lattice_k * coord(j, ny, p->Ly)); ly[j] = c * c; }
+    }
+    if (d->cavity_on) {
+        flags |= F_CAVITY;
+        for (int i = 0; i < nx; ++i) cxv[i] = cos(d->cavity_k * coord(i, nx, p->Lx));
+        for (int j = 0; j < ny; ++j) cyv[j] = cos(d->cavity_k * coord(j, ny, p->Ly));
+    }
+    if ((s = upload_real<T>(p, &p->latx, lx)) != GPE_OK) return s;
+    if ((s = upload_real<T>(p, &p->laty, ly)) != GPE_OK) return s;
+    if ((s = upload_real<T>(p, &p->cavx, cxv)) != GPE_OK) return s;
+    if ((s = upload_real<T>(p, &p->cavy, cyv)) != GPE_OK) return s;
+    p->h_g.assign(B, 0.0);
+    if (d->g) {
+        p->h_g.assign(d->g, d->g + B);
+        for (int b = 0; b < B; ++b) if (p->h_g[b] != 0.0) flags |= F_HAS_G;
+    }
+    if ((s = upload_real<T>(p, &p->g, p->h_g)) != GPE_OK) return s;
+    if (d->v_static) {
+        flags |= F_HAS_V2D;
+        if (d->v_static_batched) flags |= F_V2D_BATCHED;
+        size_t elems = (size_t)nx * ny * (d->v_static_batched ? B : 1);
+        if (p->v2d && p->v2d_elems != elems) { cudaFree(p->v2d); p->v2d = nullptr; }
+        if (!p->v2d) GPE_CUDA(p, cudaMalloc(&p->v2d, sizeof(T) * elems));
+        p->v2d_elems = elems;
+        GPE_CUDA(p, cudaMemcpyAsync(p->v2d, d->v_static, sizeof(T) * elems, cudaMemcpyDeviceToDevice, p->stream));
+    }
+    p->flags = flags;
+    return GPE_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ C ABI
+extern "C" {
+
+const char *gpe_version(void) { return "libgpe 0.1 sm_100a"; }
+
+const char *gpe_last_error(const gpe_plan *p) { return p ? p->err.c_str() : g_create_error.c_str(); }
+
+gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly, gpe_dtype dtype, int batch) {
+    if (!out) return fail(nullptr, GPE_EINVAL, "out is NULL");
+    if (nx <= 0 || ny <= 0 || batch < 1 || !(Lx > 0) || !(Ly > 0) || !std::isfinite(Lx) || !std::isfinite(Ly))
+        return fail(nullptr, GPE_EINVAL, "nx, ny, batch must be positive and Lx, Ly finite and > 0");
+    if (dtype != GPE_C64 && dtype != GPE_C128) return fail(nullptr, GPE_EINVAL, "unknown dtype");
+    if (!pow2_in_range(nx) || !pow2_in_range(ny))
+        return fail(nullptr, GPE_EUNSUPPORTED, "nx and ny must be powers of two in [64, 2048]");
+    gpe_plan *p = new (std::nothrow) gpe_plan();
+    if (!p) return fail(nullptr, GPE_ENOMEM, "out of host memory");
+    p->nx = nx; p->ny = ny; p->batch = batch; p->Lx = Lx; p->Ly = Ly; p->dtype = dtype;
+    gpe_status s = GPE_OK;
+    auto body = [&]() -> gpe_status {
+        int dev_count = 0;
+        GPE_CUDA(p, cudaGetDeviceCount(&dev_count));
+        if (dev_count <= 0) return fail(p, GPE_ECUDA, "no CUDA device");
+        GPE_CUDA(p, cudaMalloc((void **)&p->st, sizeof(MemberState) * batch));
+        GPE_CUDA(p, cudaMemset(p->st, 0, sizeof(MemberState) * batch));
+        GPE_CUDA(p, cudaMalloc((void **)&p->partials, sizeof(double2) * (size_t)batch * kMaxCpm));
+        GPE_CUDA(p, cudaMalloc((void **)&p->counters, sizeof(unsigned int) * batch));
+        GPE_CUDA(p, cudaMemset(p->counters, 0, sizeof(unsigned int) * batch));
+        GPE_CUDA(p, cudaMalloc((void **)&p->nonfinite, sizeof(int)));
+        GPE_CUDA(p, cudaMemset(p->nonfinite, 0, sizeof(int)));
+        return dtype == GPE_C64 ? make_twiddles<float>(p) : make_twiddles<double>(p);
+    };
+    s = body();
+    if (s != GPE_OK) {
+        g_create_error = p->err;
+        gpe_plan_destroy(p);
+        return s;
+    }
+    *out = p;
+    return GPE_OK;
+}
+
+gpe_status gpe_plan_set_stream(gpe_plan *p, void *cuda_stream) {
+    if (!p) return GPE_EINVAL;
+    p->stream = (cudaStream_t)cuda_stream;
+    return GPE_OK;
+}
+
+gpe_status gpe_plan_destroy(gpe_plan *p) {
+    if (!p) return GPE_OK;
+    cudaStreamSynchronize(p->stream);
+    void *bufs[] = {p->tw_x, p->tw_y, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
+                    p->g, p->v2d, p->st, p->partials, p->counters, p->nonfinite, p->d_sched_step,
+                    p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->scratch, p->obs_dev,
+                    p->pop_dev, p->obsA_dev};
+    for (void *b : bufs)
+        if (b) cudaFree(b);
+    delete p;
+    return GPE_OK;
+}
+
+gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
+    if (!p) return GPE_EINVAL;
+    if (!d) return fail(p, GPE_EINVAL, "descriptor is NULL");
+    const int B = p->batch;
+    if (d->lattice_axis < -1 || d->lattice_axis > 1) return fail(p, GPE_EINVAL, "lattice_axis must be -1, 0 or 1");
+    if (d->sched_len < 0 || (d->sched_len > 0 && (!d->sched_step || !d->sched_amp)))
+        return fail(p, GPE_EINVAL, "schedule arrays missing");
+    for (int i = 0; i < d->sched_len; ++i) {
+        if (!std::isfinite(d->sched_step[i])) return fail(p, GPE_EINVAL, "sched_step not finite");
+        if (i > 0 && d->sched_step[i] < d->sched_step[i - 1])
+            return fail(p, GPE_EINVAL, "sched_step must be non-decreasing");
+    }
+    if (d->cavity_on && (!d->eta_or_u || !d->delta || !d->kappa))
+        return fail(p, GPE_EINVAL, "cavity_on needs eta_or_u, delta and kappa");
+    if (d->cavity_on && d->eta_mode != 0 && d->eta_mode != 1) return fail(p, GPE_EINVAL, "eta_mode must be 0 or 1");
+    if (d->cavity_on)
+        for (int b = 0; b < B; ++b)
+            if (d->delta[b] == 0.0 && d->kappa[b] == 0.0) return fail(p, GPE_EINVAL, "Delta + i kappa is zero");
+    if (d->v_static && ((uintptr_t)d->v_static % real_bytes(p)) != 0) return fail(p, GPE_EINVAL, "v_static misaligned");
+
+    p->lattice_axis = d->lattice_axis; p->lattice_k = d->lattice_k;
+    p->sched_len = d->sched_len; p->sched_batched = d->sched_len > 0 ? (d->sched_batched ? 1 : 0) : 0;
+    p->cavity_on = d->cavity_on ? 1 : 0; p->cavity_k = d->cavity_k; p->eta_mode = d->eta_mode;
+    p->h_sched_step.clear(); p->h_sched_amp.clear();
+    if (d->sched_len > 0) {
+        p->h_sched_step.assign(d->sched_step, d->sched_step + d->sched_len);
+        size_t na = (size_t)d->sched_len * (p->sched_batched ? B : 1);
+        p->h_sched_amp.assign(d->sched_amp, d->sched_amp + na);
+    }
+    p->h_eta.assign(B, 0.0); p->h_natoms.assign(B, 1.0); p->h_delta.assign(B, -1.0); p->h_kappa.assign(B, 1.0);
+    if (d->cavity_on) {
+        p->h_eta.assign(d->eta_or_u, d->eta_or_u + B);
+        if (d->n_atoms) p->h_natoms.assign(d->n_atoms, d->n_atoms + B);
+        p->h_delta.assign(d->delta, d->delta + B);
+        p->h_kappa.assign(d->kappa, d->kappa + B);
+    }
+    gpe_status s;
+    if ((s = upload_f64(p, &p->d_sched_step, p->h_sched_step)) != GPE_OK) return s;
+    if ((s = upload_f64(p, &p->d_sched_amp, p->h_sched_amp)) != GPE_OK) return s;
+    if ((s = upload_f64(p, &p->d_eta, p->h_eta)) != GPE_OK) return s;
+    if ((s = upload_f64(p, &p->d_natoms, p->h_natoms)) != GPE_OK) return s;
+    if ((s = upload_f64(p, &p->d_delta, p->h_delta)) != GPE_OK) return s;
+    if ((s = upload_f64(p, &p->d_kappa, p->h_kappa)) != GPE_OK) return s;
+    s = p->dtype == GPE_C64 ? set_potential_impl<float>(p, d) : set_potential_impl<double>(p, d);
+    if (s != GPE_OK) return s;
+    p->pot_set = true;
+    return GPE_OK;
+}
+
+gpe_status gpe_evolve(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode mode, long record_every,
+                      double *records) {
+    if (!p) return GPE_EINVAL;
+    if (!p->pot_set) return fail(p, GPE_ESTATE, "gpe_evolve before gpe_set_potential");
+    if (!psi || ((uintptr_t)psi % 16) != 0) return fail(p, GPE_EINVAL, "psi is NULL or not 16-byte aligned");
+    if (mode != GPE_REAL_TIME && mode != GPE_IMAG_TIME) return fail(p, GPE_EINVAL, "unknown mode");
+    if (!std::isfinite(dt) || dt == 0.0 || (mode == GPE_IMAG_TIME && dt < 0.0))
+        return fail(p, GPE_EINVAL, "dt must be finite, non-zero, and > 0 in imaginary time");
+    if (n_steps < 0 || record_every < 0) return fail(p, GPE_EINVAL, "n_steps and record_every must be >= 0");
+    if (record_every > 0 && !records) return fail(p, GPE_EINVAL, "record_every > 0 needs a records buffer");
+    if (n_steps == 0) return GPE_OK;
+    return p->dtype == GPE_C64 ? evolve_impl<float>(p, psi, dt, n_steps, mode, record_every, records)
+                               : evolve_impl<double>(p, psi, dt, n_steps, mode, record_every, records);
+}
+
+gpe_status gpe_profile_passes(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode mode, double *ms_out) {
+    if (!p) return GPE_EINVAL;
+    if (!p->pot_set) return fail(p, GPE_ESTATE, "gpe_profile_passes before gpe_set_potential");
+    if (!psi || !ms_out || ((uintptr_t)psi % 16) != 0) return fail(p, GPE_EINVAL, "psi/ms_out NULL or misaligned");
+    if (!std::isfinite(dt) || dt == 0.0 || (mode == GPE_IMAG_TIME && dt < 0.0) || n_steps < 3 || n_steps > 30000)
+        return fail(p, GPE_EINVAL, "dt invalid or n_steps outside [3, 30000]");
+    PassProfile prof;
+    gpe_status s = p->dtype == GPE_C64 ? evolve_impl<float>(p, psi, dt, n_steps, mode, 0, nullptr, &prof)
+                                       : evolve_impl<double>(p, psi, dt, n_steps, mode, 0, nullptr, &prof);
+    cudaError_t e = cudaStreamSynchronize(p->stream);
+    double sum[3] = {0, 0, 0};
+    long cnt[3] = {0, 0, 0};
+    for (size_t i = 0; i < prof.e0.size(); ++i) {
+        float ms = 0.f;
+        if (s == GPE_OK && e == cudaSuccess && cudaEventElapsedTime(&ms, prof.e0[i], prof.e1[i]) == cudaSuccess) {
+            sum[prof.which[i]] += ms;
+            cnt[prof.which[i]] += 1;
+        }
+        cudaEventDestroy(prof.e0[i]);
+        cudaEventDestroy(prof.e1[i]);
+    }
+    if (s != GPE_OK) return s;
+    if (e != cudaSuccess) return cuda_fail(p, e, "cudaStreamSynchronize");
+    for (int k = 0; k < 3; ++k) ms_out[k] = cnt[k] ? sum[k] / (double)cnt[k] : 0.0;
+    return GPE_OK;
+}
+
+gpe_status gpe_observables(gpe_plan *p, const void *psi, gpe_obs *out, void *density, void *kdensity) {
+    if (!p) return GPE_EINVAL;
+    if (!p->pot_set) return fail(p, GPE_ESTATE, "gpe_observables before gpe_set_potential");
+    if (!psi || !out || ((uintptr_t)psi % 16) != 0) return fail(p, GPE_EINVAL, "psi/out NULL or psi misaligned");
+    return p->dtype == GPE_C64 ? observables_impl<float>(p, psi, out, density, kdensity)
+                               : observables_impl<double>(p, psi, out, density, kdensity);
+}
+
+gpe_status gpe_populations(gpe_plan *p, const void *psi, int axis, double k_l, int m_max, double *out) {
+    if (!p) return GPE_EINVAL;
+    if (!psi || !out || ((uintptr_t)psi % 16) != 0) return fail(p, GPE_EINVAL, "psi/out NULL or psi misaligned");
+    if ((axis != 0 && axis != 1) || !(k_l > 0) || m_max < 0 || m_max > 64)
+        return fail(p, GPE_EINVAL, "axis in {0,1}, k_l > 0, 0 <= m_max <= 64");
+    return p->dtype == GPE_C64 ? populations_impl<float>(p, psi, axis, k_l, m_max, out)
+                               : populations_impl<double>(p, psi, axis, k_l, m_max, out);
+}
+
+gpe_status gpe_get_step(const gpe_plan *p, long *step) {
+    if (!p || !step) return GPE_EINVAL;
+    *step = p->step;
+    return GPE_OK;
+}
+
+gpe_status gpe_set_step(gpe_plan *p, long step) {
+    if (!p) return GPE_EINVAL;
+    p->step = step;
+    return GPE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,70 @@
+// gpe_types.h -- plain structs shared by the host side (gpe_api.cu) and the kernels.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace gpe {
+
+// Per-member device scalars: written by the last block of the
+// reducing pass, read by the next pass.  Never read by the host inside gpe_evolve.
+struct MemberState {
+    double scale;      // lazy renormalisation: the stored psi times `scale` is the wavefunction
+    double A;          // schedule amplitude A_n of the upcoming step
+    double C;          // cavity coefficient C_n = 2 eta_n Re(alpha_n) of the upcoming step
+    double norm;       // sum |psi|^2 dx dy of the current wavefunction
+    double theta;      // cavity overlap Theta (Eq. 14)
+    double re_alpha, im_alpha;
+    long long step;    // step counter n
+};
+
+// Everything the finalising block needs (schedule, cavity parameters, records).
+struct FinalizeParams {
+    MemberState *st;          // [batch]
+    double2 *partials;        // [batch][cpm] (sum |psi|^2, sum cos cos |psi|^2)
+    unsigned int *counters;   // [batch]
+    int *nonfinite;           // sticky flag
+    int cpm;                  // CTAs per member in the reducing pass
+    int sched_len;
+    const double *sched_step; // [sched_len]
+    const double *sched_amp;  // [sched_len] or [batch][sched_len]
+    int sched_batched;
+    int cavity_on, eta_mode;
+    const double *eta_or_u, *n_atoms, *delta, *kappa;  // [batch]
+    double dxdy;
+    long long record_every, rec_first;  // rec_first = floor(step0 / record_every)
+    double *records;          // [n_rec][batch][6] or nullptr
+    int batch;
+    int normalise;            // 1: imaginary-time step (scale <- 1/sqrt(norm), Theta /= norm)
+    int advance;              // 1: a step was taken (step += 1); 0: prologue reduction
+    long long step0;          // used when advance == 0: sets the step counter
+};
+
+enum : int {
+    F_HAS_V2D = 1,    // general 2-D static potential array
+    F_V2D_BATCHED = 2,
+    F_HAS_SEP = 4,    // separable static part vx[i] + vy[j]
+    F_LAT_X = 8,      // A cos^2(k_l x)
+    F_LAT_Y = 16,     // A cos^2(k_l y)
+    F_CAVITY = 32,
+    F_HAS_G = 64,
+    F_NO_POT = 128    // plain FFT pass (observables)
+};
+
+// Arguments of the three passes of one step.  T = float / double.
+template <typename T, typename C> struct StepArgs {
+    const C *src;  // [batch][nx][ny]
+    C *dst;        // same buffer as src inside gpe_evolve
+    int nx, ny, batch, flags;
+    const T *v2d;                  // [nx][ny] or [batch][nx][ny]
+    const T *vx, *vy;              // separable static part
+    const T *latx, *laty;          // cos^2(k_l x_i), cos^2(k_l y_j)
+    const T *cavx, *cavy;          // cos(k_c x_i), cos(k_c y_j)
+    const T *g;                    // [batch]
+    T half_dt;                     // dt/2
+    const C *tw_x, *tw_y;          // exp(-2 pi i m / nx), exp(-2 pi i m / ny)
+    const C *kin_xc, *kin_yc;      // real time: (exp(-i kx^2 dt/2) - 1)/(nx ny), exp(-i ky^2 dt/2) - 1
+    T inv_p;                       // 1/(nx ny)
+    const T *kin_xr, *kin_yr;      // imaginary time: exp(-kx^2 dt/2)/(nx ny), exp(-ky^2 dt/2)
+    FinalizeParams fin;
+};
+
+}  // namespace gpe

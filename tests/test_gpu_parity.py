@@ -1,0 +1,327 @@
+"""Parity of the CUDA path (libgpe.so through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+relative L2 error of psi per step <= 1e-5 (complex64) / 1e-12 (complex128); after a full run
+<= 1e-3 / 1e-10; energies and cavity order parameter within 1e-5 relative (complex64).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle.gpe_oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+PER_STEP = {"c64": 1e-5, "c128": 1e-12}
+FULL_RUN = {"c64": 1e-3, "c128": 1e-10}
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _gpu_plan(p, dtype, use_separable=True):
+    import paper_2404_14401_b200 as G
+    plan = G.Plan(p["nx"], p["ny"], p["Lx"], p["Ly"], dtype, p.get("batch", 1))
+    plan.set_potential(p, use_separable=use_separable)
+    return plan
+
+
+def _to_dev(psi0, dtype):
+    torch = _torch()
+    cd = np.complex64 if dtype == "c64" else np.complex128
+    return torch.from_numpy(np.ascontiguousarray(psi0.astype(cd))).cuda()
+
+
+def _oracle_input(psi0, dtype):
+    """The oracle gets the same values the GPU gets: for complex64 the fp32-rounded array."""
+    cd = np.complex64 if dtype == "c64" else np.complex128
+    return np.ascontiguousarray(psi0.astype(cd).astype(np.complex128))
+
+
+def _rel(a, b):
+    return float(np.linalg.norm(a.astype(np.complex128).ravel() - b.ravel()) / np.linalg.norm(b.ravel()))
+
+
+def _general_workload(nx, ny, batch=1, mode="real"):
+    """Everything switched on: 2-D static array, lattice, cavity, g, ramped schedule."""
+    Lx, Ly = 4 * math.pi, 4 * math.pi
+    p = W._base(nx, ny, Lx, batch)
+    p["Ly"] = Ly
+    v2d, vx, vy = W.harmonic_trap(nx, ny, Lx, Ly, 1.0, 0.7)
+    p["v_static"], p["vx"], p["vy"] = v2d, vx, vy
+    p["g"] = np.linspace(20.0, 60.0, batch)
+    p["lattice_axis"], p["lattice_k"] = 1, 4.0
+    p["sched_step"] = np.array([0.0, 4.0, 4.0, 50.0])
+    p["sched_amp"] = np.array([6.0, 6.0, 9.0, 12.0])
+    p["cavity_on"], p["cavity_k"], p["eta_mode"] = 1, 4.0, 1
+    p["eta_or_u"] = np.full(batch, 4.0)
+    p["n_atoms"] = np.full(batch, 1.5)
+    p["delta"] = np.linspace(-1.0, -2.0, batch)
+    p["kappa"] = np.full(batch, 0.5)
+    one = W.noisy_gaussian(nx, ny, Lx, Ly, 1.2, 7)
+    p["psi0"] = np.ascontiguousarray(np.broadcast_to(one, (batch, nx, ny))) if batch > 1 else one
+    return p
+
+
+SIZES = [(64, 64), (128, 128), (256, 256), (512, 512), (1024, 1024), (2048, 2048),
+         (64, 256), (1024, 128), (128, 2048), (2048, 64)]
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("mode", ["real", "imag"])
+@pytest.mark.parametrize("nx,ny", SIZES)
+def test_per_step_parity_all_sizes(nx, ny, mode, dtype):
+    """One step and then three more, every supported size (square and ragged nx != ny)."""
+    p = _general_workload(nx, ny)
+    dt = 1e-3
+    plan = _gpu_plan(p, dtype, use_separable=False)
+    psi = _to_dev(p["psi0"], dtype)
+    ref = _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    plan.evolve(psi, dt, 1, mode)
+    o.evolve(ref, dt, 1, mode == "imag")
+    e1 = _rel(psi.cpu().numpy(), ref)
+    assert e1 <= PER_STEP[dtype], f"1 step: {e1:.3e}"
+    plan.evolve(psi, dt, 3, mode)
+    o.evolve(ref, dt, 3, mode == "imag")
+    e4 = _rel(psi.cpu().numpy(), ref)
+    assert e4 <= 4 * PER_STEP[dtype], f"4 steps: {e4:.3e}"
+    assert plan.step == 4
+    plan.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_separable_and_2d_static_agree_with_oracle(dtype):
+    p = _general_workload(256, 128)
+    outs = []
+    for sep in (True, False):
+        plan = _gpu_plan(p, dtype, use_separable=sep)
+        psi = _to_dev(p["psi0"], dtype)
+        plan.evolve(psi, 1e-3, 5, "real")
+        outs.append(psi.cpu().numpy())
+        plan.close()
+    ref = _oracle_input(p["psi0"], dtype)
+    Oracle(p).evolve(ref, 1e-3, 5, False)
+    assert _rel(outs[0], ref) <= 5 * PER_STEP[dtype]
+    assert _rel(outs[1], ref) <= 5 * PER_STEP[dtype]
+
+
+@pytest.mark.parametrize("g", [0.0, 10.0])
+def test_config1_full_run(g):
+    """BASELINE.json configs[0]: 64^2 complex128, 2000 imaginary-time steps."""
+    p = W.config1(g=g)
+    plan = _gpu_plan(p, "c128")
+    psi = _to_dev(p["psi0"], "c128")
+    ref = p["psi0"].copy()
+    o = Oracle(p)
+    plan.evolve(psi, 1e-3, 2000, "imag")
+    o.evolve(ref, 1e-3, 2000, True)
+    assert _rel(psi.cpu().numpy(), ref) <= FULL_RUN["c128"]
+    go = plan.observables(psi)[0][0]
+    ro = o.observables(ref)[0][0]
+    for k in ("norm", "e_kin", "e_pot", "e_int"):
+        assert go[k] == pytest.approx(ro[k], rel=1e-10, abs=1e-13), k
+    if g == 0.0:
+        assert abs(go["e_kin"] + go["e_pot"] - 1.0) <= 2e-4   # hbar (wx+wy)/2, north_star pin
+    plan.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_config2_kapitza_dirac(dtype):
+    """BASELINE.json configs[1] (256^2), shortened ground-state phase (500 steps instead of
+    5000 to keep the oracle's share of the test short); pulse 200 steps + 500 free steps."""
+    p = W.config2(V0=20.0, dtype=dtype, n_ground=500)
+    pg = dict(p)
+    pg["sched_step"], pg["sched_amp"] = None, None           # lattice off for the ground state
+    plan = _gpu_plan(pg, dtype)
+    psi = _to_dev(p["psi0"], dtype)
+    ref = _oracle_input(p["psi0"], dtype)
+    o = Oracle(pg)
+    plan.evolve(psi, 1e-3, 500, "imag")
+    o.evolve(ref, 1e-3, 500, True)
+    assert _rel(psi.cpu().numpy(), ref) <= FULL_RUN[dtype]
+    # pulse + free evolution, same plan, new potential, step counter reset
+    plan.set_potential(p)
+    plan.step = 0
+    o2 = Oracle(p)
+    for n in (200, 500):
+        plan.evolve(psi, 1e-4, n, "real")
+        o2.evolve(ref, 1e-4, n, False)
+        assert _rel(psi.cpu().numpy(), ref) <= FULL_RUN[dtype]
+        gp = plan.populations(psi, 0, 4.0, 3)[0]
+        rp = o2.populations(ref, 0, 4.0, 3)[0]
+        tol = 1e-5 if dtype == "c64" else 1e-10
+        assert np.max(np.abs(gp - rp)) <= tol * max(1.0, rp.max())
+        assert gp[4] > 5e-3                                   # first order really populated
+    plan.close()
+
+
+def test_config3_cavity_imag_reduced():
+    """BASELINE.json configs[2] at 256^2 / 400 steps (the oracle finishes in seconds), complex64:
+    imaginary-time cavity ground-state search with per-step Theta and renormalisation."""
+    p = W.config3(n=256, n_steps=400)
+    plan = _gpu_plan(p, "c64")
+    psi = _to_dev(p["psi0"], "c64")
+    ref = _oracle_input(p["psi0"], "c64")
+    o = Oracle(p)
+    rec = plan.evolve(psi, 5e-4, 400, "imag", record_every=50)
+    rref = o.evolve(ref, 5e-4, 400, True, record_every=50)
+    assert _rel(psi.cpu().numpy(), ref) <= FULL_RUN["c64"]
+    rec = rec.cpu().numpy()
+    assert rec.shape == rref.shape
+    assert np.array_equal(rec[:, :, 0], rref[:, :, 0])
+    assert np.allclose(rec[:, :, 1], 1.0, atol=1e-12)
+    # order parameter: |dTheta| <= 1e-5 max(|Theta|, 1e-2)  (reading Q17), or within
+    # 3x the fp32 floor of the method itself where the instability amplifies round-off (R2):
+    # the floor is the oracle's own statements run in complex64 (float build) vs complex128.
+    f32 = p["psi0"].astype(np.complex64)
+    rfloor = Oracle(p, "f32").evolve(f32, 5e-4, 400, True, record_every=50)
+    floor = np.abs(rfloor[:, :, 2] - rref[:, :, 2])
+    dth = np.abs(rec[:, :, 2] - rref[:, :, 2])
+    print("theta err gpu", dth.ravel(), "fp32 floor", floor.ravel())
+    assert np.all(dth <= np.maximum(1e-5 * np.maximum(np.abs(rref[:, :, 2]), 1e-2), 3 * floor))
+    go = plan.observables(psi)[0][0]
+    ro = o.observables(ref)[0][0]
+    for k in ("e_kin", "e_pot", "e_int"):
+        assert go[k] == pytest.approx(ro[k], rel=1e-5), k
+    plan.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_config4_ramp_reduced(dtype):
+    """BASELINE.json configs[3] at 256^2 / 300 steps: real-time pump ramp, records every 100."""
+    p = W.config4(n=256, n_steps=300, ramp_steps=300)
+    plan = _gpu_plan(p, dtype)
+    psi = _to_dev(p["psi0"], dtype)
+    ref = _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    rec = plan.evolve(psi, 1e-4, 300, "real", record_every=100).cpu().numpy()
+    rref = o.evolve(ref, 1e-4, 300, False, record_every=100)
+    assert _rel(psi.cpu().numpy(), ref) <= FULL_RUN[dtype]
+    tol = 1e-5 if dtype == "c64" else 1e-10
+    assert np.allclose(rec[:, :, 1], rref[:, :, 1], rtol=tol)
+    assert np.all(np.abs(rec[:, :, 2] - rref[:, :, 2]) <= tol * np.maximum(np.abs(rref[:, :, 2]), 1e-2))
+    assert np.allclose(rec[:, :, 3:5], rref[:, :, 3:5], rtol=10 * tol, atol=tol * 1e-2)
+    assert np.allclose(rec[:, :, 5], rref[:, :, 5], rtol=1e-14)
+    plan.close()
+
+
+def test_config5_batch_reduced_and_member_equivalence():
+    """BASELINE.json configs[4] at 2x2 members of 128^2, 200 steps; member b of the batched run
+    equals the single-grid run with the same parameters (bitwise: fixed reduction order)."""
+    p = W.config5(n=128, side=2, n_steps=200)
+    plan = _gpu_plan(p, "c64")
+    psi = _to_dev(p["psi0"], "c64")
+    ref = _oracle_input(p["psi0"], "c64")
+    o = Oracle(p)
+    plan.evolve(psi, 5e-4, 200, "imag")
+    o.evolve(ref, 5e-4, 200, True)
+    out = psi.cpu().numpy()
+    for b in range(4):
+        assert _rel(out[b], ref[b]) <= FULL_RUN["c64"], b
+    gth = np.array([ob["theta"] for ob in plan.observables(psi)[0]])
+    rth = np.array([ob["theta"] for ob in o.observables(ref)[0]])
+    assert np.all(np.abs(gth - rth) <= 1e-5 * np.maximum(np.abs(rth), 1e-2))
+    for b in (0, 3):
+        q = W.member(p, b)
+        plan1 = _gpu_plan(q, "c64")
+        s = _to_dev(q["psi0"], "c64")
+        plan1.evolve(s, 5e-4, 200, "imag")
+        assert np.array_equal(s.cpu().numpy(), out[b])
+        plan1.close()
+    plan.close()
+
+
+def test_observables_and_kdensity_parity():
+    p = _general_workload(128, 256)
+    for dtype, tol in (("c64", 1e-5), ("c128", 1e-11)):
+        plan = _gpu_plan(p, dtype, use_separable=False)
+        psi = _to_dev(p["psi0"], dtype)
+        ref = _oracle_input(p["psi0"], dtype)
+        o = Oracle(p)
+        plan.evolve(psi, 1e-3, 3, "real")
+        o.evolve(ref, 1e-3, 3, False)
+        gobs, gd, gk = plan.observables(psi, density=True, kdensity=True)
+        robs, rd, rk = o.observables(ref, density=True, kdensity=True)
+        for k in ("norm", "e_kin", "e_pot", "e_int", "e_cav", "theta", "re_alpha", "im_alpha"):
+            assert gobs[0][k] == pytest.approx(robs[0][k], rel=tol, abs=tol * 1e-3), k
+        assert np.max(np.abs(gd.cpu().numpy() - rd)) <= tol * rd.max()
+        assert np.max(np.abs(gk.cpu().numpy() - rk)) <= tol * rk.max()
+        plan.close()
+
+
+def test_real_time_invariants_on_device():
+    """Properties that hold at any size (used again at full size in test_gpu_fullsize.py)."""
+    p = _general_workload(256, 256)
+    plan = _gpu_plan(p, "c128")
+    psi0 = _to_dev(p["psi0"], "c128")
+    psi = psi0.clone()
+    plan.evolve(psi, 1e-3, 20, "real")
+    assert plan.observables(psi)[0][0]["norm"] == pytest.approx(1.0, abs=1e-12)
+    plan.close()
+    # time reversal without the cavity (Strang is symmetric)
+    q = dict(p)
+    q["cavity_on"] = 0
+    q["sched_step"], q["sched_amp"] = np.array([0.0]), np.array([6.0])
+    plan = _gpu_plan(q, "c128")
+    psi = psi0.clone()
+    plan.evolve(psi, 1e-3, 20, "real")
+    plan.evolve(psi, -1e-3, 20, "real")
+    assert _rel(psi.cpu().numpy(), psi0.cpu().numpy()) <= 1e-12
+    plan.close()
+
+
+def test_step_counter_resume_equals_one_call():
+    """Checkpoint/resume: 2 x 10 steps == 20 steps (schedule time origin persists)."""
+    p = _general_workload(128, 128)
+    outs = []
+    for split in (False, True):
+        plan = _gpu_plan(p, "c64")
+        psi = _to_dev(p["psi0"], "c64")
+        if split:
+            plan.evolve(psi, 1e-3, 10, "real")
+            plan.evolve(psi, 1e-3, 10, "real")
+        else:
+            plan.evolve(psi, 1e-3, 20, "real")
+        outs.append(psi.cpu().numpy())
+        plan.close()
+    # the second call re-derives Theta from the stored psi in a different summation order,
+    # so equality is to fp32 round-off of C_n, not bitwise
+    assert _rel(outs[1], outs[0].astype(np.complex128)) <= 1e-6
+
+
+def test_error_behaviour():
+    import paper_2404_14401_b200 as G
+    torch = _torch()
+    for bad in ((100, 64), (64, 4096), (32, 64)):
+        with pytest.raises(G.GpeError) as e:
+            G.gpe_plan_create(bad[0], bad[1], 1.0, 1.0, G.GPE_C64, 1)
+        assert e.value.status == 2
+    with pytest.raises(G.GpeError) as e:
+        G.gpe_plan_create(64, 64, -1.0, 1.0, G.GPE_C64, 1)
+    assert e.value.status == 1
+    plan = G.gpe_plan_create(64, 64, 16.0, 16.0, G.GPE_C64, 1)
+    psi = torch.zeros((64, 64), dtype=torch.complex64, device="cuda")
+    with pytest.raises(G.GpeError) as e:
+        G.gpe_evolve(plan, psi.data_ptr(), 1e-3, 1, G.GPE_REAL_TIME)
+    assert e.value.status == 5                                  # before gpe_set_potential
+    G.gpe_set_potential(plan, G.gpe_potential_desc(lattice_axis=-1))
+    with pytest.raises(G.GpeError) as e:
+        G.gpe_evolve(plan, psi.data_ptr(), 0.0, 1, G.GPE_REAL_TIME)
+    assert e.value.status == 1
+    with pytest.raises(G.GpeError) as e:
+        G.gpe_evolve(plan, psi.data_ptr() + 8, 1e-3, 1, G.GPE_REAL_TIME)
+    assert e.value.status == 1
+    with pytest.raises(G.GpeError) as e:
+        G.gpe_evolve(plan, psi.data_ptr(), -1e-3, 1, G.GPE_IMAG_TIME)
+    assert e.value.status == 1
+    G.gpe_evolve(plan, psi.data_ptr(), 1e-3, 0, G.GPE_REAL_TIME)  # empty run is fine
+    # all-zero psi in imaginary time: norm 0 -> non-finite scale -> sticky flag
+    G.gpe_evolve(plan, psi.data_ptr(), 1e-3, 2, G.GPE_IMAG_TIME)
+    with pytest.raises(G.GpeError) as e:
+        G.gpe_observables(plan, psi.data_ptr(), 1)
+    assert e.value.status == 6
+    G.gpe_plan_destroy(plan)
