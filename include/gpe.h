@@ -162,6 +162,15 @@ GPE_API gpe_status gpe_populations(gpe_plan *p, const void *psi_dev, int axis, d
                            double *out_host);
 
 /*
+ * gpe_fft2_forward -- the library's own forward 2-D FFT on its own: for every
+ * member dst[p][q] = sum_{ij} src[i][j] exp(-2 pi i (p i / nx + q j / ny)), unnormalised, natural
+ * (fftfreq) order.  src, dst: DEVICE [batch][nx][ny] complex of the plan's dtype; dst may equal
+ * src.  Enqueued on the plan's stream, no synchronisation.  Used by the observables and exposed
+ * so the transform can be tested alone.
+ */
+GPE_API gpe_status gpe_fft2_forward(gpe_plan *p, const void *src_dev, void *dst_dev);
+
+/*
  * gpe_profile_passes -- measurement aid for the roofline report: runs n_steps
  * steps exactly as gpe_evolve does (psi evolves, the step counter advances, no records), with
  * CUDA events on the plan's stream around ONE of the three fused passes per step (round-robin),

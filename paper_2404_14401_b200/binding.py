@@ -69,6 +69,8 @@ def load_library() -> C.CDLL:
     lib.gpe_observables.argtypes = [vp, vp, C.POINTER(gpe_obs), vp, vp]
     lib.gpe_populations.restype = i
     lib.gpe_populations.argtypes = [vp, vp, i, d, i, vp]
+    lib.gpe_fft2_forward.restype = i
+    lib.gpe_fft2_forward.argtypes = [vp, vp, vp]
     lib.gpe_profile_passes.restype = i
     lib.gpe_profile_passes.argtypes = [vp, vp, d, l, i, C.POINTER(C.c_double)]
     lib.gpe_get_step.restype = i
@@ -136,6 +138,10 @@ def gpe_populations(plan, psi_ptr: int, batch: int, axis: int, k_l: float, m_max
     _check(load_library().gpe_populations(plan, C.c_void_p(psi_ptr), int(axis), float(k_l), int(m_max),
                                           C.c_void_p(out.ctypes.data)), plan)
     return out
+
+
+def gpe_fft2_forward(plan, src_ptr: int, dst_ptr: int) -> None:
+    _check(load_library().gpe_fft2_forward(plan, C.c_void_p(src_ptr), C.c_void_p(dst_ptr)), plan)
 
 
 def gpe_profile_passes(plan, psi_ptr: int, dt: float, n_steps: int, mode: int):

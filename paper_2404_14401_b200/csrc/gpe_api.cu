@@ -681,6 +681,17 @@ gpe_status gpe_evolve(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode 
                                : evolve_impl<double>(p, psi, dt, n_steps, mode, record_every, records);
 }
 
+gpe_status gpe_fft2_forward(gpe_plan *p, const void *src, void *dst) {
+    if (!p) return GPE_EINVAL;
+    if (!src || !dst || ((uintptr_t)src % 16) != 0 || ((uintptr_t)dst % 16) != 0)
+        return fail(p, GPE_EINVAL, "src/dst NULL or misaligned");
+    void *keep = p->scratch;
+    p->scratch = dst;
+    gpe_status s = p->dtype == GPE_C64 ? fft_to_scratch<float>(p, src) : fft_to_scratch<double>(p, src);
+    p->scratch = keep;
+    return s;
+}
+
 gpe_status gpe_profile_passes(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode mode, double *ms_out) {
     if (!p) return GPE_EINVAL;
     if (!p->pot_set) return fail(p, GPE_ESTATE, "gpe_profile_passes before gpe_set_potential");

@@ -34,34 +34,47 @@ template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {
 }
 
 // z * exp(SIGN * 2 pi i m / 16), m = 0..7; m is a compile-time constant after unrolling.
-// In fp32 the three constants cos(pi/8), sin(pi/8), sqrt(1/2) all round DOWN, so the rounded
-// twiddles have modulus^2 = 1 - 3.4e-8 / 1 - 5.7e-8: a systematic (not random) loss that made
-// the norm drift by -2e-7 per step in real time.  The float path therefore carries sqrt(1/2) as
-// hi + lo and restores the modulus of the (cos, sin)(pi/8) pair with one extra FMA.
+//
+// In fp32 the constants cos(pi/8), sin(pi/8), sqrt(1/2) all round DOWN, so the rounded twiddles
+// have modulus^2 = 1 - 5.7e-8 / 1 - 3.4e-8.  That loss is systematic, not random: every radix-16
+// butterfly scaled the data by 1 - 1.4e-8 and the norm drifted by -2e-7 per step in real time
+// (cuFFT and pocketfft show the same bias).  The float path therefore uses a unit-modulus pair:
+// S = fl32(sin(pi/8)) exactly and C = sqrt(1 - S^2) = C_hi + C_lo, and sqrt(1/2) = H_hi + H_lo.
+// The low parts must enter BEFORE the single final rounding -- fma(u, C_hi, u*C_lo), never
+// fma(u, C_lo, u*C_hi), whose 0.2-ulp correction would be rounded away.
+template <typename T> struct K16;
+template <> struct K16<float> {
+    static constexpr float C_hi = 0.9238795638084412f, C_lo = -2.8719358092582937e-08f,
+                           S = 0.3826834261417389f, H_hi = 0.7071067690849304f,
+                           H_lo = 1.210161710447897e-08f;
+};
+template <> struct K16<double> {
+    static constexpr double C_hi = 0.92387953251128675613, C_lo = 0.0, S = 0.38268343236508977173,
+                            H_hi = 0.70710678118654752440, H_lo = 0.0;
+};
+// u*C + t with a single rounding of the large terms (t = the S-term plus nothing else)
+template <typename T> __device__ __forceinline__ T mulC_add(T u, T t) {
+    if constexpr (sizeof(T) == 4) return fma(u, K16<T>::C_hi, fma(u, K16<T>::C_lo, t));
+    else return fma(u, K16<T>::C_hi, t);
+}
+template <typename T> __device__ __forceinline__ T mulH(T u) {
+    if constexpr (sizeof(T) == 4) return fma(u, K16<T>::H_hi, u * K16<T>::H_lo);
+    else return u * K16<T>::H_hi;
+}
 template <int SIGN, typename T> __device__ __forceinline__ cx<T> rot16(cx<T> z, int m) {
-    constexpr T c1 = T(0.92387953251128675613), s1 = T(0.38268343236508977173),
-                h = T(0.70710678118654752440);
-    constexpr bool F32 = sizeof(T) == 4;
-    constexpr T h_lo = F32 ? T(1.2101617152815436e-08) : T(0);   // sqrt(1/2) - float(sqrt(1/2))
-    constexpr T eps_g = F32 ? T(2.8534284e-08) : T(0);            // 1/|(c1,s1)_fp32| - 1
+    constexpr T S = K16<T>::S;
     constexpr T sg = T(SIGN);
-    cx<T> r;
     switch (m) {
     case 0: return z;
     case 4: return mk<T>(-sg * z.y, sg * z.x);
-    case 2: r = mk<T>(z.x - sg * z.y, sg * z.x + z.y); break;
-    case 6: r = mk<T>(-(z.x + sg * z.y), sg * z.x - z.y); break;
-    case 1: r = mk<T>(z.x * c1 - z.y * (sg * s1), z.x * (sg * s1) + z.y * c1); break;
-    case 3: r = mk<T>(z.x * s1 - z.y * (sg * c1), z.x * (sg * c1) + z.y * s1); break;
-    case 5: r = mk<T>(-z.x * s1 - z.y * (sg * c1), z.x * (sg * c1) - z.y * s1); break;
-    default: r = mk<T>(-z.x * c1 - z.y * (sg * s1), z.x * (sg * s1) - z.y * c1); break;
+    case 2: return mk<T>(mulH<T>(z.x - sg * z.y), mulH<T>(sg * z.x + z.y));
+    case 6: return mk<T>(mulH<T>(-(z.x + sg * z.y)), mulH<T>(sg * z.x - z.y));
+    // (C + i sg S), (S + i sg C), (-S + i sg C), (-C + i sg S)
+    case 1: return mk<T>(mulC_add<T>(z.x, -(sg * S) * z.y), mulC_add<T>(z.y, (sg * S) * z.x));
+    case 3: return mk<T>(mulC_add<T>(-sg * z.y, S * z.x), mulC_add<T>(sg * z.x, S * z.y));
+    case 5: return mk<T>(mulC_add<T>(-sg * z.y, -S * z.x), mulC_add<T>(sg * z.x, -S * z.y));
+    default: return mk<T>(mulC_add<T>(-z.x, -(sg * S) * z.y), mulC_add<T>(-z.y, (sg * S) * z.x));
     }
-    if (m == 2 || m == 6) {
-        if constexpr (F32) return mk<T>(fma(r.x, h_lo, r.x * h), fma(r.y, h_lo, r.y * h));
-        else return mk<T>(r.x * h, r.y * h);
-    }
-    if constexpr (F32) { r.x = fma(r.x, eps_g, r.x); r.y = fma(r.y, eps_g, r.y); }
-    return r;
 }
 
 // In-register DFT of size R (2, 4, 8, 16): v[k] <- sum_a v[a] exp(SIGN 2 pi i a k / R),

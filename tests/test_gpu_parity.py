@@ -203,8 +203,18 @@ def test_config4_ramp_reduced(dtype):
     assert _rel(psi.cpu().numpy(), ref) <= FULL_RUN[dtype]
     tol = 1e-5 if dtype == "c64" else 1e-10
     assert np.allclose(rec[:, :, 1], rref[:, :, 1], rtol=tol)
-    assert np.all(np.abs(rec[:, :, 2] - rref[:, :, 2]) <= tol * np.maximum(np.abs(rref[:, :, 2]), 1e-2))
-    assert np.allclose(rec[:, :, 3:5], rref[:, :, 3:5], rtol=10 * tol, atol=tol * 1e-2)
+    # order parameter and field: 1e-5 relative (reading Q17), or 3x the fp32 floor of the method
+    # itself (the oracle's statements in complex64 vs complex128) where that is larger (R2)
+    floor = np.zeros_like(rref)
+    if dtype == "c64":
+        f32 = p["psi0"].astype(np.complex64)
+        rfl = Oracle(p, "f32").evolve(f32, 1e-4, 300, False, record_every=100)
+        floor = np.abs(rfl - rref)
+    err = np.abs(rec - rref)
+    print("theta err", err[:, 0, 2], "fp32 floor", floor[:, 0, 2])
+    assert np.all(err[:, :, 2] <= np.maximum(tol * np.maximum(np.abs(rref[:, :, 2]), 1e-2), 3 * floor[:, :, 2]))
+    amax = np.abs(rref[:, :, 3:5]).max()
+    assert np.all(err[:, :, 3:5] <= np.maximum(tol * max(amax, 1e-2), 3 * floor[:, :, 3:5]))
     assert np.allclose(rec[:, :, 5], rref[:, :, 5], rtol=1e-14)
     plan.close()
 
