@@ -192,3 +192,34 @@ def member(p: dict, b: int) -> dict:
     if p.get("psi0") is not None and np.asarray(p["psi0"]).ndim == 3:
         q["psi0"] = np.ascontiguousarray(np.asarray(p["psi0"])[b])
     return q
+
+
+def shard_members(batch: int, rank: int, world: int) -> range:
+    """Batch members owned by `rank` when the independent grids of a batched workload are
+    partitioned over `world` processes (contiguous blocks, sizes differ by at most one).
+    No data-path collective is needed: members never interact."""
+    if world < 1 or not (0 <= rank < world) or batch < 0:
+        raise ValueError("need world >= 1, 0 <= rank < world, batch >= 0")
+    base, extra = divmod(batch, world)
+    lo = rank * base + min(rank, extra)
+    return range(lo, lo + base + (1 if rank < extra else 0))
+
+
+def shard(p: dict, rank: int, world: int) -> dict:
+    """The sub-workload holding only this rank's members of a batched workload `p`."""
+    idx = list(shard_members(p["batch"], rank, world))
+    B = p["batch"]
+    q = copy.deepcopy(p)
+    q["batch"] = len(idx)
+    for k in ("g", "eta_or_u", "n_atoms", "delta", "kappa"):
+        q[k] = np.asarray(p[k], dtype=np.float64).reshape(B)[idx].copy()
+    if p.get("sched_amp") is not None:
+        sa = np.asarray(p["sched_amp"], dtype=np.float64)
+        L = len(p["sched_step"])
+        if sa.size == B * L and B > 1:
+            q["sched_amp"] = sa.reshape(B, L)[idx].copy()
+    if p.get("v_static") is not None and np.asarray(p["v_static"]).ndim == 3:
+        q["v_static"] = np.asarray(p["v_static"])[idx].copy()
+    if p.get("psi0") is not None and np.asarray(p["psi0"]).ndim == 3:
+        q["psi0"] = np.ascontiguousarray(np.asarray(p["psi0"])[idx])
+    return q
