@@ -37,10 +37,12 @@ struct gpe_plan {
 
     // device tables (typed by dtype)
     void *tw_x = nullptr, *tw_y = nullptr;
+    void *tw1_x = nullptr, *tw1_y = nullptr;
     void *kin_x = nullptr, *kin_y = nullptr;
     double kin_dt = 0.0;
     int kin_mode = -1;
     void *vx = nullptr, *vy = nullptr, *latx = nullptr, *laty = nullptr, *cavx = nullptr, *cavy = nullptr;
+    void *ytab = nullptr;
     void *g = nullptr;
     void *v2d = nullptr;
     size_t v2d_elems = 0;
@@ -126,6 +128,14 @@ template <typename T> gpe_status make_twiddles(gpe_plan *p) {
             re[m] = cos(ang); im[m] = sin(ang);
         }
         gpe_status s = upload_cplx<T>(p, ax == 0 ? &p->tw_x : &p->tw_y, re, im);
+        if (s != GPE_OK) return s;
+        const int m1 = n / 16;
+        for (int k = 0; k < 16; ++k)
+            for (int j = 0; j < m1; ++j) {
+                double a1 = -2.0 * kPi * (double)((long)k * j % n) / (double)n;
+                re[k * m1 + j] = cos(a1); im[k * m1 + j] = sin(a1);
+            }
+        s = upload_cplx<T>(p, ax == 0 ? &p->tw1_x : &p->tw1_y, re, im);
         if (s != GPE_OK) return s;
     }
     return GPE_OK;
@@ -314,8 +324,10 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     a.vx = (const T *)p->vx; a.vy = (const T *)p->vy;
     a.latx = (const T *)p->latx; a.laty = (const T *)p->laty;
     a.cavx = (const T *)p->cavx; a.cavy = (const T *)p->cavy;
+    a.ytab = (const T *)p->ytab;
     a.g = (const T *)p->g;
     a.tw_x = (const cx<T> *)p->tw_x; a.tw_y = (const cx<T> *)p->tw_y;
+    a.tw1_x = (const cx<T> *)p->tw1_x; a.tw1_y = (const cx<T> *)p->tw1_y;
     a.kin_xc = (const cx<T> *)p->kin_x; a.kin_yc = (const cx<T> *)p->kin_y;
     a.kin_xr = (const T *)p->kin_x; a.kin_yr = (const T *)p->kin_y;
     a.inv_p = (T)(1.0 / ((double)p->nx * (double)p->ny));
@@ -372,7 +384,7 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
             prof->e0.push_back(e0); prof->e1.push_back(e1); prof->which.push_back(w);
         }
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, p->stream));
-        GPE_CUDA(p, oy->row_fwd(a, imag, p->stream));
+        { static int dbg = getenv("GPE_DBG") ? atoi(getenv("GPE_DBG")) : 0; StepArgs<T, cx<T>> a2 = a; a2.flags |= dbg; GPE_CUDA(p, oy->row_fwd(a2, imag, p->stream)); }
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e1, p->stream));
         if (w == 1) GPE_CUDA(p, cudaEventRecord(e0, p->stream));
         GPE_CUDA(p, ox->col(a, imag, 0, p->stream));
@@ -536,6 +548,11 @@ template <typename T> gpe_status set_potential_impl(gpe_plan *p, const gpe_poten
     if ((s = upload_real<T>(p, &p->laty, ly)) != GPE_OK) return s;
     if ((s = upload_real<T>(p, &p->cavx, cxv)) != GPE_OK) return s;
     if ((s = upload_real<T>(p, &p->cavy, cyv)) != GPE_OK) return s;
+    {   // packed per-y table for the fused passes (zeros where a term is switched off)
+        std::vector<double> yt(4 * (size_t)ny, 0.0);
+        for (int j = 0; j < ny; ++j) { yt[4 * j] = hy[j]; yt[4 * j + 1] = ly[j]; yt[4 * j + 2] = cyv[j]; }
+        if ((s = upload_real<T>(p, &p->ytab, yt)) != GPE_OK) return s;
+    }
     p->h_g.assign(B, 0.0);
     if (d->g) {
         p->h_g.assign(d->g, d->g + B);
@@ -607,8 +624,8 @@ gpe_status gpe_plan_set_stream(gpe_plan *p, void *cuda_stream) {
 gpe_status gpe_plan_destroy(gpe_plan *p) {
     if (!p) return GPE_OK;
     cudaStreamSynchronize(p->stream);
-    void *bufs[] = {p->tw_x, p->tw_y, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
-                    p->g, p->v2d, p->st, p->partials, p->counters, p->nonfinite, p->d_sched_step,
+    void *bufs[] = {p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
+                    p->ytab, p->g, p->v2d, p->st, p->partials, p->counters, p->nonfinite, p->d_sched_step,
                     p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->scratch, p->obs_dev,
                     p->pop_dev, p->obsA_dev};
     for (void *b : bufs)

@@ -23,8 +23,27 @@ template <> struct Vec2<double> { using type = double2; };
 template <typename T> using cx = typename Vec2<T>::type;
 
 template <typename T> __device__ __forceinline__ cx<T> mk(T x, T y) { cx<T> r; r.x = x; r.y = y; return r; }
-template <typename C> __device__ __forceinline__ C cadd(C a, C b) { a.x += b.x; a.y += b.y; return a; }
-template <typename C> __device__ __forceinline__ C csub(C a, C b) { a.x -= b.x; a.y -= b.y; return a; }
+// complex64 sums use the packed fp32x2 adder of sm_100 (FADD2 / FFMA2: one issue slot for both
+// components; same rounding as two scalar adds).  GPE_PACKED_ADD=0 falls back to scalar adds.
+#ifndef GPE_PACKED_ADD
+#define GPE_PACKED_ADD 0
+#endif
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) {
+#if GPE_PACKED_ADD
+    return __fadd2_rn(a, b);
+#else
+    a.x += b.x; a.y += b.y; return a;
+#endif
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b) {
+#if GPE_PACKED_ADD
+    return __ffma2_rn(b, make_float2(-1.0f, -1.0f), a);
+#else
+    a.x -= b.x; a.y -= b.y; return a;
+#endif
+}
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { a.x += b.x; a.y += b.y; return a; }
+__device__ __forceinline__ double2 csub(double2 a, double2 b) { a.x -= b.x; a.y -= b.y; return a; }
 template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
     C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
 }
@@ -184,10 +203,14 @@ template <int N, int S, typename T> struct Fft1D {
 
     // in: v[a] = x[j + (N/16) a].  out: v[i*RL + r] = X[nat(j,i,r)] (unnormalised, e^{-i}).
     // All threads of the CTA must call this together (it contains __syncthreads()).
-    __device__ __forceinline__ static void fwd(C *v, C *sm, int j, const C *__restrict__ tw) {
+    // tw1[k * M1 + j] = exp(-2 pi i k j / N): the first-stage twiddles transposed so that the
+    // lanes of a warp (consecutive j) read consecutive addresses (tw[k * j] is a stride-k gather
+    // that costs up to 30 L1 wavefronts per load).
+    __device__ __forceinline__ static void fwd(C *v, C *sm, int j, const C *__restrict__ tw,
+                                               const C *__restrict__ tw1) {
         dft<16, -1, T>(v);
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], tw[k * j]);
+        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], tw1[k * M1 + j]);
 #pragma unroll
         for (int k = 0; k < 16; ++k) sm[phys(j + M1 * k)] = v[k];
         __syncthreads();
@@ -200,7 +223,8 @@ template <int N, int S, typename T> struct Fft1D {
 
     // exact mirror of fwd (unnormalised, e^{+i}): in: v[i*RL + r] = X[nat(j,i,r)],
     // out: v[a] = sum_k X[k] e^{+2 pi i k n / N} at n = j + (N/16) a.
-    __device__ __forceinline__ static void inv(C *v, C *sm, int j, const C *__restrict__ tw) {
+    __device__ __forceinline__ static void inv(C *v, C *sm, int j, const C *__restrict__ tw,
+                                               const C *__restrict__ tw1) {
         if constexpr (NST == 3) {
             stage_inv<R3, M1 / R2, true>(v, sm, j, tw);
             __syncthreads();
@@ -212,7 +236,7 @@ template <int N, int S, typename T> struct Fft1D {
 #pragma unroll
         for (int k = 0; k < 16; ++k) v[k] = sm[phys(j + M1 * k)];
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], tw[k * j]);
+        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], tw1[k * M1 + j]);
         dft<16, +1, T>(v);
     }
 };

@@ -10,6 +10,9 @@
 #include "gpe_fft.cuh"
 #include "gpe_types.h"
 
+#ifndef GPE_ROW_MINB
+#define GPE_ROW_MINB 3
+#endif
 namespace gpe {
 
 // ---------------------------------------------------------------- launch geometry
@@ -149,84 +152,200 @@ __device__ __forceinline__ void sincosm1_t(double w, double *s, double *cm1) {
     *cm1 = -2.0 * sh * sh;
 }
 
-template <typename T, bool IMAG>
-__device__ __forceinline__ T potential_factor(cx<T> &z, T V, T g, T half_dt) {
-    T d = z.x * z.x + z.y * z.y;
-    T w = (V + g * d) * half_dt;
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { using type = float4; };
+template <> struct Vec4<double> { using type = double4; };
+
+// General-argument (cos w - 1, sin w) for the rare large phase: kept out of line so that the
+// library range reduction is not inlined sixteen times into every pass.
+static __device__ __noinline__ void sincosm1_general(float w, float *s, float *cm1) {
+    float sh, ch;
+    sincosf(0.5f * w, &sh, &ch);
+    *s = 2.0f * sh * ch;
+    *cm1 = -2.0f * sh * sh;
+}
+// |w| <= 0.5: odd/even Taylor polynomials, error < 1 ulp of the result
+__device__ __forceinline__ void sincosm1_small(float w, float *s, float *cm1) {
+    const float w2 = w * w;
+    float ps = fmaf(w2, 2.7557319e-6f, -1.9841270e-4f);
+    ps = fmaf(w2, ps, 8.3333333e-3f);
+    ps = fmaf(w2, ps, -1.6666667e-1f);
+    *s = fmaf(w * w2, ps, w);
+    float pc = fmaf(w2, 2.4801587e-5f, -1.3888889e-3f);
+    pc = fmaf(w2, pc, 4.1666667e-2f);
+    pc = fmaf(w2, pc, -0.5f);
+    *cm1 = w2 * pc;
+}
+
+// Potential half-step on the 16 points of one thread (rows a1 / a5), y_k = j + M1 k:
+//   psi <- psi * exp(-s (V + g|psi|^2) dt/2),  V = vrow + vy[y] + A cos^2(k_l y) + crow cos(k_c y) [+ V2d]
+// (vrow = vx[i] + A cos^2(k_l x_i), crow = C_n cos(k_c x_i)).  All table loads of the 16 points
+// are issued back to back (one 4-vector per point), the angles are formed, and only then is the
+// phase applied -- with ONE warp-uniform decision between the small-angle polynomial and the
+// general path, so the common case has no per-point branch at all.
+// REDUCE: also returns sum |psi_new|^2 and sum cos(k_c y) |psi_new|^2 over the 16 points.
+template <typename T, bool IMAG, bool REDUCE, int M1>
+__device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<T, cx<T>> &a, int b, int i, int j,
+                                                 T scale, T A, T Cc, T &sn, T &st) {
+    using V4 = typename Vec4<T>::type;
+    const int flags = a.flags;
+    T vrow = T(0);
+    if (flags & F_HAS_SEP) vrow += a.vx[i];
+    if (flags & F_LAT_X) vrow += A * a.latx[i];
+    const T crow = (flags & F_CAVITY) ? Cc * a.cavx[i] : T(0);
+    const T Ay = (flags & F_LAT_Y) ? A : T(0);
+    const T g = (flags & F_HAS_G) ? a.g[b] : T(0);
+    const T hdt = a.half_dt;
+    const V4 *__restrict__ yt = reinterpret_cast<const V4 *>(a.ytab);
+    T w[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const V4 t = yt[j + M1 * k];
+        if constexpr (IMAG) { v[k].x *= scale; v[k].y *= scale; }  // the lazy scale is 1 in real time
+        const T d = v[k].x * v[k].x + v[k].y * v[k].y;
+        const T V = fma(crow, t.z, fma(Ay, t.y, vrow + t.x));
+        w[k] = fma(g, d, V) * hdt;
+    }
+    if (flags & F_HAS_V2D) {
+        const T *__restrict__ v2 = a.v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * a.nx * a.ny : 0) + (size_t)i * a.ny;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) w[k] = fma(v2[j + M1 * k], hdt, w[k]);
+    }
     if constexpr (IMAG) {
-        T e = exp_t(-w);
-        z.x *= e; z.y *= e;
-        return d * e * e;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const T e = exp_t(-w[k]);
+            v[k].x *= e; v[k].y *= e;
+        }
+    } else if constexpr (sizeof(T) == 4) {
+        // psi <- psi + psi * (cos w - 1 - i sin w), three warp-uniform tiers by the largest |w|:
+        //   |w| <= 2^-5: sin w = w - w^3/6, cos w - 1 = -w^2/2 + w^4/24 (truncation < 2^-27 relative)
+        //   |w| <= 0.5 : degree-9 / degree-8 polynomials;   else: library range reduction
+        float wmax = 0.f;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) wmax = fmaxf(wmax, fabsf(w[k]));
+        if (__all_sync(0xffffffffu, wmax <= 0.03125f)) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const float w2 = w[k] * w[k];
+                const float sn_ = -fmaf(w[k] * w2, -1.6666667e-1f, w[k]);   // sin(-w)
+                const float cm1 = w2 * fmaf(w2, 4.1666667e-2f, -0.5f);
+                const float nx_ = fmaf(v[k].x, cm1, fmaf(-v[k].y, sn_, v[k].x));
+                const float ny_ = fmaf(v[k].x, sn_, fmaf(v[k].y, cm1, v[k].y));
+                v[k].x = nx_; v[k].y = ny_;
+            }
+        } else if (__all_sync(0xffffffffu, wmax <= 0.5f)) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                float sn_, cm1;
+                sincosm1_small(-w[k], &sn_, &cm1);
+                const float nx_ = fmaf(v[k].x, cm1, fmaf(-v[k].y, sn_, v[k].x));
+                const float ny_ = fmaf(v[k].x, sn_, fmaf(v[k].y, cm1, v[k].y));
+                v[k].x = nx_; v[k].y = ny_;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                float sn_, cm1;
+                sincosm1_general(-w[k], &sn_, &cm1);
+                const float nx_ = fmaf(v[k].x, cm1, fmaf(-v[k].y, sn_, v[k].x));
+                const float ny_ = fmaf(v[k].x, sn_, fmaf(v[k].y, cm1, v[k].y));
+                v[k].x = nx_; v[k].y = ny_;
+            }
+        }
     } else {
-        T s, cm1;
-        sincosm1_t(-w, &s, &cm1);
-        const T tx = fma(z.x, cm1, -(z.y * s)), ty = fma(z.x, s, z.y * cm1);
-        z.x += tx; z.y += ty;
-        return d;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            T sn_, cm1;
+            sincosm1_t(-w[k], &sn_, &cm1);
+            const T tx = fma(v[k].x, cm1, -(v[k].y * sn_)), ty = fma(v[k].x, sn_, v[k].y * cm1);
+            v[k].x += tx; v[k].y += ty;
+        }
+    }
+    if constexpr (REDUCE) {
+        sn = T(0); st = T(0);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const T d = v[k].x * v[k].x + v[k].y * v[k].y;
+            sn += d;
+            if (flags & F_CAVITY) st = fma(d, a.ytab[4 * (j + M1 * k) + 2], st);
+        }
     }
 }
 
-template <typename T, typename C> struct RowPot {
-    T vrow, crow, A, g, half_dt;
-    const T *v2d_row, *vy, *laty, *cavy;
-    int flags;
-    __device__ __forceinline__ void init(const StepArgs<T, C> &a, int b, int i, T A_, T C_) {
-        flags = a.flags;
-        A = A_;
-        vrow = T(0);
-        if (flags & F_HAS_SEP) vrow += a.vx[i];
-        if (flags & F_LAT_X) vrow += A_ * a.latx[i];
-        crow = (flags & F_CAVITY) ? C_ * a.cavx[i] : T(0);
-        g = (flags & F_HAS_G) ? a.g[b] : T(0);
-        half_dt = a.half_dt;
-        v2d_row = nullptr;
-        if (flags & F_HAS_V2D)
-            v2d_row = a.v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * a.nx * a.ny : 0) + (size_t)i * a.ny;
-        vy = a.vy; laty = a.laty; cavy = a.cavy;
-    }
-    __device__ __forceinline__ T at(int y) const {
-        T V = vrow;
-        if (flags & F_HAS_SEP) V += vy[y];
-        if (flags & F_LAT_Y) V += A * laty[y];
-        if (flags & F_CAVITY) V += crow * cavy[y];
-        if (flags & F_HAS_V2D) V += v2d_row[y];
-        return V;
-    }
-};
+// ---------------------------------------------------------------- row staging (passes A and C)
+// The row passes are persistent: a CTA walks over groups of RPC rows (group g, g + gridDim.x, ...)
+// and fetches the NEXT group into a shared-memory stage with cp.async (16-byte chunks, L1
+// bypassed) while it computes the current one, so the L2 latency of the row loads -- half of
+// every warp's lifetime in the first version (profiles/r01_baseline.md) -- is off the critical
+// path.  STAGED = false keeps the direct register loads (complex128: the stage would halve the
+// occupancy of an ALU-bound kernel).
+#ifndef GPE_ROW_STAGE
+#define GPE_ROW_STAGE 0
+#endif
+template <typename T> struct RowStage { static constexpr bool on = GPE_ROW_STAGE && sizeof(T) == 4; };
+
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// copies the `bytes` (multiple of 16) at gsrc into the stage, all threads of the CTA
+__device__ __forceinline__ void stage_fetch(unsigned char *stage, const void *gsrc, int bytes) {
+    const unsigned char *g = reinterpret_cast<const unsigned char *>(gsrc);
+    for (int q = threadIdx.x * 16; q < bytes; q += blockDim.x * 16) cp_async16(stage + q, g + q);
+    cp_async_commit();
+}
 
 // ---------------------------------------------------------------- pass A
 template <typename T, int NY, bool IMAG>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS) k_row_fwd(const StepArgs<T, cx<T>> a) {
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : 1)) k_row_fwd(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, T>;
     using G = RowGeom<NY>;
+    constexpr bool STAGED = RowStage<T>::on;
+    constexpr int GROUP_BYTES = (int)sizeof(C) * G::RPC * NY;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
+    unsigned char *stage = smem_raw + sizeof(C) * G::RPC * F::SLOTS;
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
-    const long row = (long)blockIdx.x * G::RPC + r;
-    const int b = (int)(row / a.nx), i = (int)(row % a.nx);
     C *sm = smem + r * F::SLOTS;
-    const C *src = a.src + row * NY;
-    C *dst = a.dst + row * NY;
-    C v[16];
+    const long ngroups = (long)a.batch * a.nx / G::RPC;
+    if (STAGED && (long)blockIdx.x < ngroups) stage_fetch(stage, a.src + (long)blockIdx.x * G::RPC * NY, GROUP_BYTES);
+    for (long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        const long row = grp * G::RPC + r;
+        const int b = (int)(row / a.nx), i = (int)(row % a.nx);
+        C *dst = a.dst + row * NY;
+        C v[16];
+        if constexpr (STAGED) {
+            cp_async_wait_all();
+            __syncthreads();
+            const C *st_row = reinterpret_cast<const C *>(stage) + r * NY;
 #pragma unroll
-    for (int k = 0; k < 16; ++k) v[k] = src[j + F::M1 * k];
-    if (!(a.flags & F_NO_POT)) {
-        const MemberState &ms = a.fin.st[b];
-        const T scale = (T)ms.scale;
-        RowPot<T, C> P;
-        P.init(a, b, i, (T)ms.A, (T)ms.C);
+            for (int k = 0; k < 16; ++k) v[k] = st_row[j + F::M1 * k];
+            __syncthreads();
+            if (grp + gridDim.x < ngroups) stage_fetch(stage, a.src + (grp + gridDim.x) * G::RPC * NY, GROUP_BYTES);
+        } else {
+            const C *src = a.src + row * NY;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            v[k].x *= scale; v[k].y *= scale;
-            potential_factor<T, IMAG>(v[k], P.at(j + F::M1 * k), P.g, P.half_dt);
+            for (int k = 0; k < 16; ++k) v[k] = src[j + F::M1 * k];
         }
+        if (!(a.flags & F_NO_POT)) {
+            const MemberState &ms = a.fin.st[b];
+            T sn, st;
+            potential_step16<T, IMAG, false, F::M1>(v, a, b, i, j, (T)ms.scale, (T)ms.A, (T)ms.C, sn, st);
+        }
+        if (!(a.flags & 256)) F::fwd(v, sm, j, a.tw_y, a.tw1_y);
+        if (!(a.flags & 512) || v[0].x == 12345.678f) {
+#pragma unroll
+        for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) dst[F::nat(j, ii, rr)] = v[ii * F::RL + rr];
+        }
+        if constexpr (!STAGED) __syncthreads();
     }
-    F::fwd(v, sm, j, a.tw_y);
-#pragma unroll
-    for (int ii = 0; ii < F::GL; ++ii)
-#pragma unroll
-        for (int rr = 0; rr < F::RL; ++rr) dst[F::nat(j, ii, rr)] = v[ii * F::RL + rr];
 }
 
 // ---------------------------------------------------------------- pass B
@@ -249,7 +368,7 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<
     C v[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) v[k] = src[(size_t)(j + F::M1 * k) * ny];
-    F::fwd(v, sm, j, a.tw_x);
+    F::fwd(v, sm, j, a.tw_x, a.tw1_x);
     if constexpr (MODE == 1) {
 #pragma unroll
         for (int ii = 0; ii < F::GL; ++ii)
@@ -287,7 +406,7 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<
                     z.x = ox; z.y = oy;
                 }
         }
-        F::inv(v, sm, j, a.tw_x);
+        F::inv(v, sm, j, a.tw_x, a.tw1_x);
 #pragma unroll
         for (int k = 0; k < 16; ++k) dst[(size_t)(j + F::M1 * k) * ny] = v[k];
     }
@@ -295,48 +414,71 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<
 
 // ---------------------------------------------------------------- pass C
 template <typename T, int NY, bool IMAG>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS) k_row_inv(const StepArgs<T, cx<T>> a) {
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : 1)) k_row_inv(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, T>;
     using G = RowGeom<NY>;
+    constexpr bool STAGED = RowStage<T>::on;
+    constexpr int GROUP_BYTES = (int)sizeof(C) * G::RPC * NY;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
+    unsigned char *stage = smem_raw + sizeof(C) * G::RPC * F::SLOTS;
     __shared__ double red[64];
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
-    const long row = (long)blockIdx.x * G::RPC + r;
-    const int b = (int)(row / a.nx), i = (int)(row % a.nx);
     C *sm = smem + r * F::SLOTS;
-    const C *src = a.src + row * NY;
-    C *dst = a.dst + row * NY;
-    C v[16];
+    const long ngroups = (long)a.batch * a.nx / G::RPC;
+    const int gpm = a.nx / G::RPC;  // groups per member: all rows of a group belong to one member
+    if (STAGED && (long)blockIdx.x < ngroups) stage_fetch(stage, a.src + (long)blockIdx.x * G::RPC * NY, GROUP_BYTES);
+    for (long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+        const long row = grp * G::RPC + r;
+        const int b = (int)(row / a.nx), i = (int)(row % a.nx);
+        C *dst = a.dst + row * NY;
+        C v[16];
+        if constexpr (STAGED) {
+            cp_async_wait_all();
+            __syncthreads();
+            const C *st_row = reinterpret_cast<const C *>(stage) + r * NY;
 #pragma unroll
-    for (int ii = 0; ii < F::GL; ++ii)
+            for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
-        for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = src[F::nat(j, ii, rr)];
-    F::inv(v, sm, j, a.tw_y);
-    const MemberState &ms = a.fin.st[b];
-    RowPot<T, C> P;
-    P.init(a, b, i, (T)ms.A, (T)ms.C);
-    T sn = T(0), st = T(0);
+                for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = st_row[F::nat(j, ii, rr)];
+            __syncthreads();
+            if (grp + gridDim.x < ngroups) stage_fetch(stage, a.src + (grp + gridDim.x) * G::RPC * NY, GROUP_BYTES);
+        } else {
+            const C *src = a.src + row * NY;
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-        const int y = j + F::M1 * k;
-        T d = potential_factor<T, IMAG>(v[k], P.at(y), P.g, P.half_dt);
-        sn += d;
-        if (a.flags & F_CAVITY) st += d * a.cavy[y];
-        dst[y] = v[k];
+            for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+                for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = src[F::nat(j, ii, rr)];
+        }
+        F::inv(v, sm, j, a.tw_y, a.tw1_y);
+        const MemberState &ms = a.fin.st[b];
+        T sn, st;
+        potential_step16<T, IMAG, true, F::M1>(v, a, b, i, j, T(1), (T)ms.A, (T)ms.C, sn, st);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) dst[j + F::M1 * k] = v[k];
+        double dn = (double)sn, dt_ = (a.flags & F_CAVITY) ? (double)st * (double)a.cavx[i] : 0.0;
+        block_reduce_and_finalize(a.fin, b, (int)(grp % gpm), dn, dt_, red);
+        if constexpr (!STAGED) __syncthreads();
     }
-    double dn = (double)sn, dt_ = (a.flags & F_CAVITY) ? (double)st * (double)a.cavx[i] : 0.0;
-    // all rows of a CTA belong to one member (nx is a multiple of RPC)
-    const int cta_in_member = (int)(blockIdx.x % (unsigned)(a.nx / G::RPC));
-    block_reduce_and_finalize(a.fin, b, cta_in_member, dn, dt_, red);
 }
 
 // ---------------------------------------------------------------- launchers (one per T, N)
 template <typename T, int N> struct Launch {
     using C = cx<T>;
     using A = StepArgs<T, C>;
-    static size_t row_smem() { return sizeof(C) * RowGeom<N>::RPC * Fft1D<N, 1, T>::SLOTS; }
+    static size_t row_smem() {
+        return sizeof(C) * RowGeom<N>::RPC * Fft1D<N, 1, T>::SLOTS + (RowStage<T>::on ? sizeof(C) * RowGeom<N>::RPC * N : 0);
+    }
+    // persistent when staged: GPE_ROW_MINB CTAs per SM walk over the row groups
+    static unsigned row_grid(const A &a) {
+        long groups = (long)a.batch * a.nx / RowGeom<N>::RPC;
+        if (!RowStage<T>::on) return (unsigned)groups;
+        static int sms = 0;
+        if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
+        long cap = (long)sms * GPE_ROW_MINB;
+        return (unsigned)(groups < cap ? groups : cap);
+    }
     static size_t col_smem() { return sizeof(C) * ColGeom<T, N>::W * Fft1D<N, 1, T>::SLOTS; }
 
     template <typename K> static cudaError_t prep(K kern, size_t smem) {
@@ -346,7 +488,7 @@ template <typename T, int N> struct Launch {
     }
     // ny == N
     static cudaError_t row_fwd(const A &a, bool imag, cudaStream_t s) {
-        dim3 grid((unsigned)((long)a.batch * a.nx / RowGeom<N>::RPC)), block(RowGeom<N>::THREADS);
+        dim3 grid(row_grid(a)), block(RowGeom<N>::THREADS);
         cudaError_t e;
         if (imag) {
             if ((e = prep(k_row_fwd<T, N, true>, row_smem())) != cudaSuccess) return e;
@@ -358,7 +500,7 @@ template <typename T, int N> struct Launch {
         return cudaGetLastError();
     }
     static cudaError_t row_inv(const A &a, bool imag, cudaStream_t s) {
-        dim3 grid((unsigned)((long)a.batch * a.nx / RowGeom<N>::RPC)), block(RowGeom<N>::THREADS);
+        dim3 grid(row_grid(a)), block(RowGeom<N>::THREADS);
         cudaError_t e;
         if (imag) {
             if ((e = prep(k_row_inv<T, N, true>, row_smem())) != cudaSuccess) return e;

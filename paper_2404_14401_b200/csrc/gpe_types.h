@@ -58,9 +58,11 @@ template <typename T, typename C> struct StepArgs {
     const T *vx, *vy;              // separable static part
     const T *latx, *laty;          // cos^2(k_l x_i), cos^2(k_l y_j)
     const T *cavx, *cavy;          // cos(k_c x_i), cos(k_c y_j)
+    const T *ytab;                 // [ny][4] = {vy[j], cos^2(k_l y_j), cos(k_c y_j), 0}: one 4-vector load per point
     const T *g;                    // [batch]
     T half_dt;                     // dt/2
     const C *tw_x, *tw_y;          // exp(-2 pi i m / nx), exp(-2 pi i m / ny)
+    const C *tw1_x, *tw1_y;        // first-stage twiddles transposed: [16][n/16], exp(-2 pi i k j / n)
     const C *kin_xc, *kin_yc;      // real time: (exp(-i kx^2 dt/2) - 1)/(nx ny), exp(-i ky^2 dt/2) - 1
     T inv_p;                       // 1/(nx ny)
     const T *kin_xr, *kin_yr;      // imaginary time: exp(-kx^2 dt/2)/(nx ny), exp(-ky^2 dt/2)
