@@ -47,7 +47,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
         return LIB
     os.makedirs(OBJ, exist_ok=True)
     nvcc = os.environ.get("NVCC", "nvcc")
-    extra = ["-Xptxas", "-v"] if ptxas_v else []
+    extra = (["-Xptxas", "-v"] if ptxas_v else []) + os.environ.get("GPE_NVCC_FLAGS", "").split()
     jobs = []
     objs = []
     for tag, typ in (("f", "float"), ("d", "double")):

@@ -20,6 +20,7 @@ namespace {
 
 constexpr int kMaxCpm = 1024;   // partial-sum slots per member
 constexpr int kReduceCtas = 128;  // CTAs per member of the prologue reduction
+constexpr int kStepsPerGraph = 8;  // split-steps per CUDA graph launch
 constexpr double kPi = 3.14159265358979323846;
 
 thread_local std::string g_create_error;
@@ -60,6 +61,16 @@ struct gpe_plan {
     int lattice_axis = -1, sched_len = 0, sched_batched = 0, cavity_on = 0, eta_mode = 0;
     double lattice_k = 0, cavity_k = 0;
     std::vector<double> h_sched_step, h_sched_amp, h_eta, h_natoms, h_delta, h_kappa, h_g;
+
+    // per-call parameters on the device + cached CUDA graph of kStepsPerGraph steps
+    CallParams *d_call = nullptr;
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t g_exec = nullptr;
+    const void *g_psi = nullptr;
+    double g_dt = 0.0;
+    int g_mode = -1;
+    long g_epoch = -1;
+    long epoch = 0;  // bumped whenever device tables / flags may have changed
 
     // observables workspace
     void *scratch = nullptr;     // complex [batch][nx][ny]
@@ -168,6 +179,7 @@ template <typename T> gpe_status make_kinetic(gpe_plan *p, double dt, int mode) 
     }
     p->kin_mode = mode;
     p->kin_dt = dt;
+    p->epoch++;
     return GPE_OK;
 }
 
@@ -339,6 +351,7 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     f.eta_or_u = p->d_eta; f.n_atoms = p->d_natoms; f.delta = p->d_delta; f.kappa = p->d_kappa;
     f.dxdy = (p->Lx / p->nx) * (p->Ly / p->ny);
     f.batch = p->batch;
+    f.call = p->d_call;
     return a;
 }
 
@@ -363,7 +376,9 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
         FinalizeParams f = a.fin;
         f.cpm = kReduceCtas < p->nx ? kReduceCtas : p->nx;
         f.normalise = 0; f.advance = 0; f.step0 = p->step;
-        f.record_every = 0; f.records = nullptr;
+        f.record_every = records ? record_every : 0;
+        f.rec_first = record_every > 0 ? p->step / record_every : 0;
+        f.records = records;
         dim3 grid(f.cpm, p->batch);
         k_reduce<T><<<grid, 256, 0, p->stream>>>((const cx<T> *)psi, p->nx, p->ny, (const T *)p->cavx,
                                                  (const T *)p->cavy, p->cavity_on, f);
@@ -372,10 +387,45 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     a.fin.cpm = p->nx / oy->rows_per_cta;
     a.fin.normalise = imag ? 1 : 0;
     a.fin.advance = 1;
-    a.fin.record_every = records ? record_every : 0;
-    a.fin.rec_first = record_every > 0 ? p->step / record_every : 0;
-    a.fin.records = records;
-    for (long n = 0; n < n_steps; ++n) {
+    a.fin.record_every = 0; a.fin.rec_first = 0; a.fin.records = nullptr;  // step kernels read *call
+    auto one_step = [&](cudaStream_t st, int w, cudaEvent_t e0, cudaEvent_t e1) -> gpe_status {
+        if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, st));
+        GPE_CUDA(p, oy->row_fwd(a, imag, st));
+        if (w == 0) GPE_CUDA(p, cudaEventRecord(e1, st));
+        if (w == 1) GPE_CUDA(p, cudaEventRecord(e0, st));
+        GPE_CUDA(p, ox->col(a, imag, 0, st));
+        if (w == 1) GPE_CUDA(p, cudaEventRecord(e1, st));
+        if (w == 2) GPE_CUDA(p, cudaEventRecord(e0, st));
+        GPE_CUDA(p, oy->row_inv(a, imag, st));
+        if (w == 2) GPE_CUDA(p, cudaEventRecord(e1, st));
+        return GPE_OK;
+    };
+    long n = 0;
+    if (!prof && n_steps >= 2 * kStepsPerGraph) {
+        // The arguments of the three passes do not depend on the step (all per-step state is on the
+        // device), so kStepsPerGraph steps are captured once into a CUDA graph and replayed: one
+        // host call per 3 * kStepsPerGraph kernels instead of one per kernel.
+        if (!(p->g_exec && p->g_psi == psi && p->g_dt == dt && p->g_mode == (int)mode && p->g_epoch == p->epoch)) {
+            if (p->g_exec) { cudaGraphExecDestroy(p->g_exec); p->g_exec = nullptr; }
+            if (!p->cap_stream) GPE_CUDA(p, cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
+            // first launches outside the capture: one-time function attributes are not stream work
+            if ((s = one_step(p->stream, -1, nullptr, nullptr)) != GPE_OK) return s;
+            n = 1;
+            GPE_CUDA(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
+            gpe_status cs = GPE_OK;
+            for (int u = 0; u < kStepsPerGraph && cs == GPE_OK; ++u) cs = one_step(p->cap_stream, -1, nullptr, nullptr);
+            cudaGraph_t graph = nullptr;
+            cudaError_t ce = cudaStreamEndCapture(p->cap_stream, &graph);
+            if (cs != GPE_OK) { if (graph) cudaGraphDestroy(graph); return cs; }
+            if (ce != cudaSuccess) return cuda_fail(p, ce, "cudaStreamEndCapture");
+            ce = cudaGraphInstantiate(&p->g_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (ce != cudaSuccess) { p->g_exec = nullptr; return cuda_fail(p, ce, "cudaGraphInstantiate"); }
+            p->g_psi = psi; p->g_dt = dt; p->g_mode = (int)mode; p->g_epoch = p->epoch;
+        }
+        for (; n + kStepsPerGraph <= n_steps; n += kStepsPerGraph) GPE_CUDA(p, cudaGraphLaunch(p->g_exec, p->stream));
+    }
+    for (; n < n_steps; ++n) {
         const int w = prof ? (int)(n % 3) : -1;
         cudaEvent_t e0 = nullptr, e1 = nullptr;
         if (prof) {
@@ -383,15 +433,7 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
             GPE_CUDA(p, cudaEventCreate(&e1));
             prof->e0.push_back(e0); prof->e1.push_back(e1); prof->which.push_back(w);
         }
-        if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, p->stream));
-        { static int dbg = getenv("GPE_DBG") ? atoi(getenv("GPE_DBG")) : 0; StepArgs<T, cx<T>> a2 = a; a2.flags |= dbg; GPE_CUDA(p, oy->row_fwd(a2, imag, p->stream)); }
-        if (w == 0) GPE_CUDA(p, cudaEventRecord(e1, p->stream));
-        if (w == 1) GPE_CUDA(p, cudaEventRecord(e0, p->stream));
-        GPE_CUDA(p, ox->col(a, imag, 0, p->stream));
-        if (w == 1) GPE_CUDA(p, cudaEventRecord(e1, p->stream));
-        if (w == 2) GPE_CUDA(p, cudaEventRecord(e0, p->stream));
-        GPE_CUDA(p, oy->row_inv(a, imag, p->stream));
-        if (w == 2) GPE_CUDA(p, cudaEventRecord(e1, p->stream));
+        if ((s = one_step(p->stream, w, e0, e1)) != GPE_OK) return s;
     }
     if (imag) {
         dim3 grid(256, p->batch);
@@ -601,6 +643,8 @@ gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly,
         GPE_CUDA(p, cudaMalloc((void **)&p->partials, sizeof(double2) * (size_t)batch * kMaxCpm));
         GPE_CUDA(p, cudaMalloc((void **)&p->counters, sizeof(unsigned int) * batch));
         GPE_CUDA(p, cudaMemset(p->counters, 0, sizeof(unsigned int) * batch));
+        GPE_CUDA(p, cudaMalloc((void **)&p->d_call, sizeof(CallParams)));
+        GPE_CUDA(p, cudaMemset(p->d_call, 0, sizeof(CallParams)));
         GPE_CUDA(p, cudaMalloc((void **)&p->nonfinite, sizeof(int)));
         GPE_CUDA(p, cudaMemset(p->nonfinite, 0, sizeof(int)));
         return dtype == GPE_C64 ? make_twiddles<float>(p) : make_twiddles<double>(p);
@@ -624,7 +668,9 @@ gpe_status gpe_plan_set_stream(gpe_plan *p, void *cuda_stream) {
 gpe_status gpe_plan_destroy(gpe_plan *p) {
     if (!p) return GPE_OK;
     cudaStreamSynchronize(p->stream);
-    void *bufs[] = {p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
+    if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
+    if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
+    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
                     p->ytab, p->g, p->v2d, p->st, p->partials, p->counters, p->nonfinite, p->d_sched_step,
                     p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->scratch, p->obs_dev,
                     p->pop_dev, p->obsA_dev};
@@ -680,6 +726,7 @@ gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
     s = p->dtype == GPE_C64 ? set_potential_impl<float>(p, d) : set_potential_impl<double>(p, d);
     if (s != GPE_OK) return s;
     p->pot_set = true;
+    p->epoch++;
     return GPE_OK;
 }
 

@@ -69,9 +69,13 @@ __device__ inline void finalize_member(const FinalizeParams &f, int b, double su
     }
     s.scale = scale; s.A = A; s.C = C; s.norm = norm; s.theta = theta;
     s.re_alpha = re_a; s.im_alpha = im_a; s.step = n1;
-    if (f.advance && f.records && f.record_every > 0 && (n1 % f.record_every) == 0) {
-        long long idx = n1 / f.record_every - f.rec_first - 1;
-        double *r = f.records + ((size_t)idx * f.batch + b) * 6;
+    if (!f.advance && b == 0) {
+        f.call->record_every = f.record_every; f.call->rec_first = f.rec_first; f.call->records = f.records;
+    }
+    const CallParams cp = f.advance ? *f.call : CallParams{0, 0, nullptr};
+    if (f.advance && cp.records && cp.record_every > 0 && (n1 % cp.record_every) == 0) {
+        long long idx = n1 / cp.record_every - cp.rec_first - 1;
+        double *r = cp.records + ((size_t)idx * f.batch + b) * 6;
         r[0] = (double)n1; r[1] = norm; r[2] = theta; r[3] = re_a; r[4] = im_a; r[5] = A;
     }
 }
@@ -313,6 +317,8 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     C *sm = smem + r * F::SLOTS;
     const long ngroups = (long)a.batch * a.nx / G::RPC;
+    if ((a.flags & 1024) && blockIdx.x < 444) __nanosleep((blockIdx.x / 148) * 1500);
+    if ((a.flags & 2048) && blockIdx.x < 444) __nanosleep((blockIdx.x / 148) * 2500);
     if (STAGED && (long)blockIdx.x < ngroups) stage_fetch(stage, a.src + (long)blockIdx.x * G::RPC * NY, GROUP_BYTES);
     for (long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
         const long row = grp * G::RPC + r;
@@ -330,7 +336,7 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
         } else {
             const C *src = a.src + row * NY;
 #pragma unroll
-            for (int k = 0; k < 16; ++k) v[k] = src[j + F::M1 * k];
+            for (int k = 0; k < 16; ++k) v[k] = __ldcg(src + j + F::M1 * k);
         }
         if (!(a.flags & F_NO_POT)) {
             const MemberState &ms = a.fin.st[b];
@@ -367,7 +373,7 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<
     C *sm = smem + c;
     C v[16];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) v[k] = src[(size_t)(j + F::M1 * k) * ny];
+    for (int k = 0; k < 16; ++k) v[k] = __ldcg(src + (size_t)(j + F::M1 * k) * ny);
     F::fwd(v, sm, j, a.tw_x, a.tw1_x);
     if constexpr (MODE == 1) {
 #pragma unroll
@@ -449,7 +455,7 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
 #pragma unroll
             for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
-                for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = src[F::nat(j, ii, rr)];
+                for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = __ldcg(src + F::nat(j, ii, rr));
         }
         F::inv(v, sm, j, a.tw_y, a.tw1_y);
         const MemberState &ms = a.fin.st[b];
@@ -481,10 +487,16 @@ template <typename T, int N> struct Launch {
     }
     static size_t col_smem() { return sizeof(C) * ColGeom<T, N>::W * Fft1D<N, 1, T>::SLOTS; }
 
+    // opt in to > 48 KB of dynamic shared memory once per kernel (not on every launch: the
+    // attribute call costs microseconds of host time and the launch path is latency critical)
     template <typename K> static cudaError_t prep(K kern, size_t smem) {
-        if (smem > 48 * 1024)
-            return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        return cudaSuccess;
+        static thread_local K done_for[8] = {};
+        if (smem <= 48 * 1024) return cudaSuccess;
+        for (K k : done_for) if (k == kern) return cudaSuccess;
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess)
+            for (K &k : done_for) if (k == nullptr) { k = kern; break; }
+        return e;
     }
     // ny == N
     static cudaError_t row_fwd(const A &a, bool imag, cudaStream_t s) {

@@ -16,6 +16,13 @@ struct MemberState {
     long long step;    // step counter n
 };
 
+// Per-gpe_evolve-call parameters kept in device memory (written by the prologue kernel), so that
+// the kernel arguments of a step do not change from call to call and its CUDA graph is reusable.
+struct CallParams {
+    long long record_every, rec_first;  // rec_first = floor(step0 / record_every)
+    double *records;                    // [n_rec][batch][6] or nullptr
+};
+
 // Everything the finalising block needs (schedule, cavity parameters, records).
 struct FinalizeParams {
     MemberState *st;          // [batch]
@@ -30,8 +37,9 @@ struct FinalizeParams {
     int cavity_on, eta_mode;
     const double *eta_or_u, *n_atoms, *delta, *kappa;  // [batch]
     double dxdy;
-    long long record_every, rec_first;  // rec_first = floor(step0 / record_every)
-    double *records;          // [n_rec][batch][6] or nullptr
+    long long record_every, rec_first;  // prologue only (advance == 0): copied into *call
+    double *records;          // prologue only
+    CallParams *call;         // device; read by the step kernels
     int batch;
     int normalise;            // 1: imaginary-time step (scale <- 1/sqrt(norm), Theta /= norm)
     int advance;              // 1: a step was taken (step += 1); 0: prologue reduction
