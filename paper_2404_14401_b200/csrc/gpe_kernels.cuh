@@ -7,6 +7,8 @@
 //                     (a0: A_{n+1}, C_{n+1}; a7: scale; a8: record) -- no host round trip.
 // PAPER.md:62-76 (Eqs. 2-4), :116 (renormalisation), :183-186 (Eq. 14).
 #pragma once
+#include <cstdlib>
+#include <utility>
 #include "gpe_fft.cuh"
 #include "gpe_types.h"
 
@@ -14,6 +16,25 @@
 #define GPE_ROW_MINB 3
 #endif
 namespace gpe {
+
+// ---------------------------------------------------------------- programmatic dependent launch
+// Small grids launch every pass with cudaLaunchAttributeProgrammaticStreamSerialization: its CTAs
+// may be scheduled while the previous pass drains (launch latency and prologue off the critical
+// path) and block in pdl_wait() until that pass has completed and its writes are visible.  Without
+// the attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl, Args &&...args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, std::forward<Args>(args)...);
+}
 
 // ---------------------------------------------------------------- launch geometry
 template <int N> struct RowGeom {
@@ -317,8 +338,8 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     C *sm = smem + r * F::SLOTS;
     const long ngroups = (long)a.batch * a.nx / G::RPC;
-    if ((a.flags & 1024) && blockIdx.x < 444) __nanosleep((blockIdx.x / 148) * 1500);
-    if ((a.flags & 2048) && blockIdx.x < 444) __nanosleep((blockIdx.x / 148) * 2500);
+    pdl_launch_dependents();
+    pdl_wait();
     if (STAGED && (long)blockIdx.x < ngroups) stage_fetch(stage, a.src + (long)blockIdx.x * G::RPC * NY, GROUP_BYTES);
     for (long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
         const long row = grp * G::RPC + r;
@@ -372,6 +393,8 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<
     C *dst = a.dst + (size_t)b * NX * ny + col;
     C *sm = smem + c;
     C v[16];
+    pdl_launch_dependents();
+    pdl_wait();
 #pragma unroll
     for (int k = 0; k < 16; ++k) v[k] = __ldcg(src + (size_t)(j + F::M1 * k) * ny);
     F::fwd(v, sm, j, a.tw_x, a.tw1_x);
@@ -434,6 +457,8 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
     C *sm = smem + r * F::SLOTS;
     const long ngroups = (long)a.batch * a.nx / G::RPC;
     const int gpm = a.nx / G::RPC;  // groups per member: all rows of a group belong to one member
+    pdl_launch_dependents();
+    pdl_wait();
     if (STAGED && (long)blockIdx.x < ngroups) stage_fetch(stage, a.src + (long)blockIdx.x * G::RPC * NY, GROUP_BYTES);
     for (long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
         const long row = grp * G::RPC + r;
@@ -476,6 +501,9 @@ template <typename T, int N> struct Launch {
     static size_t row_smem() {
         return sizeof(C) * RowGeom<N>::RPC * Fft1D<N, 1, T>::SLOTS + (RowStage<T>::on ? sizeof(C) * RowGeom<N>::RPC * N : 0);
     }
+    // Measured on B200: overlapping the next pass's launch with the tail of
+    // the current one pays for launch-bound grids (<= 256^2 points) and costs 1-4 us per step above.
+    static bool use_pdl(const A &a) { return (long)a.batch * a.nx * a.ny <= 65536L; }
     // persistent when staged: GPE_ROW_MINB CTAs per SM walk over the row groups
     static unsigned row_grid(const A &a) {
         long groups = (long)a.batch * a.nx / RowGeom<N>::RPC;
@@ -504,10 +532,10 @@ template <typename T, int N> struct Launch {
         cudaError_t e;
         if (imag) {
             if ((e = prep(k_row_fwd<T, N, true>, row_smem())) != cudaSuccess) return e;
-            k_row_fwd<T, N, true><<<grid, block, row_smem(), s>>>(a);
+            { cudaError_t le = launch_pdl(k_row_fwd<T, N, true>, grid, block, row_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
         } else {
             if ((e = prep(k_row_fwd<T, N, false>, row_smem())) != cudaSuccess) return e;
-            k_row_fwd<T, N, false><<<grid, block, row_smem(), s>>>(a);
+            { cudaError_t le = launch_pdl(k_row_fwd<T, N, false>, grid, block, row_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
         }
         return cudaGetLastError();
     }
@@ -516,10 +544,10 @@ template <typename T, int N> struct Launch {
         cudaError_t e;
         if (imag) {
             if ((e = prep(k_row_inv<T, N, true>, row_smem())) != cudaSuccess) return e;
-            k_row_inv<T, N, true><<<grid, block, row_smem(), s>>>(a);
+            { cudaError_t le = launch_pdl(k_row_inv<T, N, true>, grid, block, row_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
         } else {
             if ((e = prep(k_row_inv<T, N, false>, row_smem())) != cudaSuccess) return e;
-            k_row_inv<T, N, false><<<grid, block, row_smem(), s>>>(a);
+            { cudaError_t le = launch_pdl(k_row_inv<T, N, false>, grid, block, row_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
         }
         return cudaGetLastError();
     }
@@ -529,13 +557,13 @@ template <typename T, int N> struct Launch {
         cudaError_t e;
         if (mode == 1) {
             if ((e = prep(k_col<T, N, false, 1>, col_smem())) != cudaSuccess) return e;
-            k_col<T, N, false, 1><<<grid, block, col_smem(), s>>>(a);
+            { cudaError_t le = launch_pdl(k_col<T, N, false, 1>, grid, block, col_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
         } else if (imag) {
             if ((e = prep(k_col<T, N, true, 0>, col_smem())) != cudaSuccess) return e;
-            k_col<T, N, true, 0><<<grid, block, col_smem(), s>>>(a);
+            { cudaError_t le = launch_pdl(k_col<T, N, true, 0>, grid, block, col_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
         } else {
             if ((e = prep(k_col<T, N, false, 0>, col_smem())) != cudaSuccess) return e;
-            k_col<T, N, false, 0><<<grid, block, col_smem(), s>>>(a);
+            { cudaError_t le = launch_pdl(k_col<T, N, false, 0>, grid, block, col_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
         }
         return cudaGetLastError();
     }
