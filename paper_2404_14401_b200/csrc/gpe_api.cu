@@ -39,6 +39,8 @@ struct gpe_plan {
     // device tables (typed by dtype)
     void *tw_x = nullptr, *tw_y = nullptr;
     void *tw1_x = nullptr, *tw1_y = nullptr;
+    void *tw_hy = nullptr, *tw1_hy = nullptr;  // length ny/2 (paired row passes)
+    void *ytab2 = nullptr;
     void *kin_x = nullptr, *kin_y = nullptr;
     double kin_dt = 0.0;
     int kin_mode = -1;
@@ -147,6 +149,23 @@ template <typename T> gpe_status make_twiddles(gpe_plan *p) {
                 re[k * m1 + j] = cos(a1); im[k * m1 + j] = sin(a1);
             }
         s = upload_cplx<T>(p, ax == 0 ? &p->tw1_x : &p->tw1_y, re, im);
+        if (s != GPE_OK) return s;
+    }
+    {   // the same two tables for length ny/2 (gpe_pair.cuh, passes A and C)
+        const int n = p->ny / 2, m1 = n / 16;
+        std::vector<double> re(n), im(n);
+        for (int m = 0; m < n; ++m) {
+            double ang = -2.0 * kPi * (double)m / (double)n;
+            re[m] = cos(ang); im[m] = sin(ang);
+        }
+        gpe_status s = upload_cplx<T>(p, &p->tw_hy, re, im);
+        if (s != GPE_OK) return s;
+        for (int k = 0; k < 16; ++k)
+            for (int j = 0; j < m1; ++j) {
+                double a1 = -2.0 * kPi * (double)((long)k * j % n) / (double)n;
+                re[k * m1 + j] = cos(a1); im[k * m1 + j] = sin(a1);
+            }
+        s = upload_cplx<T>(p, &p->tw1_hy, re, im);
         if (s != GPE_OK) return s;
     }
     return GPE_OK;
@@ -340,6 +359,8 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     a.g = (const T *)p->g;
     a.tw_x = (const cx<T> *)p->tw_x; a.tw_y = (const cx<T> *)p->tw_y;
     a.tw1_x = (const cx<T> *)p->tw1_x; a.tw1_y = (const cx<T> *)p->tw1_y;
+    a.tw_hy = (const cx<T> *)p->tw_hy; a.tw1_hy = (const cx<T> *)p->tw1_hy;
+    a.ytab2 = (const T *)p->ytab2;
     a.kin_xc = (const cx<T> *)p->kin_x; a.kin_yc = (const cx<T> *)p->kin_y;
     a.kin_xr = (const T *)p->kin_x; a.kin_yr = (const T *)p->kin_y;
     a.inv_p = (T)(1.0 / ((double)p->nx * (double)p->ny));
@@ -384,19 +405,22 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
                                                  (const T *)p->cavy, p->cavity_on, f);
         GPE_CUDA(p, cudaGetLastError());
     }
-    a.fin.cpm = p->nx / oy->rows_per_cta;
+    // complex64 hot path: paired passes (gpe_pair.cuh) when built for both axis lengths
+    if (const char *dbg = getenv("GPE_DEBUG_FLAGS")) a.flags |= atoi(dbg);   // ablation experiments only
+    const bool paired = oy->p_row_fwd && ox->p_col && !getenv("GPE_NO_PAIR");
+    a.fin.cpm = p->nx / (paired ? oy->p_rows_per_cta : oy->rows_per_cta);
     a.fin.normalise = imag ? 1 : 0;
     a.fin.advance = 1;
     a.fin.record_every = 0; a.fin.rec_first = 0; a.fin.records = nullptr;  // step kernels read *call
     auto one_step = [&](cudaStream_t st, int w, cudaEvent_t e0, cudaEvent_t e1) -> gpe_status {
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, st));
-        GPE_CUDA(p, oy->row_fwd(a, imag, st));
+        GPE_CUDA(p, paired ? oy->p_row_fwd(a, imag, st) : oy->row_fwd(a, imag, st));
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e1, st));
         if (w == 1) GPE_CUDA(p, cudaEventRecord(e0, st));
-        GPE_CUDA(p, ox->col(a, imag, 0, st));
+        GPE_CUDA(p, paired ? ox->p_col(a, imag, st) : ox->col(a, imag, 0, st));
         if (w == 1) GPE_CUDA(p, cudaEventRecord(e1, st));
         if (w == 2) GPE_CUDA(p, cudaEventRecord(e0, st));
-        GPE_CUDA(p, oy->row_inv(a, imag, st));
+        GPE_CUDA(p, paired ? oy->p_row_inv(a, imag, st) : oy->row_inv(a, imag, st));
         if (w == 2) GPE_CUDA(p, cudaEventRecord(e1, st));
         return GPE_OK;
     };
@@ -594,6 +618,14 @@ template <typename T> gpe_status set_potential_impl(gpe_plan *p, const gpe_poten
         std::vector<double> yt(4 * (size_t)ny, 0.0);
         for (int j = 0; j < ny; ++j) { yt[4 * j] = hy[j]; yt[4 * j + 1] = ly[j]; yt[4 * j + 2] = cyv[j]; }
         if ((s = upload_real<T>(p, &p->ytab, yt)) != GPE_OK) return s;
+        // the same for the paired row passes: points n and n + ny/2 side by side
+        const int h = ny / 2;
+        std::vector<double> y2(8 * (size_t)h, 0.0);
+        for (int n = 0; n < h; ++n) {
+            y2[8 * n] = hy[n]; y2[8 * n + 1] = hy[n + h]; y2[8 * n + 2] = ly[n]; y2[8 * n + 3] = ly[n + h];
+            y2[8 * n + 4] = cyv[n]; y2[8 * n + 5] = cyv[n + h];
+        }
+        if ((s = upload_real<T>(p, &p->ytab2, y2)) != GPE_OK) return s;
     }
     p->h_g.assign(B, 0.0);
     if (d->g) {
@@ -670,7 +702,7 @@ gpe_status gpe_plan_destroy(gpe_plan *p) {
     cudaStreamSynchronize(p->stream);
     if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
-    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
+    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
                     p->ytab, p->g, p->v2d, p->st, p->partials, p->counters, p->nonfinite, p->d_sched_step,
                     p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->scratch, p->obs_dev,
                     p->pop_dev, p->obsA_dev};

@@ -12,6 +12,11 @@ template <typename T> struct Ops {
     cudaError_t (*row_inv)(const A &, bool imag, cudaStream_t);            // ny == N
     cudaError_t (*col)(const A &, bool imag, int mode, cudaStream_t);      // nx == N
     int rows_per_cta;
+    // paired complex64 hot path (gpe_pair.cuh); null when not built for this (dtype, N)
+    cudaError_t (*p_row_fwd)(const A &, bool imag, cudaStream_t);
+    cudaError_t (*p_row_inv)(const A &, bool imag, cudaStream_t);
+    cudaError_t (*p_col)(const A &, bool imag, cudaStream_t);
+    int p_rows_per_cta;
 };
 
 #define GPE_DECL_OPS(N)                    \

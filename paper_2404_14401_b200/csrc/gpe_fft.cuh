@@ -12,6 +12,14 @@
 // reordering at all: that is what the column pass does (kinetic factor in the middle).
 // Lanes of a warp always run over the oldest digit k1 (16 values) and the slot index carries
 // one padding element per k1 block, which keeps all shared-memory accesses conflict free.
+//
+// Element types.  The transform is written once over an element type E:
+//   float2 / double2 : one complex number per element (scalar arithmetic);
+//   cpair            : TWO complex64 numbers of two independent transforms in lock step, stored
+//                      as (re0, re1), (im0, im1).  Every add, multiply and fma is then one packed
+//                      fp32x2 instruction of sm_100 (FADD2 / FMUL2 / FFMA2 -- the twiddle enters
+//                      as a broadcast scalar operand), so a butterfly costs half the issue slots
+//                      per point, and a shared-memory exchange is one 128-bit access per pair.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -22,34 +30,68 @@ template <> struct Vec2<float> { using type = float2; };
 template <> struct Vec2<double> { using type = double2; };
 template <typename T> using cx = typename Vec2<T>::type;
 
+struct __align__(16) cpair { float2 re, im; };
+
+template <typename E> struct El;
+// T scalar type, R real vector (one value per lane), SE shared-memory element, PLANES of SE per element
+template <> struct El<float2> { using T = float; using R = float; using SE = float2; static constexpr int PLANES = 1; };
+template <> struct El<double2> { using T = double; using R = double; using SE = double2; static constexpr int PLANES = 1; };
+template <> struct El<cpair> { using T = float; using R = float2; using SE = float2; static constexpr int PLANES = 2; };
+
 template <typename T> __device__ __forceinline__ cx<T> mk(T x, T y) { cx<T> r; r.x = x; r.y = y; return r; }
-// complex64 sums use the packed fp32x2 adder of sm_100 (FADD2 / FFMA2: one issue slot for both
-// components; same rounding as two scalar adds).  GPE_PACKED_ADD=0 falls back to scalar adds.
-#ifndef GPE_PACKED_ADD
-#define GPE_PACKED_ADD 0
-#endif
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) {
-#if GPE_PACKED_ADD
-    return __fadd2_rn(a, b);
-#else
-    a.x += b.x; a.y += b.y; return a;
-#endif
+
+// ---- "real vector" arithmetic: R = float | double | float2 (two lanes), s = scalar (broadcast)
+__device__ __forceinline__ float radd(float a, float b) { return a + b; }
+__device__ __forceinline__ float rsub(float a, float b) { return a - b; }
+__device__ __forceinline__ float rneg(float a) { return -a; }
+__device__ __forceinline__ float rmuls(float a, float s) { return a * s; }
+__device__ __forceinline__ float rfmas(float a, float s, float c) { return fmaf(a, s, c); }
+__device__ __forceinline__ double radd(double a, double b) { return a + b; }
+__device__ __forceinline__ double rsub(double a, double b) { return a - b; }
+__device__ __forceinline__ double rneg(double a) { return -a; }
+__device__ __forceinline__ double rmuls(double a, double s) { return a * s; }
+__device__ __forceinline__ double rfmas(double a, double s, double c) { return fma(a, s, c); }
+__device__ __forceinline__ float2 rneg(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 radd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 rsub(float2 a, float2 b) { return __fadd2_rn(a, rneg(b)); }
+__device__ __forceinline__ float2 rmuls(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
+__device__ __forceinline__ float2 rfmas(float2 a, float s, float2 c) { return __ffma2_rn(a, make_float2(s, s), c); }
+__device__ __forceinline__ float2 rmul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 rfma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+template <int SG, typename R> __device__ __forceinline__ R rsg(R a) { if constexpr (SG > 0) return a; else return rneg(a); }
+
+// ---- element access
+__device__ __forceinline__ float ere(float2 z) { return z.x; }
+__device__ __forceinline__ float eim(float2 z) { return z.y; }
+__device__ __forceinline__ double ere(double2 z) { return z.x; }
+__device__ __forceinline__ double eim(double2 z) { return z.y; }
+__device__ __forceinline__ float2 ere(cpair z) { return z.re; }
+__device__ __forceinline__ float2 eim(cpair z) { return z.im; }
+template <typename E> __device__ __forceinline__ E emk(typename El<E>::R x, typename El<E>::R y);
+template <> __device__ __forceinline__ float2 emk<float2>(float x, float y) { return make_float2(x, y); }
+template <> __device__ __forceinline__ double2 emk<double2>(double x, double y) { return make_double2(x, y); }
+template <> __device__ __forceinline__ cpair emk<cpair>(float2 x, float2 y) { cpair r; r.re = x; r.im = y; return r; }
+
+// shared-memory exchange.  A cpair goes to two 64-bit planes (all real parts, then all imaginary
+// parts, PLANE elements apart): the packed arithmetic keeps (re0, re1) and (im0, im1) in two
+// unrelated register pairs, and a single 128-bit access would cost two MOVs per element to line
+// them up in one aligned quad.
+template <int PLANE> __device__ __forceinline__ void sst(float2 *sm, int i, float2 v) { sm[i] = v; }
+template <int PLANE> __device__ __forceinline__ void sst(double2 *sm, int i, double2 v) { sm[i] = v; }
+template <int PLANE> __device__ __forceinline__ void sst(float2 *sm, int i, cpair v) { sm[i] = v.re; sm[i + PLANE] = v.im; }
+template <int PLANE, typename E> __device__ __forceinline__ E sld(const typename El<E>::SE *sm, int i) {
+    if constexpr (El<E>::PLANES == 2) { E r; r.re = sm[i]; r.im = sm[i + PLANE]; return r; }
+    else return sm[i];
 }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) {
-#if GPE_PACKED_ADD
-    return __ffma2_rn(b, make_float2(-1.0f, -1.0f), a);
-#else
-    a.x -= b.x; a.y -= b.y; return a;
-#endif
+
+template <typename E> __device__ __forceinline__ E cadd(E a, E b) { return emk<E>(radd(ere(a), ere(b)), radd(eim(a), eim(b))); }
+template <typename E> __device__ __forceinline__ E csub(E a, E b) { return emk<E>(rsub(ere(a), ere(b)), rsub(eim(a), eim(b))); }
+// a * w and a * conj(w); w = one twiddle (cos, sin) shared by all lanes of the element
+template <typename E> __device__ __forceinline__ E cmul(E a, cx<typename El<E>::T> w) {
+    return emk<E>(rfmas(ere(a), w.x, rmuls(eim(a), -w.y)), rfmas(ere(a), w.y, rmuls(eim(a), w.x)));
 }
-__device__ __forceinline__ double2 cadd(double2 a, double2 b) { a.x += b.x; a.y += b.y; return a; }
-__device__ __forceinline__ double2 csub(double2 a, double2 b) { a.x -= b.x; a.y -= b.y; return a; }
-template <typename C> __device__ __forceinline__ C cmul(C a, C b) {
-    C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r;
-}
-// a * conj(b)
-template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {
-    C r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r;
+template <typename E> __device__ __forceinline__ E cmulc(E a, cx<typename El<E>::T> w) {
+    return emk<E>(rfmas(ere(a), w.x, rmuls(eim(a), w.y)), rfmas(eim(a), w.x, rmuls(ere(a), -w.y)));
 }
 
 // z * exp(SIGN * 2 pi i m / 16), m = 0..7; m is a compile-time constant after unrolling.
@@ -72,50 +114,62 @@ template <> struct K16<double> {
                             H_hi = 0.70710678118654752440, H_lo = 0.0;
 };
 // u*C + t with a single rounding of the large terms (t = the S-term plus nothing else)
-template <typename T> __device__ __forceinline__ T mulC_add(T u, T t) {
-    if constexpr (sizeof(T) == 4) return fma(u, K16<T>::C_hi, fma(u, K16<T>::C_lo, t));
-    else return fma(u, K16<T>::C_hi, t);
+template <typename T, typename R> __device__ __forceinline__ R mulC_add(R u, R t) {
+    if constexpr (sizeof(T) == 4) return rfmas(u, K16<T>::C_hi, rfmas(u, K16<T>::C_lo, t));
+    else return rfmas(u, K16<T>::C_hi, t);
 }
-template <typename T> __device__ __forceinline__ T mulH(T u) {
-    if constexpr (sizeof(T) == 4) return fma(u, K16<T>::H_hi, u * K16<T>::H_lo);
-    else return u * K16<T>::H_hi;
+template <typename T, typename R> __device__ __forceinline__ R mulH(R u) {
+    if constexpr (sizeof(T) == 4) return rfmas(u, K16<T>::H_hi, rmuls(u, K16<T>::H_lo));
+    else return rmuls(u, K16<T>::H_hi);
 }
-template <int SIGN, typename T> __device__ __forceinline__ cx<T> rot16(cx<T> z, int m) {
+template <int SIGN, typename E> __device__ __forceinline__ E rot16(E z, int m) {
+    using T = typename El<E>::T;
+    using R = typename El<E>::R;
     constexpr T S = K16<T>::S;
-    constexpr T sg = T(SIGN);
+    constexpr T sS = T(SIGN) * S;
+    const R x = ere(z), y = eim(z);
     switch (m) {
     case 0: return z;
-    case 4: return mk<T>(-sg * z.y, sg * z.x);
-    case 2: return mk<T>(mulH<T>(z.x - sg * z.y), mulH<T>(sg * z.x + z.y));
-    case 6: return mk<T>(mulH<T>(-(z.x + sg * z.y)), mulH<T>(sg * z.x - z.y));
+    case 4: return emk<E>(rsg<-SIGN>(y), rsg<SIGN>(x));
+    case 2: return emk<E>(mulH<T>(radd(x, rsg<-SIGN>(y))), mulH<T>(radd(rsg<SIGN>(x), y)));
+    case 6: return emk<E>(mulH<T>(rneg(radd(x, rsg<SIGN>(y)))), mulH<T>(rsub(rsg<SIGN>(x), y)));
     // (C + i sg S), (S + i sg C), (-S + i sg C), (-C + i sg S)
-    case 1: return mk<T>(mulC_add<T>(z.x, -(sg * S) * z.y), mulC_add<T>(z.y, (sg * S) * z.x));
-    case 3: return mk<T>(mulC_add<T>(-sg * z.y, S * z.x), mulC_add<T>(sg * z.x, S * z.y));
-    case 5: return mk<T>(mulC_add<T>(-sg * z.y, -S * z.x), mulC_add<T>(sg * z.x, -S * z.y));
-    default: return mk<T>(mulC_add<T>(-z.x, -(sg * S) * z.y), mulC_add<T>(-z.y, (sg * S) * z.x));
+    case 1: return emk<E>(mulC_add<T>(x, rmuls(y, -sS)), mulC_add<T>(y, rmuls(x, sS)));
+    case 3: return emk<E>(mulC_add<T>(rsg<-SIGN>(y), rmuls(x, S)), mulC_add<T>(rsg<SIGN>(x), rmuls(y, S)));
+    case 5: return emk<E>(mulC_add<T>(rsg<-SIGN>(y), rmuls(x, -S)), mulC_add<T>(rsg<SIGN>(x), rmuls(y, -S)));
+    default: return emk<E>(mulC_add<T>(rneg(x), rmuls(y, -sS)), mulC_add<T>(rneg(y), rmuls(x, sS)));
     }
 }
 
 // In-register DFT of size R (2, 4, 8, 16): v[k] <- sum_a v[a] exp(SIGN 2 pi i a k / R),
 // natural order in and out, radix-2 decimation in time with constant twiddles.
-template <int R, int SIGN, typename T> __device__ __forceinline__ void dft(cx<T> *v) {
+template <int R, int SIGN, typename E> __device__ __forceinline__ void dft(E *v) {
     if constexpr (R == 2) {
-        cx<T> a = v[0];
+        E a = v[0];
         v[0] = cadd(a, v[1]);
         v[1] = csub(a, v[1]);
     } else {
-        cx<T> e[R / 2], o[R / 2];
+        E e[R / 2], o[R / 2];
 #pragma unroll
         for (int k = 0; k < R / 2; ++k) { e[k] = v[2 * k]; o[k] = v[2 * k + 1]; }
-        dft<R / 2, SIGN, T>(e);
-        dft<R / 2, SIGN, T>(o);
+        dft<R / 2, SIGN, E>(e);
+        dft<R / 2, SIGN, E>(o);
 #pragma unroll
         for (int k = 0; k < R / 2; ++k) {
-            cx<T> t = rot16<SIGN, T>(o[k], k * (16 / R));
+            E t = rot16<SIGN, E>(o[k], k * (16 / R));
             v[k] = cadd(e[k], t);
             v[k + R / 2] = csub(e[k], t);
         }
     }
+}
+
+// twiddle fetch (GPE_ABL_NOTW: ablation experiment only -- no table load, wrong numerics)
+template <typename C> __device__ __forceinline__ C ldtw(const C *__restrict__ t, int i) {
+#ifdef GPE_ABL_NOTW
+    C r; r.x = 1.0f; r.y = 1e-9f * (float)i; return r;
+#else
+    return t[i];
+#endif
 }
 
 template <int N> struct Fact;
@@ -128,13 +182,18 @@ template <> struct Fact<2048> { static constexpr int R2 = 16, R3 = 8; };
 
 // One 1-D FFT of length N worked on by N/16 threads (index j), S = element stride of the
 // shared-memory tile (1 for a row, W for a tile of W columns).  tw[m] = exp(-2 pi i m / N).
-template <int N, int S, typename T> struct Fft1D {
+// E = element type (see the top of this file); twiddles are always one cx<T> per element.
+template <int N, int S, typename E> struct Fft1D {
+    using T = typename El<E>::T;
     using C = cx<T>;
+    using SE = typename El<E>::SE;
     static constexpr int TPF = N / 16;
     static constexpr int M1 = N / 16;
     static constexpr int R2 = Fact<N>::R2, R3 = Fact<N>::R3;
     static constexpr int NST = R3 > 1 ? 3 : 2;
     static constexpr int SLOTS = N + 16;           // one padding slot per k1 block
+    static constexpr int PLANE = SLOTS * S;        // distance between the planes of a cpair tile
+    static constexpr int TILE = SLOTS * S * El<E>::PLANES;  // SE elements of one tile (S transforms)
     static constexpr int RL = NST == 3 ? R3 : R2;  // radix of the last stage
     static constexpr int GL = 16 / RL;             // butterflies per thread in the last stage
 
@@ -156,88 +215,99 @@ template <int N, int S, typename T> struct Fft1D {
     }
 
     template <int R, int Mp, bool LAST>
-    __device__ __forceinline__ static void stage_fwd(C *v, C *sm, int j, const C *__restrict__ tw) {
+    __device__ __forceinline__ static void stage_fwd(E *v, SE *sm, int j, const C *__restrict__ tw) {
         constexpr int G = 16 / R, M = Mp / R;
 #pragma unroll
         for (int i = 0; i < G; ++i) {
             int q, b = base_slot<R, Mp>(j + i * TPF, q);
 #pragma unroll
-            for (int a = 0; a < R; ++a) v[i * R + a] = sm[phys(b + M * a)];
+            for (int a = 0; a < R; ++a) v[i * R + a] = sld<PLANE, E>(sm, phys(b + M * a));
         }
 #pragma unroll
-        for (int i = 0; i < G; ++i) dft<R, -1, T>(v + i * R);
+        for (int i = 0; i < G; ++i) dft<R, -1, E>(v + i * R);
         if constexpr (!LAST) {
 #pragma unroll
             for (int i = 0; i < G; ++i) {
                 int q, b = base_slot<R, Mp>(j + i * TPF, q);
 #pragma unroll
-                for (int k = 1; k < R; ++k) v[i * R + k] = cmul(v[i * R + k], tw[(N / Mp) * k * q]);
+                for (int k = 1; k < R; ++k) v[i * R + k] = cmul(v[i * R + k], ldtw(tw, (N / Mp) * k * q));
 #pragma unroll
-                for (int k = 0; k < R; ++k) sm[phys(b + M * k)] = v[i * R + k];
+                for (int k = 0; k < R; ++k) sst<PLANE>(sm, phys(b + M * k), v[i * R + k]);
             }
         }
     }
 
     template <int R, int Mp, bool LAST>
-    __device__ __forceinline__ static void stage_inv(C *v, C *sm, int j, const C *__restrict__ tw) {
+    __device__ __forceinline__ static void stage_inv(E *v, SE *sm, int j, const C *__restrict__ tw) {
         constexpr int G = 16 / R, M = Mp / R;
         if constexpr (!LAST) {
 #pragma unroll
             for (int i = 0; i < G; ++i) {
                 int q, b = base_slot<R, Mp>(j + i * TPF, q);
 #pragma unroll
-                for (int k = 0; k < R; ++k) v[i * R + k] = sm[phys(b + M * k)];
+                for (int k = 0; k < R; ++k) v[i * R + k] = sld<PLANE, E>(sm, phys(b + M * k));
 #pragma unroll
-                for (int k = 1; k < R; ++k) v[i * R + k] = cmulc(v[i * R + k], tw[(N / Mp) * k * q]);
+                for (int k = 1; k < R; ++k) v[i * R + k] = cmulc(v[i * R + k], ldtw(tw, (N / Mp) * k * q));
             }
         }
 #pragma unroll
-        for (int i = 0; i < G; ++i) dft<R, +1, T>(v + i * R);
+        for (int i = 0; i < G; ++i) dft<R, +1, E>(v + i * R);
 #pragma unroll
         for (int i = 0; i < G; ++i) {
             int q, b = base_slot<R, Mp>(j + i * TPF, q);
 #pragma unroll
-            for (int a = 0; a < R; ++a) sm[phys(b + M * a)] = v[i * R + a];
+            for (int a = 0; a < R; ++a) sst<PLANE>(sm, phys(b + M * a), v[i * R + a]);
         }
     }
 
     // in: v[a] = x[j + (N/16) a].  out: v[i*RL + r] = X[nat(j,i,r)] (unnormalised, e^{-i}).
-    // All threads of the CTA must call this together (it contains __syncthreads()).
+    // All threads that share `sm` must call this together: SYNC() is the barrier between them
+    // (__syncthreads, or a named barrier over the threads of one transform).
     // tw1[k * M1 + j] = exp(-2 pi i k j / N): the first-stage twiddles transposed so that the
     // lanes of a warp (consecutive j) read consecutive addresses (tw[k * j] is a stride-k gather
     // that costs up to 30 L1 wavefronts per load).
-    __device__ __forceinline__ static void fwd(C *v, C *sm, int j, const C *__restrict__ tw,
-                                               const C *__restrict__ tw1) {
-        dft<16, -1, T>(v);
+    template <typename Sync>
+    __device__ __forceinline__ static void fwd(E *v, SE *sm, int j, const C *__restrict__ tw,
+                                               const C *__restrict__ tw1, Sync SYNC) {
+        dft<16, -1, E>(v);
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], tw1[k * M1 + j]);
+        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], ldtw(tw1, k * M1 + j));
 #pragma unroll
-        for (int k = 0; k < 16; ++k) sm[phys(j + M1 * k)] = v[k];
-        __syncthreads();
+        for (int k = 0; k < 16; ++k) sst<PLANE>(sm, phys(j + M1 * k), v[k]);
+        SYNC();
         stage_fwd<R2, M1, NST == 2>(v, sm, j, tw);
         if constexpr (NST == 3) {
-            __syncthreads();
+            SYNC();
             stage_fwd<R3, M1 / R2, true>(v, sm, j, tw);
         }
+    }
+    __device__ __forceinline__ static void fwd(E *v, SE *sm, int j, const C *__restrict__ tw,
+                                               const C *__restrict__ tw1) {
+        fwd(v, sm, j, tw, tw1, [] { __syncthreads(); });
     }
 
     // exact mirror of fwd (unnormalised, e^{+i}): in: v[i*RL + r] = X[nat(j,i,r)],
     // out: v[a] = sum_k X[k] e^{+2 pi i k n / N} at n = j + (N/16) a.
-    __device__ __forceinline__ static void inv(C *v, C *sm, int j, const C *__restrict__ tw,
-                                               const C *__restrict__ tw1) {
+    template <typename Sync>
+    __device__ __forceinline__ static void inv(E *v, SE *sm, int j, const C *__restrict__ tw,
+                                               const C *__restrict__ tw1, Sync SYNC) {
         if constexpr (NST == 3) {
             stage_inv<R3, M1 / R2, true>(v, sm, j, tw);
-            __syncthreads();
+            SYNC();
             stage_inv<R2, M1, false>(v, sm, j, tw);
         } else {
             stage_inv<R2, M1, true>(v, sm, j, tw);
         }
-        __syncthreads();
+        SYNC();
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = sm[phys(j + M1 * k)];
+        for (int k = 0; k < 16; ++k) v[k] = sld<PLANE, E>(sm, phys(j + M1 * k));
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], tw1[k * M1 + j]);
-        dft<16, +1, T>(v);
+        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], ldtw(tw1, k * M1 + j));
+        dft<16, +1, E>(v);
+    }
+    __device__ __forceinline__ static void inv(E *v, SE *sm, int j, const C *__restrict__ tw,
+                                               const C *__restrict__ tw1) {
+        inv(v, sm, j, tw, tw1, [] { __syncthreads(); });
     }
 };
 

@@ -328,7 +328,7 @@ __device__ __forceinline__ void stage_fetch(unsigned char *stage, const void *gs
 template <typename T, int NY, bool IMAG>
 __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : 1)) k_row_fwd(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
-    using F = Fft1D<NY, 1, T>;
+    using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
     constexpr bool STAGED = RowStage<T>::on;
     constexpr int GROUP_BYTES = (int)sizeof(C) * G::RPC * NY;
@@ -382,7 +382,7 @@ template <typename T, int NX, bool IMAG, int MODE>
 __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using G = ColGeom<T, NX>;
-    using F = Fft1D<NX, G::W, T>;
+    using F = Fft1D<NX, G::W, cx<T>>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
     const int c = threadIdx.x % G::W, j = threadIdx.x / G::W;
@@ -445,7 +445,7 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<
 template <typename T, int NY, bool IMAG>
 __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : 1)) k_row_inv(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
-    using F = Fft1D<NY, 1, T>;
+    using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
     constexpr bool STAGED = RowStage<T>::on;
     constexpr int GROUP_BYTES = (int)sizeof(C) * G::RPC * NY;
@@ -499,7 +499,7 @@ template <typename T, int N> struct Launch {
     using C = cx<T>;
     using A = StepArgs<T, C>;
     static size_t row_smem() {
-        return sizeof(C) * RowGeom<N>::RPC * Fft1D<N, 1, T>::SLOTS + (RowStage<T>::on ? sizeof(C) * RowGeom<N>::RPC * N : 0);
+        return sizeof(C) * RowGeom<N>::RPC * Fft1D<N, 1, cx<T>>::SLOTS + (RowStage<T>::on ? sizeof(C) * RowGeom<N>::RPC * N : 0);
     }
     // Measured on B200: overlapping the next pass's launch with the tail of
     // the current one pays for launch-bound grids (<= 256^2 points) and costs 1-4 us per step above.
@@ -513,12 +513,12 @@ template <typename T, int N> struct Launch {
         long cap = (long)sms * GPE_ROW_MINB;
         return (unsigned)(groups < cap ? groups : cap);
     }
-    static size_t col_smem() { return sizeof(C) * ColGeom<T, N>::W * Fft1D<N, 1, T>::SLOTS; }
+    static size_t col_smem() { return sizeof(C) * ColGeom<T, N>::W * Fft1D<N, 1, cx<T>>::SLOTS; }
 
     // opt in to > 48 KB of dynamic shared memory once per kernel (not on every launch: the
     // attribute call costs microseconds of host time and the launch path is latency critical)
     template <typename K> static cudaError_t prep(K kern, size_t smem) {
-        static thread_local K done_for[8] = {};
+        static thread_local K done_for[16] = {};
         if (smem <= 48 * 1024) return cudaSuccess;
         for (K k : done_for) if (k == kern) return cudaSuccess;
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -1,0 +1,323 @@
+// gpe_pair.cuh -- the complex64 hot path: the three passes of gpe_kernels.cuh with every
+// thread working on TWO complex numbers in lock step (element type cpair of gpe_fft.cuh), so that
+// all butterfly and twiddle arithmetic is packed fp32x2 (FADD2 / FMUL2 / FFMA2 of sm_100) and
+// every shared-memory exchange and every access to the intermediate array is 128 bits wide.
+//
+//   pass B (columns): the two lanes are two ADJACENT COLUMNS (two independent transforms).
+//   pass A (rows):    the two lanes are the even and the odd half of ONE row transform: a
+//                     decimation-in-frequency radix-2 layer, written with scalar instructions
+//                     right after the potential half-step (which is scalar anyway and so converts
+//                     the interleaved (re, im) input to the split lane layout for free), followed
+//                     by two independent NY/2-point transforms.  Lane 0 ends with psi^[2k'],
+//                     lane 1 with psi^[2k'+1]: exactly the column pair pass B wants.
+//   pass C (rows):    the mirror of pass A.
+// Intermediate layout (between A and C, inside the caller's psi buffer, same bytes per row):
+//   [batch][nx][ny/2] of cpair = (Re psi^[i][2k'], Re psi^[i][2k'+1], Im .., Im ..).
+// Same mathematics as gpe_kernels.cuh (PAPER.md:62-76 Eqs. 2-4, :116, :183-186 Eq. 14).
+#pragma once
+#include "gpe_kernels.cuh"
+
+#ifndef GPE_ABL
+#define GPE_ABL 0   // ablation experiments only (timing with wrong numerics)
+#endif
+#ifndef GPE_COLP_THREADS
+#define GPE_COLP_THREADS 256
+#endif
+
+namespace gpe {
+
+template <int N> struct RowGeomP {
+    static constexpr int H = N / 2;
+    static constexpr int TPF = H / 16;                               // threads per row
+    static constexpr int RPC = (128 / TPF) < 1 ? 1 : (128 / TPF);    // rows per CTA
+    static constexpr int THREADS = RPC * TPF;                        // 128
+    static constexpr bool NAMED = RPC > 1 && TPF % 32 == 0;          // rows own whole warps
+};
+template <int N> struct ColGeomP {
+    static constexpr int TPF = N / 16;                               // threads per column pair
+    static constexpr int CPW0 = GPE_COLP_THREADS / TPF;
+    static constexpr int CPW = CPW0 < 2 ? 2 : CPW0;                  // column pairs per CTA
+    static constexpr int THREADS = CPW * TPF;
+};
+
+__device__ __forceinline__ void bar_named(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ cpair ldcg_pair(const cpair *p) {
+    const float4 t = __ldcg(reinterpret_cast<const float4 *>(p));
+    cpair r; r.re = make_float2(t.x, t.y); r.im = make_float2(t.z, t.w); return r;
+}
+__device__ __forceinline__ void st_pair(cpair *p, cpair v) {
+    *reinterpret_cast<float4 *>(p) = make_float4(v.re.x, v.re.y, v.im.x, v.im.y);
+}
+
+// Potential half-step (rows a1 / a5) on the 32 points of one thread: p0[k] at y = j + M1 k,
+// p1[k] at y + H, same row i.  ytab2[n] = {vy[n], vy[n+H], cos^2(k_l y_n), cos^2(k_l y_{n+H})},
+// {cos(k_c y_n), cos(k_c y_{n+H}), 0, 0}.  The angle and its polynomial are packed over the two
+// points; |psi|^2 and the final rotation are scalar (they read / write the interleaved layout).
+// REDUCE: sn += |psi_new|^2, st += cos(k_c y) |psi_new|^2 (one lane per point).
+template <bool IMAG, bool REDUCE, int M1, int H>
+__device__ __forceinline__ void potential_pair16(float2 (&p0)[16], float2 (&p1)[16], const StepArgs<float, float2> &a,
+                                                 int b, int i, int j, float scale, float A, float Cc,
+                                                 float2 &sn, float2 &st) {
+    const int flags = a.flags;
+    float vrow = 0.f;
+    if (flags & F_HAS_SEP) vrow += a.vx[i];
+    if (flags & F_LAT_X) vrow += A * a.latx[i];
+    const float crow = (flags & F_CAVITY) ? Cc * a.cavx[i] : 0.f;
+    const float Ay = (flags & F_LAT_Y) ? A : 0.f;
+    const float g = (flags & F_HAS_G) ? a.g[b] : 0.f;
+    const float hdt = a.half_dt;
+    const float4 *__restrict__ yt = reinterpret_cast<const float4 *>(a.ytab2);
+    // in chunks of CH points per half row: bounds the live angles (registers); the tier vote is per chunk
+    constexpr int CH = 8;
+#pragma unroll
+    for (int k0 = 0; k0 < 16; k0 += CH) {
+        float2 w[16];   // only the CH entries of the current chunk are live
+    #pragma unroll
+        for (int k = k0; k < k0 + CH; ++k) {
+            const int n = j + M1 * k;
+            const float4 t0 = yt[2 * n];
+            const float2 cav = *reinterpret_cast<const float2 *>(yt + 2 * n + 1);
+            if constexpr (IMAG) { p0[k].x *= scale; p0[k].y *= scale; p1[k].x *= scale; p1[k].y *= scale; }
+            const float2 d = make_float2(fmaf(p0[k].x, p0[k].x, p0[k].y * p0[k].y), fmaf(p1[k].x, p1[k].x, p1[k].y * p1[k].y));
+            const float2 V = rfmas(cav, crow, rfmas(make_float2(t0.z, t0.w), Ay, radd(make_float2(t0.x, t0.y), make_float2(vrow, vrow))));
+            w[k] = rmuls(rfmas(d, g, V), hdt);
+        }
+        if (flags & F_HAS_V2D) {
+            const float *__restrict__ v2 = a.v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * a.nx * a.ny : 0) + (size_t)i * a.ny;
+    #pragma unroll
+            for (int k = k0; k < k0 + CH; ++k) w[k] = rfmas(make_float2(v2[j + M1 * k], v2[j + M1 * k + H]), hdt, w[k]);
+        }
+        if constexpr (IMAG) {
+    #pragma unroll
+            for (int k = k0; k < k0 + CH; ++k) {
+                const float e0 = expf(-w[k].x), e1 = expf(-w[k].y);
+                p0[k].x *= e0; p0[k].y *= e0; p1[k].x *= e1; p1[k].y *= e1;
+            }
+        } else {
+            // psi <- psi + psi * (cos w - 1 - i sin w); warp-uniform tiers by the largest |w| (see
+            // potential_step16 in gpe_kernels.cuh for the polynomials and why the "minus one" form).
+            float wmax = 0.f;
+    #pragma unroll
+            for (int k = k0; k < k0 + CH; ++k) wmax = fmaxf(wmax, fmaxf(fabsf(w[k].x), fabsf(w[k].y)));
+            auto rotate = [&](int k, float2 sn_, float2 cm1) {
+                const float ax = fmaf(p0[k].x, cm1.x, fmaf(-p0[k].y, sn_.x, p0[k].x));
+                const float ay = fmaf(p0[k].x, sn_.x, fmaf(p0[k].y, cm1.x, p0[k].y));
+                const float bx = fmaf(p1[k].x, cm1.y, fmaf(-p1[k].y, sn_.y, p1[k].x));
+                const float by = fmaf(p1[k].x, sn_.y, fmaf(p1[k].y, cm1.y, p1[k].y));
+                p0[k] = make_float2(ax, ay); p1[k] = make_float2(bx, by);
+            };
+            if (__all_sync(0xffffffffu, wmax <= 0.03125f)) {
+    #pragma unroll
+                for (int k = k0; k < k0 + CH; ++k) {
+                    const float2 w2 = rmul(w[k], w[k]);
+                    const float2 sn_ = rneg(rfmas(rmul(w[k], w2), -1.6666667e-1f, w[k]));   // sin(-w)
+                    const float2 cm1 = rmul(w2, rfmas(w2, 4.1666667e-2f, make_float2(-0.5f, -0.5f)));
+                    rotate(k, sn_, cm1);
+                }
+            } else if (__all_sync(0xffffffffu, wmax <= 0.5f)) {
+    #pragma unroll
+                for (int k = k0; k < k0 + CH; ++k) {
+                    float2 sn_, cm1;
+                    sincosm1_small(-w[k].x, &sn_.x, &cm1.x);
+                    sincosm1_small(-w[k].y, &sn_.y, &cm1.y);
+                    rotate(k, sn_, cm1);
+                }
+            } else {
+    #pragma unroll
+                for (int k = k0; k < k0 + CH; ++k) {
+                    float2 sn_, cm1;
+                    sincosm1_general(-w[k].x, &sn_.x, &cm1.x);
+                    sincosm1_general(-w[k].y, &sn_.y, &cm1.y);
+                    rotate(k, sn_, cm1);
+                }
+            }
+        }
+    }
+    if constexpr (REDUCE) {
+        sn = make_float2(0.f, 0.f); st = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            const float2 d = make_float2(fmaf(p0[k].x, p0[k].x, p0[k].y * p0[k].y), fmaf(p1[k].x, p1[k].x, p1[k].y * p1[k].y));
+            sn = radd(sn, d);
+            if (flags & F_CAVITY) st = rfma(d, *reinterpret_cast<const float2 *>(yt + 2 * (j + M1 * k) + 1), st);
+        }
+    }
+}
+
+// ---------------------------------------------------------------- pass A (rows, forward)
+template <int NY, bool IMAG>
+__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_fwd_p(const StepArgs<float, float2> a) {
+    using G = RowGeomP<NY>;
+    using F = Fft1D<G::H, 1, cpair>;
+    constexpr int H = G::H, M1 = F::M1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw) + r * F::TILE;
+    const long row = (long)blockIdx.x * G::RPC + r;
+    const int b = (int)(row / a.nx), i = (int)(row % a.nx);
+    const float2 *src = a.src + row * NY;
+    pdl_launch_dependents();
+    pdl_wait();
+    float2 p0[16], p1[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { p0[k] = __ldcg(src + j + M1 * k); p1[k] = __ldcg(src + H + j + M1 * k); }
+    {
+        const MemberState &ms = a.fin.st[b];
+        float2 sn, st;
+        potential_pair16<IMAG, false, M1, H>(p0, p1, a, b, i, j, (float)ms.scale, (float)ms.A, (float)ms.C, sn, st);
+    }
+    // radix-2 decimation in frequency across the two halves of the row: lane 0 <- x[n] + x[n+H],
+    // lane 1 <- (x[n] - x[n+H]) w_NY^n; scalar instructions, they write the split lane layout
+    cpair v[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const float2 w = a.tw_y[j + M1 * k];
+        const float dx = p0[k].x - p1[k].x, dy = p0[k].y - p1[k].y;
+        v[k].re = make_float2(p0[k].x + p1[k].x, fmaf(dx, w.x, -(dy * w.y)));
+        v[k].im = make_float2(p0[k].y + p1[k].y, fmaf(dx, w.y, dy * w.x));
+    }
+    if constexpr (G::NAMED) F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
+    else F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+    cpair *dst = reinterpret_cast<cpair *>(a.dst) + row * H;
+#pragma unroll
+    for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+        for (int rr = 0; rr < F::RL; ++rr) st_pair(dst + F::nat(j, ii, rr), v[ii * F::RL + rr]);
+}
+
+// ---------------------------------------------------------------- pass B (columns)
+template <int NX, bool IMAG>
+__global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS <= 256 ? 2 : 1)) k_col_p(const StepArgs<float, float2> a) {
+    using G = ColGeomP<NX>;
+    using F = Fft1D<NX, G::CPW, cpair>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int c = threadIdx.x % G::CPW, j = threadIdx.x / G::CPW;
+    const int cp = blockIdx.x * G::CPW + c;      // column pair: columns 2 cp, 2 cp + 1
+    const int b = blockIdx.y;
+    const size_t hy = a.ny / 2;
+    const cpair *src = reinterpret_cast<const cpair *>(a.src) + (size_t)b * NX * hy + cp;
+    cpair *dst = reinterpret_cast<cpair *>(a.dst) + (size_t)b * NX * hy + cp;
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw) + c;
+    cpair v[16];
+    pdl_launch_dependents();
+    pdl_wait();
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        if ((GPE_ABL & 1) || (a.flags & 512)) { v[k].re = make_float2(1e-3f * k, 2e-3f * j); v[k].im = make_float2(1e-3f * c, -1e-3f * k); }
+        else v[k] = ldcg_pair(src + (size_t)(j + F::M1 * k) * hy);
+    }
+    if (a.flags & 256) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) st_pair(dst + (size_t)(j + F::M1 * k) * hy, v[k]);
+        return;
+    }
+    F::fwd(v, sm, j, a.tw_x, a.tw1_x, [] { if (!(GPE_ABL & 16)) __syncthreads(); });
+    if constexpr (IMAG) {
+        const float2 ey = *reinterpret_cast<const float2 *>(a.kin_yr + 2 * cp);
+#pragma unroll
+        for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) {
+                const float2 f = rmuls(ey, a.kin_xr[F::nat(j, ii, rr)]);
+                cpair &z = v[ii * F::RL + rr];
+                z.re = rmul(z.re, f); z.im = rmul(z.im, f);
+            }
+    } else {
+        // kinetic factor (1+a)(1+b)/P applied as v/P + v*g, g = a' + b' + a'b (k_col of
+        // gpe_kernels.cuh); b differs between the two columns (lanes), a is common to both
+        const float4 bq4 = *reinterpret_cast<const float4 *>(a.kin_yc + 2 * cp);
+        const float2 bqx = make_float2(bq4.x, bq4.z), bqy = make_float2(bq4.y, bq4.w);
+        const float invp = a.inv_p;
+        const float2 cb = radd(bqx, make_float2(1.f, 1.f));
+        const float2 bpx = rmuls(bqx, invp), bpy = rmuls(bqy, invp);
+#pragma unroll
+        for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) {
+                const float2 ap = (GPE_ABL & 8) ? make_float2(1e-7f * ii, 1e-7f * rr) : a.kin_xc[F::nat(j, ii, rr)];
+                const float2 gx = rfmas(cb, ap.x, rfmas(bqy, -ap.y, bpx));
+                const float2 gy = rfmas(bqy, ap.x, rfmas(cb, ap.y, bpy));
+                cpair &z = v[ii * F::RL + rr];
+                const float2 ox = rfma(z.re, gx, rfma(rneg(z.im), gy, rmuls(z.re, invp)));
+                const float2 oy = rfma(z.re, gy, rfma(z.im, gx, rmuls(z.im, invp)));
+                z.re = ox; z.im = oy;
+            }
+    }
+    F::inv(v, sm, j, a.tw_x, a.tw1_x, [] { if (!(GPE_ABL & 16)) __syncthreads(); });
+    if (((GPE_ABL & 2) || (a.flags & 1024)) && v[0].re.x != 12345.678f) return;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) st_pair(dst + (size_t)(j + F::M1 * k) * hy, v[k]);
+}
+
+// ---------------------------------------------------------------- pass C (rows, inverse)
+template <int NY, bool IMAG>
+__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_inv_p(const StepArgs<float, float2> a) {
+    using G = RowGeomP<NY>;
+    using F = Fft1D<G::H, 1, cpair>;
+    constexpr int H = G::H, M1 = F::M1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[64];
+    const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw) + r * F::TILE;
+    const long row = (long)blockIdx.x * G::RPC + r;
+    const int b = (int)(row / a.nx), i = (int)(row % a.nx);
+    const int gpm = a.nx / G::RPC;
+    const cpair *src = reinterpret_cast<const cpair *>(a.src) + row * H;
+    pdl_launch_dependents();
+    pdl_wait();
+    cpair v[16];
+#pragma unroll
+    for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+        for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = ldcg_pair(src + F::nat(j, ii, rr));
+    if constexpr (G::NAMED) F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
+    else F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+    // mirror of pass A's radix-2 layer: x[n] = e[n] + conj(w^n) o[n], x[n+H] = e[n] - conj(w^n) o[n]
+    float2 p0[16], p1[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const float2 w = a.tw_y[j + M1 * k];
+        const float tx = fmaf(v[k].re.y, w.x, v[k].im.y * w.y), ty = fmaf(v[k].im.y, w.x, -(v[k].re.y * w.y));
+        p0[k] = make_float2(v[k].re.x + tx, v[k].im.x + ty);
+        p1[k] = make_float2(v[k].re.x - tx, v[k].im.x - ty);
+    }
+    const MemberState &ms = a.fin.st[b];
+    float2 sn, st;
+    potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, (float)ms.A, (float)ms.C, sn, st);
+    float2 *dst = a.dst + row * NY;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { dst[j + M1 * k] = p0[k]; dst[H + j + M1 * k] = p1[k]; }
+    const double dn = (double)sn.x + (double)sn.y;
+    const double dt_ = (a.flags & F_CAVITY) ? ((double)st.x + (double)st.y) * (double)a.cavx[i] : 0.0;
+    block_reduce_and_finalize(a.fin, b, (int)(blockIdx.x % gpm), dn, dt_, red);
+}
+
+// ---------------------------------------------------------------- launchers
+template <int N> struct LaunchP {
+    using A = StepArgs<float, float2>;
+    static size_t row_smem() { return sizeof(float2) * RowGeomP<N>::RPC * Fft1D<N / 2, 1, cpair>::TILE; }
+    static size_t col_smem() { return sizeof(float2) * Fft1D<N, ColGeomP<N>::CPW, cpair>::TILE; }
+    static bool use_pdl(const A &a) { return (long)a.batch * a.nx * a.ny <= 65536L; }
+    template <typename K> static cudaError_t go(K kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, const A &a) {
+        cudaError_t e = Launch<float, N>::prep(kern, smem);
+        if (e != cudaSuccess) return e;
+        e = launch_pdl(kern, grid, block, smem, s, use_pdl(a), a);
+        return e != cudaSuccess ? e : cudaGetLastError();
+    }
+    static cudaError_t row_fwd(const A &a, bool imag, cudaStream_t s) {   // ny == N
+        dim3 grid((unsigned)((long)a.batch * a.nx / RowGeomP<N>::RPC)), block(RowGeomP<N>::THREADS);
+        return imag ? go(k_row_fwd_p<N, true>, grid, block, row_smem(), s, a) : go(k_row_fwd_p<N, false>, grid, block, row_smem(), s, a);
+    }
+    static cudaError_t row_inv(const A &a, bool imag, cudaStream_t s) {   // ny == N
+        dim3 grid((unsigned)((long)a.batch * a.nx / RowGeomP<N>::RPC)), block(RowGeomP<N>::THREADS);
+        return imag ? go(k_row_inv_p<N, true>, grid, block, row_smem(), s, a) : go(k_row_inv_p<N, false>, grid, block, row_smem(), s, a);
+    }
+    static cudaError_t col(const A &a, bool imag, cudaStream_t s) {       // nx == N
+        dim3 grid((unsigned)(a.ny / 2 / ColGeomP<N>::CPW), (unsigned)a.batch), block(ColGeomP<N>::THREADS);
+        return imag ? go(k_col_p<N, true>, grid, block, col_smem(), s, a) : go(k_col_p<N, false>, grid, block, col_smem(), s, a);
+    }
+};
+
+}  // namespace gpe
