@@ -162,8 +162,11 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_fwd_p(const St
     pdl_wait();
     float2 p0[16], p1[16];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) { p0[k] = __ldcg(src + j + M1 * k); p1[k] = __ldcg(src + H + j + M1 * k); }
-    {
+    for (int k = 0; k < 16; ++k) {
+        if (GPE_ABL & 32) { p0[k] = make_float2(1e-3f * k, 1e-3f * j); p1[k] = make_float2(-1e-3f * j, 2e-3f * k); }
+        else { p0[k] = __ldcg(src + j + M1 * k); p1[k] = __ldcg(src + H + j + M1 * k); }
+    }
+    if (!(GPE_ABL & 128)) {
         const MemberState &ms = a.fin.st[b];
         float2 sn, st;
         potential_pair16<IMAG, false, M1, H>(p0, p1, a, b, i, j, (float)ms.scale, (float)ms.A, (float)ms.C, sn, st);
@@ -181,6 +184,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_fwd_p(const St
     if constexpr (G::NAMED) F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
     else F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
     cpair *dst = reinterpret_cast<cpair *>(a.dst) + row * H;
+    if ((GPE_ABL & 64) && v[0].re.x != 12345.678f) return;
 #pragma unroll
     for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
@@ -206,6 +210,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         if ((GPE_ABL & 1) || (a.flags & 512)) { v[k].re = make_float2(1e-3f * k, 2e-3f * j); v[k].im = make_float2(1e-3f * c, -1e-3f * k); }
+        else if (GPE_ABL & 8192) v[k] = ldcg_pair(reinterpret_cast<const cpair *>(a.src) + ((size_t)b * NX * hy + (size_t)blockIdx.x * 16 * G::THREADS + k * G::THREADS + threadIdx.x));
         else v[k] = ldcg_pair(src + (size_t)(j + F::M1 * k) * hy);
     }
     if (a.flags & 256) {
@@ -248,7 +253,10 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
     F::inv(v, sm, j, a.tw_x, a.tw1_x, [] { if (!(GPE_ABL & 16)) __syncthreads(); });
     if (((GPE_ABL & 2) || (a.flags & 1024)) && v[0].re.x != 12345.678f) return;
 #pragma unroll
-    for (int k = 0; k < 16; ++k) st_pair(dst + (size_t)(j + F::M1 * k) * hy, v[k]);
+    for (int k = 0; k < 16; ++k) {
+        if (GPE_ABL & 8192) st_pair(reinterpret_cast<cpair *>(a.dst) + ((size_t)b * NX * hy + (size_t)blockIdx.x * 16 * G::THREADS + k * G::THREADS + threadIdx.x), v[k]);
+        else st_pair(dst + (size_t)(j + F::M1 * k) * hy, v[k]);
+    }
 }
 
 // ---------------------------------------------------------------- pass C (rows, inverse)
@@ -271,7 +279,10 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_inv_p(const St
 #pragma unroll
     for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
-        for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = ldcg_pair(src + F::nat(j, ii, rr));
+        for (int rr = 0; rr < F::RL; ++rr) {
+            if (GPE_ABL & 256) { v[ii * F::RL + rr].re = make_float2(1e-3f * rr, 1e-3f * j); v[ii * F::RL + rr].im = make_float2(-1e-3f * j, 2e-3f * ii); }
+            else v[ii * F::RL + rr] = ldcg_pair(src + F::nat(j, ii, rr));
+        }
     if constexpr (G::NAMED) F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
     else F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
     // mirror of pass A's radix-2 layer: x[n] = e[n] + conj(w^n) o[n], x[n+H] = e[n] - conj(w^n) o[n]
@@ -284,14 +295,54 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_inv_p(const St
         p1[k] = make_float2(v[k].re.x - tx, v[k].im.x - ty);
     }
     const MemberState &ms = a.fin.st[b];
-    float2 sn, st;
-    potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, (float)ms.A, (float)ms.C, sn, st);
+    float2 sn = make_float2(0.f, 0.f), st = sn;
+    if (!(GPE_ABL & 1024)) potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, (float)ms.A, (float)ms.C, sn, st);
     float2 *dst = a.dst + row * NY;
+    // Reduction first, wavefunction stores second: the partial sums of this CTA are published
+    // (store, fence, counter increment) while thread 0 has no stores in flight, so the fence does
+    // not wait for 16 KB of psi to be acknowledged by L2, and the counter's round trip overlaps
+    // the stores.  Fixed summation order everywhere (bitwise reproducible, batch == single).
+    const FinalizeParams &f = a.fin;
+    const int cim = (int)(blockIdx.x % gpm);
+    double dn = warp_sum((double)sn.x + (double)sn.y);
+    double dt_ = (a.flags & F_CAVITY) ? warp_sum(((double)st.x + (double)st.y) * (double)a.cavx[i]) : 0.0;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    constexpr int NW = G::THREADS / 32;
+    __shared__ int is_last;
+    if (lane == 0) { red[wid] = dn; red[32 + wid] = dt_; }
+    __syncthreads();
+    unsigned int old = 0;
+    if (threadIdx.x == 0 && !(GPE_ABL & 2048)) {
+        double s0 = 0.0, s1 = 0.0;
 #pragma unroll
-    for (int k = 0; k < 16; ++k) { dst[j + M1 * k] = p0[k]; dst[H + j + M1 * k] = p1[k]; }
-    const double dn = (double)sn.x + (double)sn.y;
-    const double dt_ = (a.flags & F_CAVITY) ? ((double)st.x + (double)st.y) * (double)a.cavx[i] : 0.0;
-    block_reduce_and_finalize(a.fin, b, (int)(blockIdx.x % gpm), dn, dt_, red);
+        for (int q = 0; q < NW; ++q) { s0 += red[q]; s1 += red[32 + q]; }
+        f.partials[(size_t)b * f.cpm + cim] = make_double2(s0, s1);
+        __threadfence();
+        old = atomicAdd(&f.counters[b], 1u);
+    }
+    if (!((GPE_ABL & 512) && p0[0].x != 12345.678f)) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) { dst[j + M1 * k] = p0[k]; dst[H + j + M1 * k] = p1[k]; }
+    }
+    if (threadIdx.x == 0) is_last = (old == (unsigned int)(f.cpm - 1)) && !(GPE_ABL & 2048);
+    __syncthreads();
+    if (is_last && !(GPE_ABL & 4096)) {   // the last CTA of the member: all its threads sum the partials
+        __threadfence();
+        const volatile double2 *pp = f.partials + (size_t)b * f.cpm;
+        double s0 = 0.0, s1 = 0.0;
+        for (int q = threadIdx.x; q < f.cpm; q += G::THREADS) { s0 += pp[q].x; s1 += pp[q].y; }
+        s0 = warp_sum(s0); s1 = warp_sum(s1);
+        __syncthreads();
+        if (lane == 0) { red[wid] = s0; red[32 + wid] = s1; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t0 = 0.0, t1 = 0.0;
+#pragma unroll
+            for (int q = 0; q < NW; ++q) { t0 += red[q]; t1 += red[32 + q]; }
+            finalize_member(f, b, t0, t1);
+            f.counters[b] = 0u;
+        }
+    }
 }
 
 // ---------------------------------------------------------------- launchers
