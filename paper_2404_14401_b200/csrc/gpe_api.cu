@@ -238,6 +238,40 @@ __global__ void __launch_bounds__(256) k_rescale(cx<T> *psi, size_t npts, Member
         w[q] = z;
     }
 }
+// Epilogue of a real-time gpe_evolve on the paired passes: the second potential half-step of the
+// last step, left pending by pass C (MemberState::pend), rows a5 of SURVEY.md 8(a).
+template <typename T>
+__global__ void __launch_bounds__(256) k_pending_halfstep(cx<T> *psi, int nx, int ny, int flags, const T *v2d,
+                                                          const T *vx, const T *vy, const T *latx, const T *laty,
+                                                          const T *cavx, const T *cavy, const T *g, T half_dt,
+                                                          const MemberState *st) {
+    const int b = blockIdx.y;
+    if (!st[b].pend) return;
+    const T A = (T)st[b].A_pend, Cc = (T)st[b].C_pend, gg = (flags & F_HAS_G) ? g[b] : T(0);
+    const size_t npts = (size_t)nx * ny;
+    cx<T> *w = psi + (size_t)b * npts;
+    const T *v2 = (flags & F_HAS_V2D) ? v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * npts : 0) : nullptr;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < npts; q += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(q / ny), j = (int)(q % ny);
+        T V = T(0);
+        if (flags & F_HAS_SEP) V += vx[i] + vy[j];
+        if (flags & F_LAT_X) V += A * latx[i];
+        if (flags & F_LAT_Y) V += A * laty[j];
+        if (flags & F_CAVITY) V += Cc * cavx[i] * cavy[j];
+        if (v2) V += v2[q];
+        cx<T> z = w[q];
+        const T ang = (V + gg * (z.x * z.x + z.y * z.y)) * half_dt;
+        T sn, cm1;
+        sincosm1_t(-ang, &sn, &cm1);
+        const T ox = fma(z.x, cm1, fma(-z.y, sn, z.x)), oy = fma(z.x, sn, fma(z.y, cm1, z.y));
+        z.x = ox; z.y = oy;
+        w[q] = z;
+    }
+}
+__global__ void k_clear_pend(MemberState *st, int batch) {
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < batch) st[b].pend = 0;
+}
 __global__ void k_reset_scale(MemberState *st, int batch) {
     int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b < batch) st[b].scale = 1.0;
@@ -411,6 +445,9 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     a.fin.cpm = p->nx / (paired ? oy->p_rows_per_cta : oy->rows_per_cta);
     a.fin.normalise = imag ? 1 : 0;
     a.fin.advance = 1;
+    // real time on the paired passes: pass C leaves its half-step to the next pass A (one multiply
+    // by exp(-i (V_n + V_{n+1} + 2 g |psi|^2) dt/2) instead of two; |psi|^2, hence Theta, is unchanged)
+    a.fin.merged = (paired && !imag && !getenv("GPE_NO_MERGE")) ? 1 : 0;
     a.fin.record_every = 0; a.fin.rec_first = 0; a.fin.records = nullptr;  // step kernels read *call
     auto one_step = [&](cudaStream_t st, int w, cudaEvent_t e0, cudaEvent_t e1) -> gpe_status {
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, st));
@@ -458,6 +495,15 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
             prof->e0.push_back(e0); prof->e1.push_back(e1); prof->which.push_back(w);
         }
         if ((s = one_step(p->stream, w, e0, e1)) != GPE_OK) return s;
+    }
+    if (a.fin.merged) {
+        dim3 grid(592, p->batch);
+        k_pending_halfstep<T><<<grid, 256, 0, p->stream>>>((cx<T> *)psi, p->nx, p->ny, p->flags, (const T *)p->v2d,
+            (const T *)p->vx, (const T *)p->vy, (const T *)p->latx, (const T *)p->laty, (const T *)p->cavx,
+            (const T *)p->cavy, (const T *)p->g, a.half_dt, p->st);
+        GPE_CUDA(p, cudaGetLastError());
+        k_clear_pend<<<(p->batch + 127) / 128, 128, 0, p->stream>>>(p->st, p->batch);
+        GPE_CUDA(p, cudaGetLastError());
     }
     if (imag) {
         dim3 grid(256, p->batch);

@@ -88,6 +88,7 @@ __device__ inline void finalize_member(const FinalizeParams &f, int b, double su
         im_a = -num * K / den;
         C = 2.0 * eta * re_a;
     }
+    if (f.advance && f.merged) { s.A_pend = s.A; s.C_pend = s.C; s.pend = 1; } else s.pend = 0;
     s.scale = scale; s.A = A; s.C = C; s.norm = norm; s.theta = theta;
     s.re_alpha = re_a; s.im_alpha = im_a; s.step = n1;
     if (!f.advance && b == 0) {

@@ -58,15 +58,17 @@ __device__ __forceinline__ void st_pair(cpair *p, cpair v) {
 // REDUCE: sn += |psi_new|^2, st += cos(k_c y) |psi_new|^2 (one lane per point).
 template <bool IMAG, bool REDUCE, int M1, int H>
 __device__ __forceinline__ void potential_pair16(float2 (&p0)[16], float2 (&p1)[16], const StepArgs<float, float2> &a,
-                                                 int b, int i, int j, float scale, float A, float Cc,
+                                                 int b, int i, int j, float scale, float fac, float A, float Cc,
                                                  float2 &sn, float2 &st) {
     const int flags = a.flags;
     float vrow = 0.f;
-    if (flags & F_HAS_SEP) vrow += a.vx[i];
+    // fac = 1, or 2 when this multiply also carries the pending second half-step of the previous
+    // step (then A, Cc are the sums of the two steps' coefficients): static terms and g count twice
+    if (flags & F_HAS_SEP) vrow += fac * a.vx[i];
     if (flags & F_LAT_X) vrow += A * a.latx[i];
     const float crow = (flags & F_CAVITY) ? Cc * a.cavx[i] : 0.f;
     const float Ay = (flags & F_LAT_Y) ? A : 0.f;
-    const float g = (flags & F_HAS_G) ? a.g[b] : 0.f;
+    const float g = (flags & F_HAS_G) ? fac * a.g[b] : 0.f;
     const float hdt = a.half_dt;
     const float4 *__restrict__ yt = reinterpret_cast<const float4 *>(a.ytab2);
     // in chunks of CH points per half row: bounds the live angles (registers); the tier vote is per chunk
@@ -81,13 +83,13 @@ __device__ __forceinline__ void potential_pair16(float2 (&p0)[16], float2 (&p1)[
             const float2 cav = *reinterpret_cast<const float2 *>(yt + 2 * n + 1);
             if constexpr (IMAG) { p0[k].x *= scale; p0[k].y *= scale; p1[k].x *= scale; p1[k].y *= scale; }
             const float2 d = make_float2(fmaf(p0[k].x, p0[k].x, p0[k].y * p0[k].y), fmaf(p1[k].x, p1[k].x, p1[k].y * p1[k].y));
-            const float2 V = rfmas(cav, crow, rfmas(make_float2(t0.z, t0.w), Ay, radd(make_float2(t0.x, t0.y), make_float2(vrow, vrow))));
+            const float2 V = rfmas(cav, crow, rfmas(make_float2(t0.z, t0.w), Ay, rfmas(make_float2(t0.x, t0.y), fac, make_float2(vrow, vrow))));
             w[k] = rmuls(rfmas(d, g, V), hdt);
         }
         if (flags & F_HAS_V2D) {
             const float *__restrict__ v2 = a.v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * a.nx * a.ny : 0) + (size_t)i * a.ny;
     #pragma unroll
-            for (int k = k0; k < k0 + CH; ++k) w[k] = rfmas(make_float2(v2[j + M1 * k], v2[j + M1 * k + H]), hdt, w[k]);
+            for (int k = k0; k < k0 + CH; ++k) w[k] = rfmas(make_float2(v2[j + M1 * k], v2[j + M1 * k + H]), fac * hdt, w[k]);
         }
         if constexpr (IMAG) {
     #pragma unroll
@@ -146,6 +148,21 @@ __device__ __forceinline__ void potential_pair16(float2 (&p0)[16], float2 (&p1)[
     }
 }
 
+// sums only (merged real-time half-steps: pass C leaves the multiply to the next pass A; a phase
+// factor does not change |psi|^2, so norm and Theta of the stored array are those of psi_{n+1})
+template <int M1>
+__device__ __forceinline__ void reduce_pair16(const float2 (&p0)[16], const float2 (&p1)[16], const StepArgs<float, float2> &a,
+                                              int j, float2 &sn, float2 &st) {
+    const float4 *__restrict__ yt = reinterpret_cast<const float4 *>(a.ytab2);
+    sn = make_float2(0.f, 0.f); st = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const float2 d = make_float2(fmaf(p0[k].x, p0[k].x, p0[k].y * p0[k].y), fmaf(p1[k].x, p1[k].x, p1[k].y * p1[k].y));
+        sn = radd(sn, d);
+        if (a.flags & F_CAVITY) st = rfma(d, *reinterpret_cast<const float2 *>(yt + 2 * (j + M1 * k) + 1), st);
+    }
+}
+
 // ---------------------------------------------------------------- pass A (rows, forward)
 template <int NY, bool IMAG>
 __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_fwd_p(const StepArgs<float, float2> a) {
@@ -169,7 +186,9 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_fwd_p(const St
     if (!(GPE_ABL & 128)) {
         const MemberState &ms = a.fin.st[b];
         float2 sn, st;
-        potential_pair16<IMAG, false, M1, H>(p0, p1, a, b, i, j, (float)ms.scale, (float)ms.A, (float)ms.C, sn, st);
+        const bool pend = !IMAG && ms.pend;
+        potential_pair16<IMAG, false, M1, H>(p0, p1, a, b, i, j, (float)ms.scale, pend ? 2.f : 1.f,
+                                             (float)(pend ? ms.A + ms.A_pend : ms.A), (float)(pend ? ms.C + ms.C_pend : ms.C), sn, st);
     }
     // radix-2 decimation in frequency across the two halves of the row: lane 0 <- x[n] + x[n+H],
     // lane 1 <- (x[n] - x[n+H]) w_NY^n; scalar instructions, they write the split lane layout
@@ -260,7 +279,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
 }
 
 // ---------------------------------------------------------------- pass C (rows, inverse)
-template <int NY, bool IMAG>
+template <int NY, bool IMAG, bool MERGED>
 __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_inv_p(const StepArgs<float, float2> a) {
     using G = RowGeomP<NY>;
     using F = Fft1D<G::H, 1, cpair>;
@@ -296,7 +315,8 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_inv_p(const St
     }
     const MemberState &ms = a.fin.st[b];
     float2 sn = make_float2(0.f, 0.f), st = sn;
-    if (!(GPE_ABL & 1024)) potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, (float)ms.A, (float)ms.C, sn, st);
+    if constexpr (MERGED) reduce_pair16<M1>(p0, p1, a, j, sn, st);
+    else if (!(GPE_ABL & 1024)) potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, 1.f, (float)ms.A, (float)ms.C, sn, st);
     float2 *dst = a.dst + row * NY;
     // Reduction first, wavefunction stores second: the partial sums of this CTA are published
     // (store, fence, counter increment) while thread 0 has no stores in flight, so the fence does
@@ -363,7 +383,8 @@ template <int N> struct LaunchP {
     }
     static cudaError_t row_inv(const A &a, bool imag, cudaStream_t s) {   // ny == N
         dim3 grid((unsigned)((long)a.batch * a.nx / RowGeomP<N>::RPC)), block(RowGeomP<N>::THREADS);
-        return imag ? go(k_row_inv_p<N, true>, grid, block, row_smem(), s, a) : go(k_row_inv_p<N, false>, grid, block, row_smem(), s, a);
+        if (imag) return go(k_row_inv_p<N, true, false>, grid, block, row_smem(), s, a);
+        return a.fin.merged ? go(k_row_inv_p<N, false, true>, grid, block, row_smem(), s, a) : go(k_row_inv_p<N, false, false>, grid, block, row_smem(), s, a);
     }
     static cudaError_t col(const A &a, bool imag, cudaStream_t s) {       // nx == N
         dim3 grid((unsigned)(a.ny / 2 / ColGeomP<N>::CPW), (unsigned)a.batch), block(ColGeomP<N>::THREADS);

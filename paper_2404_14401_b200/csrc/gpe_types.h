@@ -14,6 +14,10 @@ struct MemberState {
     double theta;      // cavity overlap Theta (Eq. 14)
     double re_alpha, im_alpha;
     long long step;    // step counter n
+    // real-time merged half-steps (gpe_pair.cuh): when pend == 1 the stored psi still lacks the
+    // second potential half-step of the step just taken, whose coefficients are A_pend, C_pend
+    double A_pend, C_pend;
+    int pend;
 };
 
 // Per-gpe_evolve-call parameters kept in device memory (written by the prologue kernel), so that
@@ -43,6 +47,7 @@ struct FinalizeParams {
     int batch;
     int normalise;            // 1: imaginary-time step (scale <- 1/sqrt(norm), Theta /= norm)
     int advance;              // 1: a step was taken (step += 1); 0: prologue reduction
+    int merged;               // 1: pass C left the second half-step pending (real time, paired passes)
     long long step0;          // used when advance == 0: sets the step counter
 };
 
