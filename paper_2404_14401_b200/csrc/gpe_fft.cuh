@@ -260,6 +260,77 @@ template <int N, int S, typename E> struct Fft1D {
         }
     }
 
+    // ---- pair-mapped outer stage (row passes of gpe_pair.cuh).  Two transforms whose tiles are sm0
+    // and sm1 are worked on by 2*TPF threads (slot u in [0, 2 TPF)); in the LAST forward stage (and
+    // the mirrored FIRST inverse stage) thread u takes butterflies t = u + 2 TPF i, i < GL/2, of
+    // BOTH transforms instead of GL butterflies of its own, so that it holds the same output
+    // indices of the two transforms: register (2 i + w) * RL + r = X_w[nat_t(t, r)].  Needs GL >= 2.
+    static constexpr int RLM = NST == 3 ? M1 / R2 : M1;   // Mp of the last stage
+    __device__ __forceinline__ static int nat_t(int t, int r) {
+        int k1 = t & 15, u = t >> 4;
+        return NST == 3 ? k1 + 16 * u + 16 * R2 * r : k1 + 16 * r;
+    }
+    __device__ __forceinline__ static void last_fwd_pair(E *v, const SE *sm0, const SE *sm1, int u) {
+        constexpr int M = RLM / RL;
+#pragma unroll
+        for (int i = 0; i < GL / 2; ++i) {
+            int q, b = base_slot<RL, RLM>(u + 2 * TPF * i, q);
+#pragma unroll
+            for (int a = 0; a < RL; ++a) {
+                v[(2 * i) * RL + a] = sld<PLANE, E>(sm0, phys(b + M * a));
+                v[(2 * i + 1) * RL + a] = sld<PLANE, E>(sm1, phys(b + M * a));
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < GL; ++i) dft<RL, -1, E>(v + i * RL);
+    }
+    __device__ __forceinline__ static void first_inv_pair(E *v, SE *sm0, SE *sm1, int u) {
+        constexpr int M = RLM / RL;
+#pragma unroll
+        for (int i = 0; i < GL; ++i) dft<RL, +1, E>(v + i * RL);
+#pragma unroll
+        for (int i = 0; i < GL / 2; ++i) {
+            int q, b = base_slot<RL, RLM>(u + 2 * TPF * i, q);
+#pragma unroll
+            for (int a = 0; a < RL; ++a) {
+                sst<PLANE>(sm0, phys(b + M * a), v[(2 * i) * RL + a]);
+                sst<PLANE>(sm1, phys(b + M * a), v[(2 * i + 1) * RL + a]);
+            }
+        }
+    }
+    // forward transform whose last stage is pair-mapped; SYNC must cover both transforms' threads
+    template <typename Sync>
+    __device__ __forceinline__ static void fwd_pairlast(E *v, SE *sm, const SE *sm0, const SE *sm1, int j, int u,
+                                                        const C *__restrict__ tw, const C *__restrict__ tw1, Sync SYNC) {
+        dft<16, -1, E>(v);
+#pragma unroll
+        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], ldtw(tw1, k * M1 + j));
+#pragma unroll
+        for (int k = 0; k < 16; ++k) sst<PLANE>(sm, phys(j + M1 * k), v[k]);
+        SYNC();
+        if constexpr (NST == 3) {
+            stage_fwd<R2, M1, false>(v, sm, j, tw);
+            SYNC();
+        }
+        last_fwd_pair(v, sm0, sm1, u);
+    }
+    // mirror: in: v[(2 i + w) * RL + r] = X_w[nat_t(u + 2 TPF i, r)]; out: v[a] of the own transform
+    template <typename Sync>
+    __device__ __forceinline__ static void inv_pairfirst(E *v, SE *sm, SE *sm0, SE *sm1, int j, int u,
+                                                         const C *__restrict__ tw, const C *__restrict__ tw1, Sync SYNC) {
+        first_inv_pair(v, sm0, sm1, u);
+        SYNC();
+        if constexpr (NST == 3) {
+            stage_inv<R2, M1, false>(v, sm, j, tw);
+            SYNC();
+        }
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = sld<PLANE, E>(sm, phys(j + M1 * k));
+#pragma unroll
+        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], ldtw(tw1, k * M1 + j));
+        dft<16, +1, E>(v);
+    }
+
     // in: v[a] = x[j + (N/16) a].  out: v[i*RL + r] = X[nat(j,i,r)] (unnormalised, e^{-i}).
     // All threads that share `sm` must call this together: SYNC() is the barrier between them
     // (__syncthreads, or a named barrier over the threads of one transform).

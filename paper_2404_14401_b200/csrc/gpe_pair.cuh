@@ -11,8 +11,11 @@
 //                     by two independent NY/2-point transforms.  Lane 0 ends with psi^[2k'],
 //                     lane 1 with psi^[2k'+1]: exactly the column pair pass B wants.
 //   pass C (rows):    the mirror of pass A.
-// Intermediate layout (between A and C, inside the caller's psi buffer, same bytes per row):
-//   [batch][nx][ny/2] of cpair = (Re psi^[i][2k'], Re psi^[i][2k'+1], Im .., Im ..).
+// Intermediate layout (between A and C, inside the caller's psi buffer, same bytes per row pair):
+//   [batch][nx/2][ny/2][2] of cpair; element (i, k') = (Re psi^[i][2k'], Re psi^[i][2k'+1], Im .., Im ..)
+//   sits at ((i/2) * ny/2 + k') * 2 + i%2: rows 2m and 2m+1 are interleaved so that the column pass,
+//   whose tile is only two column pairs wide, still moves 64 contiguous bytes per row pair
+//   (measured on B200: 32-byte segments cost pass B 4 us of 35 at 2048^2).
 // Same mathematics as gpe_kernels.cuh (PAPER.md:62-76 Eqs. 2-4, :116, :183-186 Eq. 14).
 #pragma once
 #include "gpe_kernels.cuh"
@@ -32,6 +35,10 @@ template <int N> struct RowGeomP {
     static constexpr int RPC = (128 / TPF) < 1 ? 1 : (128 / TPF);    // rows per CTA
     static constexpr int THREADS = RPC * TPF;                        // 128
     static constexpr bool NAMED = RPC > 1 && TPF % 32 == 0;          // rows own whole warps
+    // outer stage pair-mapped (Fft1D::last_fwd_pair): a thread holds the same output indices of rows
+    // 2m and 2m+1, i.e. 32 contiguous bytes of the row-pair-interleaved intermediate array
+    static constexpr bool PAIRMAP = RPC >= 2 && (16 / (Fact<H>::R3 > 1 ? Fact<H>::R3 : Fact<H>::R2)) >= 2;
+    static constexpr bool PAIRNAMED = RPC > 2 && (2 * TPF) % 32 == 0;  // a row pair owns whole warps
 };
 template <int N> struct ColGeomP {
     static constexpr int TPF = N / 16;                               // threads per column pair
@@ -50,6 +57,20 @@ __device__ __forceinline__ cpair ldcg_pair(const cpair *p) {
 __device__ __forceinline__ void st_pair(cpair *p, cpair v) {
     *reinterpret_cast<float4 *>(p) = make_float4(v.re.x, v.re.y, v.im.x, v.im.y);
 }
+
+// 256-bit accesses (sm_100): the two cpairs of one column pair of rows 2m and 2m+1, 32 contiguous bytes
+__device__ __forceinline__ void st_pair2(cpair *p, cpair v0, cpair v1) {
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(v0.re.x), "f"(v0.re.y), "f"(v0.im.x),
+                 "f"(v0.im.y), "f"(v1.re.x), "f"(v1.re.y), "f"(v1.im.x), "f"(v1.im.y) : "memory");
+}
+__device__ __forceinline__ void ldcg_pair2(const cpair *p, cpair &v0, cpair &v1) {
+    asm volatile("ld.global.cg.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];" : "=f"(v0.re.x), "=f"(v0.re.y), "=f"(v0.im.x),
+                 "=f"(v0.im.y), "=f"(v1.re.x), "=f"(v1.re.y), "=f"(v1.im.x), "=f"(v1.im.y) : "l"(p) : "memory");
+}
+
+// position of element (row i, column pair kp) of the intermediate array, hy = ny/2 (rows counted
+// through the whole batch: nx is even, so a row pair never straddles two members)
+__device__ __forceinline__ size_t ipos(long i, int kp, size_t hy) { return ((size_t)(i >> 1) * hy + kp) * 2 + (i & 1); }
 
 // Potential half-step (rows a1 / a5) on the 32 points of one thread: p0[k] at y = j + M1 k,
 // p1[k] at y + H, same row i.  ytab2[n] = {vy[n], vy[n+H], cos^2(k_l y_n), cos^2(k_l y_{n+H})},
@@ -200,14 +221,33 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_fwd_p(const St
         v[k].re = make_float2(p0[k].x + p1[k].x, fmaf(dx, w.x, -(dy * w.y)));
         v[k].im = make_float2(p0[k].y + p1[k].y, fmaf(dx, w.y, dy * w.x));
     }
-    if constexpr (G::NAMED) F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
-    else F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
-    cpair *dst = reinterpret_cast<cpair *>(a.dst) + row * H;
-    if ((GPE_ABL & 64) && v[0].re.x != 12345.678f) return;
+    cpair *dst = reinterpret_cast<cpair *>(a.dst);
+    if constexpr (G::PAIRMAP) {
+        const int rp = r >> 1, u = j + (r & 1) * G::TPF;
+        float2 *sm0 = reinterpret_cast<float2 *>(smem_raw) + (2 * rp) * F::TILE, *sm1 = sm0 + F::TILE;
+        // every barrier spans the row pair: its first one also orders the pair's loads before its stores
+        if constexpr (G::PAIRNAMED) F::fwd_pairlast(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, [rp] { bar_named(1 + rp, 2 * G::TPF); });
+        else F::fwd_pairlast(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+        if ((GPE_ABL & 64) && v[0].re.x != 12345.678f) return;
+        const long rowp = (long)blockIdx.x * G::RPC + 2 * rp;
 #pragma unroll
-    for (int ii = 0; ii < F::GL; ++ii)
+        for (int ii = 0; ii < F::GL / 2; ++ii)
 #pragma unroll
-        for (int rr = 0; rr < F::RL; ++rr) st_pair(dst + F::nat(j, ii, rr), v[ii * F::RL + rr]);
+            for (int rr = 0; rr < F::RL; ++rr) {
+                const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H);
+                st_pair2(dst + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
+            }
+    } else {
+        // the rows of a pair are interleaved in the output: no store before every row's loads are done
+        if (G::RPC > 1) __syncthreads();
+        if constexpr (G::NAMED) F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
+        else F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+        if ((GPE_ABL & 64) && v[0].re.x != 12345.678f) return;
+#pragma unroll
+        for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) st_pair(dst + ipos(row, F::nat(j, ii, rr), H), v[ii * F::RL + rr]);
+    }
 }
 
 // ---------------------------------------------------------------- pass B (columns)
@@ -220,8 +260,8 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
     const int cp = blockIdx.x * G::CPW + c;      // column pair: columns 2 cp, 2 cp + 1
     const int b = blockIdx.y;
     const size_t hy = a.ny / 2;
-    const cpair *src = reinterpret_cast<const cpair *>(a.src) + (size_t)b * NX * hy + cp;
-    cpair *dst = reinterpret_cast<cpair *>(a.dst) + (size_t)b * NX * hy + cp;
+    const cpair *src = reinterpret_cast<const cpair *>(a.src) + (size_t)b * NX * hy;
+    cpair *dst = reinterpret_cast<cpair *>(a.dst) + (size_t)b * NX * hy;
     float2 *sm = reinterpret_cast<float2 *>(smem_raw) + c;
     cpair v[16];
     pdl_launch_dependents();
@@ -230,11 +270,11 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
     for (int k = 0; k < 16; ++k) {
         if ((GPE_ABL & 1) || (a.flags & 512)) { v[k].re = make_float2(1e-3f * k, 2e-3f * j); v[k].im = make_float2(1e-3f * c, -1e-3f * k); }
         else if (GPE_ABL & 8192) v[k] = ldcg_pair(reinterpret_cast<const cpair *>(a.src) + ((size_t)b * NX * hy + (size_t)blockIdx.x * 16 * G::THREADS + k * G::THREADS + threadIdx.x));
-        else v[k] = ldcg_pair(src + (size_t)(j + F::M1 * k) * hy);
+        else v[k] = ldcg_pair(src + ipos(j + F::M1 * k, cp, hy));
     }
     if (a.flags & 256) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) st_pair(dst + (size_t)(j + F::M1 * k) * hy, v[k]);
+        for (int k = 0; k < 16; ++k) st_pair(dst + ipos(j + F::M1 * k, cp, hy), v[k]);
         return;
     }
     F::fwd(v, sm, j, a.tw_x, a.tw1_x, [] { if (!(GPE_ABL & 16)) __syncthreads(); });
@@ -274,7 +314,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         if (GPE_ABL & 8192) st_pair(reinterpret_cast<cpair *>(a.dst) + ((size_t)b * NX * hy + (size_t)blockIdx.x * 16 * G::THREADS + k * G::THREADS + threadIdx.x), v[k]);
-        else st_pair(dst + (size_t)(j + F::M1 * k) * hy, v[k]);
+        else st_pair(dst + ipos(j + F::M1 * k, cp, hy), v[k]);
     }
 }
 
@@ -291,19 +331,36 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_inv_p(const St
     const long row = (long)blockIdx.x * G::RPC + r;
     const int b = (int)(row / a.nx), i = (int)(row % a.nx);
     const int gpm = a.nx / G::RPC;
-    const cpair *src = reinterpret_cast<const cpair *>(a.src) + row * H;
+    const cpair *src = reinterpret_cast<const cpair *>(a.src);
     pdl_launch_dependents();
     pdl_wait();
     cpair v[16];
+    if constexpr (G::PAIRMAP) {
+        // mirror of pass A: 32 contiguous bytes (rows 2m, 2m+1, same column pair) per thread and index
+        const int rp = r >> 1, u = j + (r & 1) * G::TPF;
+        float2 *sm0 = reinterpret_cast<float2 *>(smem_raw) + (2 * rp) * F::TILE, *sm1 = sm0 + F::TILE;
+        const long rowp = (long)blockIdx.x * G::RPC + 2 * rp;
 #pragma unroll
-    for (int ii = 0; ii < F::GL; ++ii)
+        for (int ii = 0; ii < F::GL / 2; ++ii)
 #pragma unroll
-        for (int rr = 0; rr < F::RL; ++rr) {
-            if (GPE_ABL & 256) { v[ii * F::RL + rr].re = make_float2(1e-3f * rr, 1e-3f * j); v[ii * F::RL + rr].im = make_float2(-1e-3f * j, 2e-3f * ii); }
-            else v[ii * F::RL + rr] = ldcg_pair(src + F::nat(j, ii, rr));
-        }
-    if constexpr (G::NAMED) F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
-    else F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+            for (int rr = 0; rr < F::RL; ++rr) {
+                const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H);
+                if (GPE_ABL & 256) { v[(2 * ii) * F::RL + rr].re = make_float2(1e-3f * rr, 1e-3f * j); v[(2 * ii) * F::RL + rr].im = make_float2(-1e-3f * j, 2e-3f * ii); v[(2 * ii + 1) * F::RL + rr] = v[(2 * ii) * F::RL + rr]; }
+                else ldcg_pair2(src + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
+            }
+        if constexpr (G::PAIRNAMED) F::inv_pairfirst(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, [rp] { bar_named(1 + rp, 2 * G::TPF); });
+        else F::inv_pairfirst(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+    } else {
+#pragma unroll
+        for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) {
+                if (GPE_ABL & 256) { v[ii * F::RL + rr].re = make_float2(1e-3f * rr, 1e-3f * j); v[ii * F::RL + rr].im = make_float2(-1e-3f * j, 2e-3f * ii); }
+                else v[ii * F::RL + rr] = ldcg_pair(src + ipos(row, F::nat(j, ii, rr), H));
+            }
+        if constexpr (G::NAMED) F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
+        else F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+    }
     // mirror of pass A's radix-2 layer: x[n] = e[n] + conj(w^n) o[n], x[n+H] = e[n] - conj(w^n) o[n]
     float2 p0[16], p1[16];
 #pragma unroll
