@@ -298,28 +298,29 @@ template <int N, int S, typename E> struct Fft1D {
             }
         }
     }
-    // forward transform whose last stage is pair-mapped; SYNC must cover both transforms' threads
-    template <typename Sync>
+    // forward transform whose last stage is pair-mapped; SYNC covers the threads of the own
+    // transform, SYNC2 (before the pair-mapped stage) those of both transforms
+    template <typename Sync, typename Sync2>
     __device__ __forceinline__ static void fwd_pairlast(E *v, SE *sm, const SE *sm0, const SE *sm1, int j, int u,
-                                                        const C *__restrict__ tw, const C *__restrict__ tw1, Sync SYNC) {
+                                                        const C *__restrict__ tw, const C *__restrict__ tw1, Sync SYNC, Sync2 SYNC2) {
         dft<16, -1, E>(v);
 #pragma unroll
         for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], ldtw(tw1, k * M1 + j));
 #pragma unroll
         for (int k = 0; k < 16; ++k) sst<PLANE>(sm, phys(j + M1 * k), v[k]);
-        SYNC();
         if constexpr (NST == 3) {
-            stage_fwd<R2, M1, false>(v, sm, j, tw);
             SYNC();
+            stage_fwd<R2, M1, false>(v, sm, j, tw);
         }
+        SYNC2();
         last_fwd_pair(v, sm0, sm1, u);
     }
     // mirror: in: v[(2 i + w) * RL + r] = X_w[nat_t(u + 2 TPF i, r)]; out: v[a] of the own transform
-    template <typename Sync>
+    template <typename Sync, typename Sync2>
     __device__ __forceinline__ static void inv_pairfirst(E *v, SE *sm, SE *sm0, SE *sm1, int j, int u,
-                                                         const C *__restrict__ tw, const C *__restrict__ tw1, Sync SYNC) {
+                                                         const C *__restrict__ tw, const C *__restrict__ tw1, Sync SYNC, Sync2 SYNC2) {
         first_inv_pair(v, sm0, sm1, u);
-        SYNC();
+        SYNC2();
         if constexpr (NST == 3) {
             stage_inv<R2, M1, false>(v, sm, j, tw);
             SYNC();

@@ -65,6 +65,26 @@ __device__ inline double schedule_at(const FinalizeParams &f, int b, double n) {
     return amp[i] + t * (amp[i + 1] - amp[i]);
 }
 
+// The part of row a0 that does not depend on the sums: A_n and the cavity constants of step n,
+// alpha_n = N eta_n Theta_n / (Delta + i kappa) = (kre + i kim) Theta_n, C_n = 2 eta_n Re alpha_n = kc Theta_n
+// (Eqs. 13-14).
+__device__ inline void step_coefficients(const FinalizeParams &f, int b, long long n, double &A, double &kre, double &kim, double &kc) {
+    A = schedule_at(f, b, (double)n);
+    kre = kim = kc = 0.0;
+    if (f.cavity_on) {
+        const double eta = f.eta_mode == 0 ? f.eta_or_u[b] : sqrt(fabs(A) * f.eta_or_u[b]);
+        const double D = f.delta[b], K = f.kappa[b], den = D * D + K * K, ne = f.n_atoms[b] * eta;
+        kre = ne * D / den;                       // 1 / (D + iK) = (D - iK) / (D^2 + K^2)
+        kim = -ne * K / den;
+        kc = 2.0 * eta * kre;
+    }
+}
+// Called by one thread of pass B per member while step n runs: coefficients of step n + 1.
+__device__ inline void prepare_member(const FinalizeParams &f, int b) {
+    MemberState &s = f.st[b];
+    step_coefficients(f, b, s.step + 1, s.nA, s.nKre, s.nKim, s.nKc);
+}
+
 // Called by one thread of the last block of member b with the raw sums over the stored psi.
 __device__ inline void finalize_member(const FinalizeParams &f, int b, double sum_n, double sum_t) {
     MemberState &s = f.st[b];
@@ -78,15 +98,13 @@ __device__ inline void finalize_member(const FinalizeParams &f, int b, double su
         theta = theta / norm;
         norm = 1.0;
     }
-    double A = schedule_at(f, b, (double)n1);
-    double eta = 0.0, re_a = 0.0, im_a = 0.0, C = 0.0;
-    if (f.cavity_on) {
-        eta = f.eta_mode == 0 ? f.eta_or_u[b] : sqrt(fabs(A) * f.eta_or_u[b]);
-        double D = f.delta[b], K = f.kappa[b], num = f.n_atoms[b] * eta * theta;
-        double den = D * D + K * K;               // num / (D + iK) = num (D - iK) / (D^2 + K^2)
-        re_a = num * D / den;
-        im_a = -num * K / den;
-        C = 2.0 * eta * re_a;
+    double A, re_a = 0.0, im_a = 0.0, C = 0.0;
+    if (f.advance && f.prepared) {
+        A = s.nA; re_a = s.nKre * theta; im_a = s.nKim * theta; C = s.nKc * theta;
+    } else {
+        double kre, kim, kc;
+        step_coefficients(f, b, n1, A, kre, kim, kc);
+        re_a = kre * theta; im_a = kim * theta; C = kc * theta;
     }
     if (f.advance && f.merged) { s.A_pend = s.A; s.C_pend = s.C; s.pend = 1; } else s.pend = 0;
     s.scale = scale; s.A = A; s.C = C; s.norm = norm; s.theta = theta;
@@ -396,6 +414,7 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<
     C v[16];
     pdl_launch_dependents();
     pdl_wait();
+    if (MODE == 0 && blockIdx.x == 0 && threadIdx.x == 0 && a.fin.prepared) prepare_member(a.fin, b);
 #pragma unroll
     for (int k = 0; k < 16; ++k) v[k] = __ldcg(src + (size_t)(j + F::M1 * k) * ny);
     F::fwd(v, sm, j, a.tw_x, a.tw1_x);

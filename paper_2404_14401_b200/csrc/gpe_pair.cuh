@@ -23,6 +23,9 @@
 #ifndef GPE_ABL
 #define GPE_ABL 0   // ablation experiments only (timing with wrong numerics)
 #endif
+#ifndef GPE_ROWP_MINB
+#define GPE_ROWP_MINB 4
+#endif
 #ifndef GPE_COLP_THREADS
 #define GPE_COLP_THREADS 256
 #endif
@@ -186,7 +189,7 @@ __device__ __forceinline__ void reduce_pair16(const float2 (&p0)[16], const floa
 
 // ---------------------------------------------------------------- pass A (rows, forward)
 template <int NY, bool IMAG>
-__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_fwd_p(const StepArgs<float, float2> a) {
+__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, GPE_ROWP_MINB) k_row_fwd_p(const StepArgs<float, float2> a) {
     using G = RowGeomP<NY>;
     using F = Fft1D<G::H, 1, cpair>;
     constexpr int H = G::H, M1 = F::M1;
@@ -226,8 +229,9 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_fwd_p(const St
         const int rp = r >> 1, u = j + (r & 1) * G::TPF;
         float2 *sm0 = reinterpret_cast<float2 *>(smem_raw) + (2 * rp) * F::TILE, *sm1 = sm0 + F::TILE;
         // every barrier spans the row pair: its first one also orders the pair's loads before its stores
-        if constexpr (G::PAIRNAMED) F::fwd_pairlast(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, [rp] { bar_named(1 + rp, 2 * G::TPF); });
-        else F::fwd_pairlast(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+        auto sync_row = [r] { if constexpr (G::NAMED) bar_named(1 + r, G::TPF); else __syncthreads(); };
+        auto sync_pair = [rp] { if constexpr (G::PAIRNAMED) bar_named(9 + rp, 2 * G::TPF); else __syncthreads(); };
+        F::fwd_pairlast(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, sync_row, sync_pair);
         if ((GPE_ABL & 64) && v[0].re.x != 12345.678f) return;
         const long rowp = (long)blockIdx.x * G::RPC + 2 * rp;
 #pragma unroll
@@ -266,6 +270,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
     cpair v[16];
     pdl_launch_dependents();
     pdl_wait();
+    if (blockIdx.x == 0 && threadIdx.x == 0 && a.fin.prepared) prepare_member(a.fin, b);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         if ((GPE_ABL & 1) || (a.flags & 512)) { v[k].re = make_float2(1e-3f * k, 2e-3f * j); v[k].im = make_float2(1e-3f * c, -1e-3f * k); }
@@ -320,7 +325,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
 
 // ---------------------------------------------------------------- pass C (rows, inverse)
 template <int NY, bool IMAG, bool MERGED>
-__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_inv_p(const StepArgs<float, float2> a) {
+__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, GPE_ROWP_MINB) k_row_inv_p(const StepArgs<float, float2> a) {
     using G = RowGeomP<NY>;
     using F = Fft1D<G::H, 1, cpair>;
     constexpr int H = G::H, M1 = F::M1;
@@ -348,8 +353,9 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, 4) k_row_inv_p(const St
                 if (GPE_ABL & 256) { v[(2 * ii) * F::RL + rr].re = make_float2(1e-3f * rr, 1e-3f * j); v[(2 * ii) * F::RL + rr].im = make_float2(-1e-3f * j, 2e-3f * ii); v[(2 * ii + 1) * F::RL + rr] = v[(2 * ii) * F::RL + rr]; }
                 else ldcg_pair2(src + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
             }
-        if constexpr (G::PAIRNAMED) F::inv_pairfirst(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, [rp] { bar_named(1 + rp, 2 * G::TPF); });
-        else F::inv_pairfirst(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+        auto sync_row = [r] { if constexpr (G::NAMED) bar_named(1 + r, G::TPF); else __syncthreads(); };
+        auto sync_pair = [rp] { if constexpr (G::PAIRNAMED) bar_named(9 + rp, 2 * G::TPF); else __syncthreads(); };
+        F::inv_pairfirst(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, sync_row, sync_pair);
     } else {
 #pragma unroll
         for (int ii = 0; ii < F::GL; ++ii)

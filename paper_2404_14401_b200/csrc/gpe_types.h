@@ -18,6 +18,10 @@ struct MemberState {
     // second potential half-step of the step just taken, whose coefficients are A_pend, C_pend
     double A_pend, C_pend;
     int pend;
+    // coefficients of step `step + 1` that do not depend on the sums, prepared by one thread of
+    // pass B while the step runs (prepare_member), so the last block of pass C has little left to do:
+    // A_{n+1}; Re alpha = nKre Theta, Im alpha = nKim Theta, C = nKc Theta
+    double nA, nKre, nKim, nKc;
 };
 
 // Per-gpe_evolve-call parameters kept in device memory (written by the prologue kernel), so that
@@ -47,6 +51,7 @@ struct FinalizeParams {
     int batch;
     int normalise;            // 1: imaginary-time step (scale <- 1/sqrt(norm), Theta /= norm)
     int advance;              // 1: a step was taken (step += 1); 0: prologue reduction
+    int prepared;             // 1: pass B has run prepare_member for the step being finalised
     int merged;               // 1: pass C left the second half-step pending (real time, paired passes)
     long long step0;          // used when advance == 0: sets the step counter
 };
