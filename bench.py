@@ -162,7 +162,7 @@ def run_reference(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
 # (profiles/): pass index -> bytes; each pass reads psi once from DRAM after ncu's cache flush and
 # writes nothing back (the 32 MiB array stays in L2), see profiles/r01_pair.md.
-TRAFFIC_BYTES_PER_LAUNCH = {0: 33.7e6, 1: 34.4e6, 2: 38.8e6}
+TRAFFIC_BYTES_PER_LAUNCH = {0: 33.67e6, 1: 33.67e6, 2: 33.66e6}
 
 
 def run_ours(args):

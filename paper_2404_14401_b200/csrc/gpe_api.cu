@@ -19,7 +19,7 @@ using namespace gpe;
 namespace {
 
 constexpr int kMaxCpm = 1024;   // partial-sum slots per member
-constexpr int kReduceCtas = 128;  // CTAs per member of the prologue reduction
+constexpr int kReduceCtas = 1024;  // CTAs per member of the prologue reduction
 constexpr int kStepsPerGraph = 8;  // split-steps per CUDA graph launch
 constexpr double kPi = 3.14159265358979323846;
 

@@ -264,8 +264,10 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
     const int cp = blockIdx.x * G::CPW + c;      // column pair: columns 2 cp, 2 cp + 1
     const int b = blockIdx.y;
     const size_t hy = a.ny / 2;
-    const cpair *src = reinterpret_cast<const cpair *>(a.src) + (size_t)b * NX * hy;
-    cpair *dst = reinterpret_cast<cpair *>(a.dst) + (size_t)b * NX * hy;
+    // rows j + M1 k, k = 0..15 (M1 even): ipos(j + M1 k, cp) = ipos(j, cp) + k * M1 * hy
+    const size_t base = (size_t)b * NX * hy + ipos(j, cp, hy), kstr = (size_t)F::M1 * hy;
+    const cpair *src = reinterpret_cast<const cpair *>(a.src) + base;
+    cpair *dst = reinterpret_cast<cpair *>(a.dst) + base;
     float2 *sm = reinterpret_cast<float2 *>(smem_raw) + c;
     cpair v[16];
     pdl_launch_dependents();
@@ -275,11 +277,11 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
     for (int k = 0; k < 16; ++k) {
         if ((GPE_ABL & 1) || (a.flags & 512)) { v[k].re = make_float2(1e-3f * k, 2e-3f * j); v[k].im = make_float2(1e-3f * c, -1e-3f * k); }
         else if (GPE_ABL & 8192) v[k] = ldcg_pair(reinterpret_cast<const cpair *>(a.src) + ((size_t)b * NX * hy + (size_t)blockIdx.x * 16 * G::THREADS + k * G::THREADS + threadIdx.x));
-        else v[k] = ldcg_pair(src + ipos(j + F::M1 * k, cp, hy));
+        else v[k] = ldcg_pair(src + k * kstr);
     }
     if (a.flags & 256) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) st_pair(dst + ipos(j + F::M1 * k, cp, hy), v[k]);
+        for (int k = 0; k < 16; ++k) st_pair(dst + k * kstr, v[k]);
         return;
     }
     F::fwd(v, sm, j, a.tw_x, a.tw1_x, [] { if (!(GPE_ABL & 16)) __syncthreads(); });
@@ -319,7 +321,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
         if (GPE_ABL & 8192) st_pair(reinterpret_cast<cpair *>(a.dst) + ((size_t)b * NX * hy + (size_t)blockIdx.x * 16 * G::THREADS + k * G::THREADS + threadIdx.x), v[k]);
-        else st_pair(dst + ipos(j + F::M1 * k, cp, hy), v[k]);
+        else st_pair(dst + k * kstr, v[k]);
     }
 }
 
@@ -433,7 +435,10 @@ template <int N> struct LaunchP {
     using A = StepArgs<float, float2>;
     static size_t row_smem() { return sizeof(float2) * RowGeomP<N>::RPC * Fft1D<N / 2, 1, cpair>::TILE; }
     static size_t col_smem() { return sizeof(float2) * Fft1D<N, ColGeomP<N>::CPW, cpair>::TILE; }
-    static bool use_pdl(const A &a) { return (long)a.batch * a.nx * a.ny <= 65536L; }
+    static bool use_pdl(const A &a) {
+        static const long lim = getenv("GPE_PDL_MAX_POINTS") ? atol(getenv("GPE_PDL_MAX_POINTS")) : 65536L;   // tuning knob
+        return (long)a.batch * a.nx * a.ny <= lim;
+    }
     template <typename K> static cudaError_t go(K kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, const A &a) {
         cudaError_t e = Launch<float, N>::prep(kern, smem);
         if (e != cudaSuccess) return e;
