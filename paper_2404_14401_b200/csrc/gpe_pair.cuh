@@ -23,11 +23,14 @@
 #ifndef GPE_ABL
 #define GPE_ABL 0   // ablation experiments only (timing with wrong numerics)
 #endif
+#ifndef GPE_ROWP_THREADS
+#define GPE_ROWP_THREADS 64    // measured: 64 / 128 beat 128 / 256 below 2048 (more, smaller CTAs fill the 148 SMs)
+#endif
 #ifndef GPE_ROWP_MINB
 #define GPE_ROWP_MINB 4
 #endif
 #ifndef GPE_COLP_THREADS
-#define GPE_COLP_THREADS 256
+#define GPE_COLP_THREADS 128
 #endif
 
 namespace gpe {
@@ -35,7 +38,7 @@ namespace gpe {
 template <int N> struct RowGeomP {
     static constexpr int H = N / 2;
     static constexpr int TPF = H / 16;                               // threads per row
-    static constexpr int RPC = (128 / TPF) < 1 ? 1 : (128 / TPF);    // rows per CTA
+    static constexpr int RPC = (GPE_ROWP_THREADS / TPF) < 2 ? 2 : (GPE_ROWP_THREADS / TPF);    // rows per CTA (>= one row pair)
     static constexpr int THREADS = RPC * TPF;                        // 128
     static constexpr bool NAMED = RPC > 1 && TPF % 32 == 0;          // rows own whole warps
     // outer stage pair-mapped (Fft1D::last_fwd_pair): a thread holds the same output indices of rows
@@ -189,7 +192,7 @@ __device__ __forceinline__ void reduce_pair16(const float2 (&p0)[16], const floa
 
 // ---------------------------------------------------------------- pass A (rows, forward)
 template <int NY, bool IMAG>
-__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, GPE_ROWP_MINB) k_row_fwd_p(const StepArgs<float, float2> a) {
+__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) / RowGeomP<NY>::THREADS) k_row_fwd_p(const StepArgs<float, float2> a) {
     using G = RowGeomP<NY>;
     using F = Fft1D<G::H, 1, cpair>;
     constexpr int H = G::H, M1 = F::M1;
@@ -256,7 +259,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, GPE_ROWP_MINB) k_row_fw
 
 // ---------------------------------------------------------------- pass B (columns)
 template <int NX, bool IMAG>
-__global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS <= 256 ? 2 : 1)) k_col_p(const StepArgs<float, float2> a) {
+__global__ void __launch_bounds__(ColGeomP<NX>::THREADS, 512 / ColGeomP<NX>::THREADS) k_col_p(const StepArgs<float, float2> a) {
     using G = ColGeomP<NX>;
     using F = Fft1D<NX, G::CPW, cpair>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -327,7 +330,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, (ColGeomP<NX>::THREADS 
 
 // ---------------------------------------------------------------- pass C (rows, inverse)
 template <int NY, bool IMAG, bool MERGED>
-__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, GPE_ROWP_MINB) k_row_inv_p(const StepArgs<float, float2> a) {
+__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) / RowGeomP<NY>::THREADS) k_row_inv_p(const StepArgs<float, float2> a) {
     using G = RowGeomP<NY>;
     using F = Fft1D<G::H, 1, cpair>;
     constexpr int H = G::H, M1 = F::M1;
