@@ -440,7 +440,6 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
         GPE_CUDA(p, cudaGetLastError());
     }
     // complex64 hot path: paired passes (gpe_pair.cuh) when built for both axis lengths
-    if (const char *dbg = getenv("GPE_DEBUG_FLAGS")) a.flags |= atoi(dbg);   // ablation experiments only
     const bool paired = oy->p_row_fwd && ox->p_col && !getenv("GPE_NO_PAIR");
     a.fin.cpm = p->nx / (paired ? oy->p_rows_per_cta : oy->rows_per_cta);
     a.fin.normalise = imag ? 1 : 0;

@@ -163,14 +163,7 @@ template <int R, int SIGN, typename E> __device__ __forceinline__ void dft(E *v)
     }
 }
 
-// twiddle fetch (GPE_ABL_NOTW: ablation experiment only -- no table load, wrong numerics)
-template <typename C> __device__ __forceinline__ C ldtw(const C *__restrict__ t, int i) {
-#ifdef GPE_ABL_NOTW
-    C r; r.x = 1.0f; r.y = 1e-9f * (float)i; return r;
-#else
-    return t[i];
-#endif
-}
+template <typename C> __device__ __forceinline__ C ldtw(const C *__restrict__ t, int i) { return t[i]; }
 
 template <int N> struct Fact;
 template <> struct Fact<64> { static constexpr int R2 = 4, R3 = 1; };

@@ -383,8 +383,8 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
             T sn, st;
             potential_step16<T, IMAG, false, F::M1>(v, a, b, i, j, (T)ms.scale, (T)ms.A, (T)ms.C, sn, st);
         }
-        if (!(a.flags & 256)) F::fwd(v, sm, j, a.tw_y, a.tw1_y);
-        if (!(a.flags & 512) || v[0].x == 12345.678f) {
+        F::fwd(v, sm, j, a.tw_y, a.tw1_y);
+        {
 #pragma unroll
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll

@@ -20,14 +20,14 @@
 #pragma once
 #include "gpe_kernels.cuh"
 
-#ifndef GPE_ABL
-#define GPE_ABL 0   // ablation experiments only (timing with wrong numerics)
-#endif
 #ifndef GPE_ROWP_THREADS
 #define GPE_ROWP_THREADS 64    // measured: 64 / 128 beat 128 / 256 below 2048 (more, smaller CTAs fill the 148 SMs)
 #endif
 #ifndef GPE_ROWP_MINB
 #define GPE_ROWP_MINB 4
+#endif
+#ifndef GPE_COLP_RESIDENT
+#define GPE_COLP_RESIDENT 512   // threads per SM the column pass is compiled for (128 registers each)
 #endif
 #ifndef GPE_COLP_THREADS
 #define GPE_COLP_THREADS 128
@@ -207,10 +207,9 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     float2 p0[16], p1[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        if (GPE_ABL & 32) { p0[k] = make_float2(1e-3f * k, 1e-3f * j); p1[k] = make_float2(-1e-3f * j, 2e-3f * k); }
-        else { p0[k] = __ldcg(src + j + M1 * k); p1[k] = __ldcg(src + H + j + M1 * k); }
+        p0[k] = __ldcg(src + j + M1 * k); p1[k] = __ldcg(src + H + j + M1 * k);
     }
-    if (!(GPE_ABL & 128)) {
+    {
         const MemberState &ms = a.fin.st[b];
         float2 sn, st;
         const bool pend = !IMAG && ms.pend;
@@ -235,7 +234,6 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
         auto sync_row = [r] { if constexpr (G::NAMED) bar_named(1 + r, G::TPF); else __syncthreads(); };
         auto sync_pair = [rp] { if constexpr (G::PAIRNAMED) bar_named(9 + rp, 2 * G::TPF); else __syncthreads(); };
         F::fwd_pairlast(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, sync_row, sync_pair);
-        if ((GPE_ABL & 64) && v[0].re.x != 12345.678f) return;
         const long rowp = (long)blockIdx.x * G::RPC + 2 * rp;
 #pragma unroll
         for (int ii = 0; ii < F::GL / 2; ++ii)
@@ -249,7 +247,6 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
         if (G::RPC > 1) __syncthreads();
         if constexpr (G::NAMED) F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
         else F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
-        if ((GPE_ABL & 64) && v[0].re.x != 12345.678f) return;
 #pragma unroll
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
@@ -259,7 +256,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
 
 // ---------------------------------------------------------------- pass B (columns)
 template <int NX, bool IMAG>
-__global__ void __launch_bounds__(ColGeomP<NX>::THREADS, 512 / ColGeomP<NX>::THREADS) k_col_p(const StepArgs<float, float2> a) {
+__global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / ColGeomP<NX>::THREADS) k_col_p(const StepArgs<float, float2> a) {
     using G = ColGeomP<NX>;
     using F = Fft1D<NX, G::CPW, cpair>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -278,16 +275,9 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, 512 / ColGeomP<NX>::THR
     if (blockIdx.x == 0 && threadIdx.x == 0 && a.fin.prepared) prepare_member(a.fin, b);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        if ((GPE_ABL & 1) || (a.flags & 512)) { v[k].re = make_float2(1e-3f * k, 2e-3f * j); v[k].im = make_float2(1e-3f * c, -1e-3f * k); }
-        else if (GPE_ABL & 8192) v[k] = ldcg_pair(reinterpret_cast<const cpair *>(a.src) + ((size_t)b * NX * hy + (size_t)blockIdx.x * 16 * G::THREADS + k * G::THREADS + threadIdx.x));
-        else v[k] = ldcg_pair(src + k * kstr);
+        v[k] = ldcg_pair(src + k * kstr);
     }
-    if (a.flags & 256) {
-#pragma unroll
-        for (int k = 0; k < 16; ++k) st_pair(dst + k * kstr, v[k]);
-        return;
-    }
-    F::fwd(v, sm, j, a.tw_x, a.tw1_x, [] { if (!(GPE_ABL & 16)) __syncthreads(); });
+    F::fwd(v, sm, j, a.tw_x, a.tw1_x);
     if constexpr (IMAG) {
         const float2 ey = *reinterpret_cast<const float2 *>(a.kin_yr + 2 * cp);
 #pragma unroll
@@ -310,7 +300,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, 512 / ColGeomP<NX>::THR
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
             for (int rr = 0; rr < F::RL; ++rr) {
-                const float2 ap = (GPE_ABL & 8) ? make_float2(1e-7f * ii, 1e-7f * rr) : a.kin_xc[F::nat(j, ii, rr)];
+                const float2 ap = a.kin_xc[F::nat(j, ii, rr)];
                 const float2 gx = rfmas(cb, ap.x, rfmas(bqy, -ap.y, bpx));
                 const float2 gy = rfmas(bqy, ap.x, rfmas(cb, ap.y, bpy));
                 cpair &z = v[ii * F::RL + rr];
@@ -319,12 +309,10 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, 512 / ColGeomP<NX>::THR
                 z.re = ox; z.im = oy;
             }
     }
-    F::inv(v, sm, j, a.tw_x, a.tw1_x, [] { if (!(GPE_ABL & 16)) __syncthreads(); });
-    if (((GPE_ABL & 2) || (a.flags & 1024)) && v[0].re.x != 12345.678f) return;
+    F::inv(v, sm, j, a.tw_x, a.tw1_x);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        if (GPE_ABL & 8192) st_pair(reinterpret_cast<cpair *>(a.dst) + ((size_t)b * NX * hy + (size_t)blockIdx.x * 16 * G::THREADS + k * G::THREADS + threadIdx.x), v[k]);
-        else st_pair(dst + k * kstr, v[k]);
+        st_pair(dst + k * kstr, v[k]);
     }
 }
 
@@ -355,8 +343,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
 #pragma unroll
             for (int rr = 0; rr < F::RL; ++rr) {
                 const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H);
-                if (GPE_ABL & 256) { v[(2 * ii) * F::RL + rr].re = make_float2(1e-3f * rr, 1e-3f * j); v[(2 * ii) * F::RL + rr].im = make_float2(-1e-3f * j, 2e-3f * ii); v[(2 * ii + 1) * F::RL + rr] = v[(2 * ii) * F::RL + rr]; }
-                else ldcg_pair2(src + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
+                ldcg_pair2(src + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
             }
         auto sync_row = [r] { if constexpr (G::NAMED) bar_named(1 + r, G::TPF); else __syncthreads(); };
         auto sync_pair = [rp] { if constexpr (G::PAIRNAMED) bar_named(9 + rp, 2 * G::TPF); else __syncthreads(); };
@@ -366,8 +353,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
             for (int rr = 0; rr < F::RL; ++rr) {
-                if (GPE_ABL & 256) { v[ii * F::RL + rr].re = make_float2(1e-3f * rr, 1e-3f * j); v[ii * F::RL + rr].im = make_float2(-1e-3f * j, 2e-3f * ii); }
-                else v[ii * F::RL + rr] = ldcg_pair(src + ipos(row, F::nat(j, ii, rr), H));
+                v[ii * F::RL + rr] = ldcg_pair(src + ipos(row, F::nat(j, ii, rr), H));
             }
         if constexpr (G::NAMED) F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
         else F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
@@ -384,7 +370,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     const MemberState &ms = a.fin.st[b];
     float2 sn = make_float2(0.f, 0.f), st = sn;
     if constexpr (MERGED) reduce_pair16<M1>(p0, p1, a, j, sn, st);
-    else if (!(GPE_ABL & 1024)) potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, 1.f, (float)ms.A, (float)ms.C, sn, st);
+    else potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, 1.f, (float)ms.A, (float)ms.C, sn, st);
     float2 *dst = a.dst + row * NY;
     // Reduction first, wavefunction stores second: the partial sums of this CTA are published
     // (store, fence, counter increment) while thread 0 has no stores in flight, so the fence does
@@ -400,7 +386,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     if (lane == 0) { red[wid] = dn; red[32 + wid] = dt_; }
     __syncthreads();
     unsigned int old = 0;
-    if (threadIdx.x == 0 && !(GPE_ABL & 2048)) {
+    if (threadIdx.x == 0) {
         double s0 = 0.0, s1 = 0.0;
 #pragma unroll
         for (int q = 0; q < NW; ++q) { s0 += red[q]; s1 += red[32 + q]; }
@@ -408,13 +394,11 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
         __threadfence();
         old = atomicAdd(&f.counters[b], 1u);
     }
-    if (!((GPE_ABL & 512) && p0[0].x != 12345.678f)) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) { dst[j + M1 * k] = p0[k]; dst[H + j + M1 * k] = p1[k]; }
-    }
-    if (threadIdx.x == 0) is_last = (old == (unsigned int)(f.cpm - 1)) && !(GPE_ABL & 2048);
+    for (int k = 0; k < 16; ++k) { dst[j + M1 * k] = p0[k]; dst[H + j + M1 * k] = p1[k]; }
+    if (threadIdx.x == 0) is_last = (old == (unsigned int)(f.cpm - 1));
     __syncthreads();
-    if (is_last && !(GPE_ABL & 4096)) {   // the last CTA of the member: all its threads sum the partials
+    if (is_last) {   // the last CTA of the member: all its threads sum the partials
         __threadfence();
         const volatile double2 *pp = f.partials + (size_t)b * f.cpm;
         double s0 = 0.0, s1 = 0.0;
