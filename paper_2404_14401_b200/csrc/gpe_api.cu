@@ -445,9 +445,9 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     a.fin.normalise = imag ? 1 : 0;
     a.fin.advance = 1;
     a.fin.prepared = 1;   // pass B prepares the coefficients of the next step (prepare_member)
-    // real time on the paired passes: pass C leaves its half-step to the next pass A (one multiply
+    // real time: pass C leaves its half-step to the next pass A (one multiply
     // by exp(-i (V_n + V_{n+1} + 2 g |psi|^2) dt/2) instead of two; |psi|^2, hence Theta, is unchanged)
-    a.fin.merged = (paired && !imag && !getenv("GPE_NO_MERGE")) ? 1 : 0;
+    a.fin.merged = (!imag && !getenv("GPE_NO_MERGE")) ? 1 : 0;
     a.fin.record_every = 0; a.fin.rec_first = 0; a.fin.records = nullptr;  // step kernels read *call
     auto one_step = [&](cudaStream_t st, int w, cudaEvent_t e0, cudaEvent_t e1) -> gpe_status {
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, st));

@@ -230,15 +230,17 @@ __device__ __forceinline__ void sincosm1_small(float w, float *s, float *cm1) {
 // REDUCE: also returns sum |psi_new|^2 and sum cos(k_c y) |psi_new|^2 over the 16 points.
 template <typename T, bool IMAG, bool REDUCE, int M1>
 __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<T, cx<T>> &a, int b, int i, int j,
-                                                 T scale, T A, T Cc, T &sn, T &st) {
+                                                 T scale, T fac, T A, T Cc, T &sn, T &st) {
     using V4 = typename Vec4<T>::type;
     const int flags = a.flags;
     T vrow = T(0);
-    if (flags & F_HAS_SEP) vrow += a.vx[i];
+    // fac = 1, or 2 when the multiply also carries the pending second half-step of the previous
+    // step (real time; A, Cc are then the sums of the two steps' coefficients)
+    if (flags & F_HAS_SEP) vrow += fac * a.vx[i];
     if (flags & F_LAT_X) vrow += A * a.latx[i];
     const T crow = (flags & F_CAVITY) ? Cc * a.cavx[i] : T(0);
     const T Ay = (flags & F_LAT_Y) ? A : T(0);
-    const T g = (flags & F_HAS_G) ? a.g[b] : T(0);
+    const T g = (flags & F_HAS_G) ? fac * a.g[b] : T(0);
     const T hdt = a.half_dt;
     const V4 *__restrict__ yt = reinterpret_cast<const V4 *>(a.ytab);
     T w[16];
@@ -247,13 +249,13 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
         const V4 t = yt[j + M1 * k];
         if constexpr (IMAG) { v[k].x *= scale; v[k].y *= scale; }  // the lazy scale is 1 in real time
         const T d = v[k].x * v[k].x + v[k].y * v[k].y;
-        const T V = fma(crow, t.z, fma(Ay, t.y, vrow + t.x));
+        const T V = fma(crow, t.z, fma(Ay, t.y, fma(fac, t.x, vrow)));
         w[k] = fma(g, d, V) * hdt;
     }
     if (flags & F_HAS_V2D) {
         const T *__restrict__ v2 = a.v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * a.nx * a.ny : 0) + (size_t)i * a.ny;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) w[k] = fma(v2[j + M1 * k], hdt, w[k]);
+        for (int k = 0; k < 16; ++k) w[k] = fma(v2[j + M1 * k], fac * hdt, w[k]);
     }
     if constexpr (IMAG) {
 #pragma unroll
@@ -344,8 +346,10 @@ __device__ __forceinline__ void stage_fetch(unsigned char *stage, const void *gs
 }
 
 // ---------------------------------------------------------------- pass A
+// complex128 rows: two 256-thread CTAs per SM (128 registers) from 512 points up -- measured on B200:
+// 2048^2 real time 185 -> 157 us per step, 1024^2 53 -> 45; below 512 one CTA with all registers wins.
 template <typename T, int NY, bool IMAG>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : 1)) k_row_fwd(const StepArgs<T, cx<T>> a) {
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1))) k_row_fwd(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
@@ -381,7 +385,9 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
         if (!(a.flags & F_NO_POT)) {
             const MemberState &ms = a.fin.st[b];
             T sn, st;
-            potential_step16<T, IMAG, false, F::M1>(v, a, b, i, j, (T)ms.scale, (T)ms.A, (T)ms.C, sn, st);
+            const bool pend = !IMAG && ms.pend;
+            potential_step16<T, IMAG, false, F::M1>(v, a, b, i, j, (T)ms.scale, pend ? T(2) : T(1), (T)(pend ? ms.A + ms.A_pend : ms.A),
+                                                    (T)(pend ? ms.C + ms.C_pend : ms.C), sn, st);
         }
         F::fwd(v, sm, j, a.tw_y, a.tw1_y);
         {
@@ -398,7 +404,7 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
 // MODE 0: forward, kinetic factor, inverse (the step).  MODE 1: forward only, natural order
 // (observables).
 template <typename T, int NX, bool IMAG, int MODE>
-__global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<T, cx<T>> a) {
+__global__ void __launch_bounds__(ColGeom<T, NX>::THREADS, 1) k_col(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using G = ColGeom<T, NX>;
     using F = Fft1D<NX, G::W, cx<T>>;
@@ -462,8 +468,8 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS) k_col(const StepArgs<
 }
 
 // ---------------------------------------------------------------- pass C
-template <typename T, int NY, bool IMAG>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : 1)) k_row_inv(const StepArgs<T, cx<T>> a) {
+template <typename T, int NY, bool IMAG, bool MERGED>
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1))) k_row_inv(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
@@ -505,7 +511,15 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
         F::inv(v, sm, j, a.tw_y, a.tw1_y);
         const MemberState &ms = a.fin.st[b];
         T sn, st;
-        potential_step16<T, IMAG, true, F::M1>(v, a, b, i, j, T(1), (T)ms.A, (T)ms.C, sn, st);
+        if constexpr (MERGED) {   // real time: the multiply is left to the next pass A, sums of |psi|^2 only
+            sn = T(0); st = T(0);
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const T d = v[k].x * v[k].x + v[k].y * v[k].y;
+                sn += d;
+                if (a.flags & F_CAVITY) st = fma(d, a.ytab[4 * (j + F::M1 * k) + 2], st);
+            }
+        } else potential_step16<T, IMAG, true, F::M1>(v, a, b, i, j, T(1), T(1), (T)ms.A, (T)ms.C, sn, st);
 #pragma unroll
         for (int k = 0; k < 16; ++k) dst[j + F::M1 * k] = v[k];
         double dn = (double)sn, dt_ = (a.flags & F_CAVITY) ? (double)st * (double)a.cavx[i] : 0.0;
@@ -561,15 +575,14 @@ template <typename T, int N> struct Launch {
     }
     static cudaError_t row_inv(const A &a, bool imag, cudaStream_t s) {
         dim3 grid(row_grid(a)), block(RowGeom<N>::THREADS);
-        cudaError_t e;
-        if (imag) {
-            if ((e = prep(k_row_inv<T, N, true>, row_smem())) != cudaSuccess) return e;
-            { cudaError_t le = launch_pdl(k_row_inv<T, N, true>, grid, block, row_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
-        } else {
-            if ((e = prep(k_row_inv<T, N, false>, row_smem())) != cudaSuccess) return e;
-            { cudaError_t le = launch_pdl(k_row_inv<T, N, false>, grid, block, row_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
-        }
-        return cudaGetLastError();
+        auto go = [&](auto kern) -> cudaError_t {
+            cudaError_t e = prep(kern, row_smem());
+            if (e != cudaSuccess) return e;
+            e = launch_pdl(kern, grid, block, row_smem(), s, use_pdl(a), a);
+            return e != cudaSuccess ? e : cudaGetLastError();
+        };
+        if (imag) return go(k_row_inv<T, N, true, false>);
+        return a.fin.merged ? go(k_row_inv<T, N, false, true>) : go(k_row_inv<T, N, false, false>);
     }
     // nx == N
     static cudaError_t col(const A &a, bool imag, int mode, cudaStream_t s) {

@@ -303,31 +303,33 @@ def test_step_counter_resume_equals_one_call():
     assert _rel(outs[1], outs[0].astype(np.complex128)) <= 1e-6
 
 
-def test_merged_half_steps_equal_separate_ones(monkeypatch):
-    """Real time, paired complex64 passes: the merged form (one multiply by the second half-step of
-    step n and the first of step n+1) against the same kernels with separate
-    half-steps and against the unpaired kernels: same psi to fp32 round-off, same records."""
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_merged_half_steps_equal_separate_ones(monkeypatch, dtype):
+    """Real time: the merged form (one multiply by the second half-step of step n and the first of
+    step n+1) against separate half-steps, on the paired complex64 kernels and on the
+    one-number-per-element kernels: same psi to round-off, same records."""
     torch = _torch()
     p = _general_workload(256, 128)
     outs, recs = [], []
-    for env in ({}, {"GPE_NO_MERGE": "1"}, {"GPE_NO_PAIR": "1"}):
+    for env in ({}, {"GPE_NO_MERGE": "1"}, {"GPE_NO_PAIR": "1"}, {"GPE_NO_PAIR": "1", "GPE_NO_MERGE": "1"}):
         for k in ("GPE_NO_MERGE", "GPE_NO_PAIR"):
             monkeypatch.delenv(k, raising=False)
         for k, v in env.items():
             monkeypatch.setenv(k, v)
-        plan = _gpu_plan(p, "c64")
-        psi = _to_dev(p["psi0"], "c64")
+        plan = _gpu_plan(p, dtype)
+        psi = _to_dev(p["psi0"], dtype)
         r1 = plan.evolve(psi, 1e-3, 7, "real", record_every=1)      # odd counts: no graph, epilogue twice
         r2 = plan.evolve(psi, 1e-3, 24, "real", record_every=1)     # graph replay + remainder
         torch.cuda.synchronize()
         outs.append(psi.cpu().numpy())
         recs.append(np.concatenate([r1.cpu().numpy()[:7], r2.cpu().numpy()[:24]]))
         plan.close()
+    tol = 2e-6 if dtype == "c64" else 1e-13
     for o in outs[1:]:
-        assert _rel(o, outs[0].astype(np.complex128)) <= 2e-6
+        assert _rel(o, outs[0].astype(np.complex128)) <= tol
     for r in recs[1:]:
         assert np.allclose(r[:, 0, :2], recs[0][:, 0, :2], rtol=1e-6, atol=0)          # step, norm
-        assert np.allclose(r[:, 0, 2:], recs[0][:, 0, 2:], rtol=1e-4, atol=1e-7)       # Theta, alpha, A
+        assert np.allclose(r[:, 0, 2:], recs[0][:, 0, 2:], rtol=1e-4 if dtype == "c64" else 1e-10, atol=1e-7)
 
 
 def test_error_behaviour():
