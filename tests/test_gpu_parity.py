@@ -332,6 +332,26 @@ def test_merged_half_steps_equal_separate_ones(monkeypatch, dtype):
         assert np.allclose(r[:, 0, 2:], recs[0][:, 0, 2:], rtol=1e-4 if dtype == "c64" else 1e-10, atol=1e-7)
 
 
+@pytest.mark.parametrize("mode", ["real", "imag"])
+@pytest.mark.parametrize("nx,ny,batch", [(2048, 2048, 1), (1024, 128, 1), (128, 2048, 1), (256, 512, 3), (64, 64, 2)])
+def test_runs_are_bitwise_reproducible(nx, ny, batch, mode):
+    """A race between the CTAs of a pass (in-place intermediate layout, named barriers, last-block
+    reduction) would show up as run-to-run differences: two runs must agree bit for bit, and so
+    must their records (fixed summation order)."""
+    torch = _torch()
+    p = _general_workload(nx, ny, batch=batch, mode=mode)
+    outs = []
+    for _ in range(2):
+        plan = _gpu_plan(p, "c64")
+        psi = _to_dev(p["psi0"], "c64")
+        rec = plan.evolve(psi, 1e-3 if mode == "real" else 5e-4, 5, mode, record_every=1)
+        torch.cuda.synchronize()
+        outs.append((psi.cpu().numpy().copy(), rec.cpu().numpy().copy()))
+        plan.close()
+    assert np.array_equal(outs[0][0].view(np.uint32), outs[1][0].view(np.uint32))
+    assert np.array_equal(outs[0][1].view(np.uint64), outs[1][1].view(np.uint64))
+
+
 def test_error_behaviour():
     import paper_2404_14401_b200 as G
     torch = _torch()
