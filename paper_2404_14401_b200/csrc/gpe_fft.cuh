@@ -163,6 +163,7 @@ template <int R, int SIGN, typename E> __device__ __forceinline__ void dft(E *v)
     }
 }
 
+// table fetch (plain cached load; the read-only path, __ldg, measured no faster on B200)
 template <typename C> __device__ __forceinline__ C ldtw(const C *__restrict__ t, int i) { return t[i]; }
 
 template <int N> struct Fact;

@@ -106,8 +106,8 @@ __device__ __forceinline__ void potential_pair16(float2 (&p0)[16], float2 (&p1)[
     #pragma unroll
         for (int k = k0; k < k0 + CH; ++k) {
             const int n = j + M1 * k;
-            const float4 t0 = yt[2 * n];
-            const float2 cav = *reinterpret_cast<const float2 *>(yt + 2 * n + 1);
+            const float4 t0 = ldtw(yt, 2 * n);
+            const float2 cav = ldtw(reinterpret_cast<const float2 *>(yt), 4 * n + 2);
             if constexpr (IMAG) { p0[k].x *= scale; p0[k].y *= scale; p1[k].x *= scale; p1[k].y *= scale; }
             const float2 d = make_float2(fmaf(p0[k].x, p0[k].x, p0[k].y * p0[k].y), fmaf(p1[k].x, p1[k].x, p1[k].y * p1[k].y));
             const float2 V = rfmas(cav, crow, rfmas(make_float2(t0.z, t0.w), Ay, rfmas(make_float2(t0.x, t0.y), fac, make_float2(vrow, vrow))));
@@ -221,7 +221,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     cpair v[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        const float2 w = a.tw_y[j + M1 * k];
+        const float2 w = ldtw(a.tw_y, j + M1 * k);
         const float dx = p0[k].x - p1[k].x, dy = p0[k].y - p1[k].y;
         v[k].re = make_float2(p0[k].x + p1[k].x, fmaf(dx, w.x, -(dy * w.y)));
         v[k].im = make_float2(p0[k].y + p1[k].y, fmaf(dx, w.y, dy * w.x));
@@ -300,7 +300,7 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / Col
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
             for (int rr = 0; rr < F::RL; ++rr) {
-                const float2 ap = a.kin_xc[F::nat(j, ii, rr)];
+                const float2 ap = ldtw(a.kin_xc, F::nat(j, ii, rr));
                 const float2 gx = rfmas(cb, ap.x, rfmas(bqy, -ap.y, bpx));
                 const float2 gy = rfmas(bqy, ap.x, rfmas(cb, ap.y, bpy));
                 cpair &z = v[ii * F::RL + rr];
@@ -362,7 +362,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     float2 p0[16], p1[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        const float2 w = a.tw_y[j + M1 * k];
+        const float2 w = ldtw(a.tw_y, j + M1 * k);
         const float tx = fmaf(v[k].re.y, w.x, v[k].im.y * w.y), ty = fmaf(v[k].im.y, w.x, -(v[k].re.y * w.y));
         p0[k] = make_float2(v[k].re.x + tx, v[k].im.x + ty);
         p1[k] = make_float2(v[k].re.x - tx, v[k].im.x - ty);
