@@ -23,6 +23,9 @@
  *   1. A_n = schedule(n).  Theta_n = sum cos(kc x)cos(kc y)|psi|^2 dx dy.
  *      eta_n = eta (mode 0) or sqrt(|A_n| u) (mode 1).
  *      alpha_n = N_at eta_n Theta_n / (Delta + i kappa)          [PAPER.md:183, Eq. 14]
+ *      real time with a probe: alpha_n += Omega_c exp(i (Delta_p t_n + phi)) / (Delta + i kappa),
+ *      t_n = n dt (Eq. 17; the dispersive shift of its denominator is not on
+ *      this path, reading Q6)
  *      C_n = 2 eta_n Re(alpha_n)                                 [PAPER.md:179, Eq. 13]
  *   2. V_n = V_static + A_n cos^2(k_l * (x or y)) + C_n cos(kc x)cos(kc y)   [Eqs. 9-13]
  *   3. psi <- psi * exp(-sigma (V_n + g|psi|^2) dt/2)            [PAPER.md:67,71]
@@ -72,6 +75,10 @@ typedef struct {
     const double *n_atoms;    /* [batch] */
     const double *delta;      /* [batch] */
     const double *kappa;      /* [batch] */
+    /* on-axis cavity probe (Eq. 17), real time only; NULL = none */
+    const double *probe_omega; /* [batch] Omega_c */
+    const double *probe_delta; /* [batch] Delta_p */
+    const double *probe_phi;   /* [batch] phi */
 } oracle_params;
 
 /* ------------------------------------------------------------------ FFT */
@@ -243,13 +250,16 @@ static double sum_theta(const oracle_params *P, const axis_tables *T, const cplx
 }
 
 /* step 1 of the header: per-step scalars of member b at step index n from the current psi */
-static void cavity_scalars(const oracle_params *P, int b, double A, double theta,
+/* t < 0: no probe (imaginary time, observables) */
+static void cavity_scalars(const oracle_params *P, int b, double A, double theta, double t,
                            double *eta, double _Complex *alpha, double *C)
 {
     *eta = 0.0; *alpha = 0.0; *C = 0.0;
     if (!P->cavity_on) return;
     *eta = P->eta_mode == 0 ? P->eta_or_u[b] : sqrt(fabs(A) * P->eta_or_u[b]);
     *alpha = P->n_atoms[b] * (*eta) * theta / (P->delta[b] + I * P->kappa[b]);
+    if (t >= 0.0 && P->probe_omega && P->probe_omega[b] != 0.0)
+        *alpha += P->probe_omega[b] * cexp(I * (P->probe_delta[b] * t + P->probe_phi[b])) / (P->delta[b] + I * P->kappa[b]);
     *C = 2.0 * (*eta) * creal(*alpha);
 }
 
@@ -305,7 +315,7 @@ int oracle_evolve(const oracle_params *P, cplx_t *psi, double dt, long n_steps, 
             double A = oracle_schedule(P, b, (double)n);
             double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
             double eta, C; double _Complex alpha;
-            cavity_scalars(P, b, A, theta, &eta, &alpha, &C);
+            cavity_scalars(P, b, A, theta, imag_time ? -1.0 : (double)n * dt, &eta, &alpha, &C);
             potential_half_step(P, &T, b, w, A, C, dt, imag_time);
             kinetic_step(P, w, dt, imag_time);
             potential_half_step(P, &T, b, w, A, C, dt, imag_time);
@@ -321,7 +331,7 @@ int oracle_evolve(const oracle_params *P, cplx_t *psi, double dt, long n_steps, 
                 double A = oracle_schedule(P, b, (double)(n + 1));
                 double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
                 double eta, C; double _Complex alpha;
-                cavity_scalars(P, b, A, theta, &eta, &alpha, &C);
+                cavity_scalars(P, b, A, theta, imag_time ? -1.0 : (double)(n + 1) * dt, &eta, &alpha, &C);
                 double *r = records + ((size_t)nrec * P->batch + b) * ORACLE_NREC;
                 r[0] = (double)(n + 1); r[1] = sum_norm(P, w); r[2] = theta;
                 r[3] = creal(alpha); r[4] = cimag(alpha); r[5] = A;
@@ -350,7 +360,7 @@ int oracle_observables(const oracle_params *P, const cplx_t *psi, long n, double
         double norm = sum_norm(P, w);
         double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
         double eta, C; double _Complex alpha;
-        cavity_scalars(P, b, A, theta, &eta, &alpha, &C);
+        cavity_scalars(P, b, A, theta, -1.0, &eta, &alpha, &C);
         double epot = 0.0, eint = 0.0;
         for (int i = 0; i < P->nx; ++i)
             for (int j = 0; j < P->ny; ++j) {
@@ -434,7 +444,7 @@ int oracle_potential_half_step(const oracle_params *P, cplx_t *psi, double dt, i
         double A = oracle_schedule(P, b, (double)n);
         double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
         double eta, C; double _Complex alpha;
-        cavity_scalars(P, b, A, theta, &eta, &alpha, &C);
+        cavity_scalars(P, b, A, theta, -1.0, &eta, &alpha, &C);
         potential_half_step(P, &T, b, w, A, C, dt, imag_time);
     }
     free_tables(&T);

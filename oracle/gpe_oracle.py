@@ -56,6 +56,7 @@ class _Params(C.Structure):
         ("cavity_on", C.c_int), ("cavity_k", C.c_double), ("eta_mode", C.c_int),
         ("eta_or_u", C.c_void_p), ("n_atoms", C.c_void_p), ("delta", C.c_void_p),
         ("kappa", C.c_void_p),
+        ("probe_omega", C.c_void_p), ("probe_delta", C.c_void_p), ("probe_phi", C.c_void_p),
     ]
 
 
@@ -102,7 +103,8 @@ class Oracle:
     `p` is a workload dict as produced by workloads.py (keys mirror gpe_potential_desc):
       nx, ny, Lx, Ly, batch, g[batch], v_static (None | [nx,ny] | [batch,nx,ny]),
       lattice_axis, lattice_k, sched_step[len], sched_amp ([len] | [batch,len]),
-      cavity_on, cavity_k, eta_mode, eta_or_u[batch], n_atoms[batch], delta[batch], kappa[batch]
+      cavity_on, cavity_k, eta_mode, eta_or_u[batch], n_atoms[batch], delta[batch], kappa[batch],
+      probe_omega[batch], probe_delta[batch], probe_phi[batch] (optional: on-axis probe, real time)
     precision: "f64" (the oracle) or "f32" (fp32-floor probe of the same statements).
     """
 
@@ -158,6 +160,10 @@ class Oracle:
         for name, default in (("eta_or_u", 0.0), ("n_atoms", 1.0), ("delta", -1.0), ("kappa", 1.0)):
             a = _f64(np.broadcast_to(np.asarray(p.get(name, default), dtype=np.float64), (B,)), B)
             setattr(P, name, ptr(a))
+        if p.get("probe_omega") is not None:   # on-axis probe, PAPER.md:216-221 (Eq. 17)
+            for name, default in (("probe_omega", 0.0), ("probe_delta", 0.0), ("probe_phi", 0.0)):
+                a = _f64(np.broadcast_to(np.asarray(p.get(name, default), dtype=np.float64), (B,)), B)
+                setattr(P, name, ptr(a))
         self.P = P
         self.step = 0
 

@@ -403,6 +403,55 @@ def test_cavity_self_organisation_and_fixed_point():
     assert ob["re_alpha"] == pytest.approx(alpha.real, rel=1e-12)
 
 
+def test_probe_closed_form_and_imprint():
+    """On-axis probe (Eq. 17), real time.
+    (a) With N_at = 0 the atoms do not feed the field, so the recorded cavity field is the probe
+        alone: alpha'(t_n) = Omega exp(i(Delta_p n dt + phi)) / (Delta + i kappa), whatever psi does
+        -- pins amplitude, phase, sign of the frequency and the sampling time t_n = n dt.
+    (b) The probe enters the potential as 2 eta Re(alpha') cos(kx)cos(ky) (Eq. 18): one short step
+        from a uniform state imprints the phase -dt 2 eta Re(dalpha(0)) cos cos to first order.
+    (c) Omega = 0 is the run without a probe (to the round-off of the OpenMP reduction order);
+        imaginary time ignores the probe."""
+    p = _cavity_small(6.0, g=0.0, n=64, delta=-1.3)
+    p["kappa"] = np.array([0.7])
+    Om, Dp, ph, dt = 0.8, 37.0, 0.4, 2e-3
+    p["probe_omega"], p["probe_delta"], p["probe_phi"] = np.array([Om]), np.array([Dp]), np.array([ph])
+    # (a)
+    pa = dict(p); pa["n_atoms"] = np.array([0.0])
+    psi = pa["psi0"].copy()
+    rec = Oracle(pa).evolve(psi, dt, 12, False, record_every=1)
+    n = np.arange(1, 13)
+    want = Om * np.exp(1j * (Dp * n * dt + ph)) / (-1.3 + 0.7j)
+    assert np.allclose(rec[:, 0, 3] + 1j * rec[:, 0, 4], want, rtol=1e-13, atol=1e-15)
+    # (b) uniform state, no trap, no pump lattice but eta given directly (mode 0), N_at = 0
+    L = 4 * math.pi
+    pb = W._base(64, 64, L)
+    pb["cavity_on"], pb["cavity_k"], pb["eta_mode"] = 1, 4.0, 0
+    pb["eta_or_u"], pb["n_atoms"], pb["delta"], pb["kappa"] = np.array([1.5]), np.array([0.0]), np.array([-1.3]), np.array([0.7])
+    pb["probe_omega"], pb["probe_delta"], pb["probe_phi"] = np.array([Om]), np.array([Dp]), np.array([ph])
+    psi = np.full((64, 64), 1.0 / L, dtype=np.complex128)
+    tiny = 1e-6
+    Oracle(pb).evolve(psi, tiny, 1, False)
+    x = W.axis(64, L)
+    cc = np.cos(4.0 * x)[:, None] * np.cos(4.0 * x)[None, :]
+    d0 = (Om * np.exp(1j * ph) / (-1.3 + 0.7j)).real
+    phase = np.angle(psi * L)
+    assert np.allclose(phase, -tiny * 2.0 * 1.5 * d0 * cc, rtol=1e-4, atol=1e-12)
+    # (c)
+    p0 = dict(p); p0["probe_omega"] = np.array([0.0])
+    pn = {k: v for k, v in p.items() if not k.startswith("probe_")}
+    a, b = p["psi0"].copy(), p["psi0"].copy()
+    Oracle(p0).evolve(a, dt, 5, False); Oracle(pn).evolve(b, dt, 5, False)
+    assert np.linalg.norm(a - b) <= 1e-14 * np.linalg.norm(b)
+    a, b = p["psi0"].copy(), p["psi0"].copy()
+    Oracle(p).evolve(a, dt, 5, True); Oracle(pn).evolve(b, dt, 5, True)
+    assert np.linalg.norm(a - b) <= 1e-14 * np.linalg.norm(b)
+    # and the probe does act in real time
+    a = p["psi0"].copy(); Oracle(p).evolve(a, dt, 5, False)
+    b = p["psi0"].copy(); Oracle(pn).evolve(b, dt, 5, False)
+    assert np.linalg.norm(a - b) > 1e-6
+
+
 def test_interactions_raise_threshold():
     """repulsive interactions increase the critical pump."""
     thetas = {}
