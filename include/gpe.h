@@ -104,6 +104,14 @@ typedef struct {
     const double *n_atoms;    /* HOST [batch] N_at of Eq. 14; NULL = 1                           */
     const double *delta;      /* HOST [batch] cavity detuning Delta (required if cavity_on)      */
     const double *kappa;      /* HOST [batch] cavity decay kappa  (required if cavity_on)        */
+    /* On-axis cavity probe (Eq. 17), real time only (ignored in imaginary time):
+     * alpha'_n = alpha_n + Omega_c exp(i (Delta_p t_n + phi)) / (Delta + i kappa), t_n = n dt, n the
+     * plan's step counter; alpha' replaces alpha in C_n = 2 eta_n Re(alpha'_n) (Eq. 18) and in the
+     * records.  gpe_observables reports the self-consistent alpha_n without the probe.  All three
+     * NULL = no probe; otherwise probe_omega is required, the other two default to 0.  Needs cavity_on. */
+    const double *probe_omega; /* HOST [batch] Omega_c                                            */
+    const double *probe_delta; /* HOST [batch] Delta_p                                            */
+    const double *probe_phi;   /* HOST [batch] phi                                                */
 } gpe_potential_desc;
 
 /*

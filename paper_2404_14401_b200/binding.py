@@ -32,6 +32,7 @@ class gpe_potential_desc(C.Structure):
         ("cavity_on", C.c_int), ("cavity_k", C.c_double), ("eta_mode", C.c_int),
         ("eta_or_u", C.c_void_p), ("n_atoms", C.c_void_p), ("delta", C.c_void_p),
         ("kappa", C.c_void_p),
+        ("probe_omega", C.c_void_p), ("probe_delta", C.c_void_p), ("probe_phi", C.c_void_p),
     ]
 
 
@@ -234,6 +235,10 @@ class Plan:
         for name, default in (("eta_or_u", 0.0), ("n_atoms", 1.0), ("delta", -1.0), ("kappa", 1.0)):
             a = np.broadcast_to(np.asarray(p.get(name, default), dtype=np.float64), (B,))
             setattr(d, name, hp(a, B))
+        if p.get("probe_omega") is not None:
+            for name in ("probe_omega", "probe_delta", "probe_phi"):
+                a = np.broadcast_to(np.asarray(p.get(name, 0.0), dtype=np.float64), (B,))
+                setattr(d, name, hp(a, B))
         gpe_set_potential(self.plan, d)
         torch.cuda.current_stream().synchronize()
         self._keep = keep

@@ -58,6 +58,7 @@ struct gpe_plan {
     int *nonfinite = nullptr;
     double *d_sched_step = nullptr, *d_sched_amp = nullptr;
     double *d_eta = nullptr, *d_natoms = nullptr, *d_delta = nullptr, *d_kappa = nullptr;
+    double *d_probe_omega = nullptr, *d_probe_delta = nullptr, *d_probe_phi = nullptr;   // nullptr = no probe
 
     // host copies of the descriptor
     int lattice_axis = -1, sched_len = 0, sched_batched = 0, cavity_on = 0, eta_mode = 0;
@@ -404,6 +405,8 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     f.sched_batched = p->sched_batched;
     f.cavity_on = p->cavity_on; f.eta_mode = p->eta_mode;
     f.eta_or_u = p->d_eta; f.n_atoms = p->d_natoms; f.delta = p->d_delta; f.kappa = p->d_kappa;
+    f.probe_omega = p->d_probe_omega; f.probe_delta = p->d_probe_delta; f.probe_phi = p->d_probe_phi;
+    f.probe_dt = 0.0;   // set by a real-time gpe_evolve
     f.dxdy = (p->Lx / p->nx) * (p->Ly / p->ny);
     f.batch = p->batch;
     f.call = p->d_call;
@@ -426,6 +429,7 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     const Ops<T> *oy = get_ops<T>(p->ny), *ox = get_ops<T>(p->nx);
     StepArgs<T, cx<T>> a = base_args<T>(p, psi, psi);
     a.half_dt = (T)(0.5 * dt);
+    a.fin.probe_dt = imag ? 0.0 : dt;
     // prologue: Theta_0, A_0, C_0 from the wavefunction as given (row a0)
     {
         FinalizeParams f = a.fin;
@@ -750,7 +754,8 @@ gpe_status gpe_plan_destroy(gpe_plan *p) {
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
                     p->ytab, p->g, p->v2d, p->st, p->partials, p->counters, p->nonfinite, p->d_sched_step,
-                    p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->scratch, p->obs_dev,
+                    p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->d_probe_omega, p->d_probe_delta,
+                    p->d_probe_phi, p->scratch, p->obs_dev,
                     p->pop_dev, p->obsA_dev};
     for (void *b : bufs)
         if (b) cudaFree(b);
@@ -770,6 +775,8 @@ gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
         if (i > 0 && d->sched_step[i] < d->sched_step[i - 1])
             return fail(p, GPE_EINVAL, "sched_step must be non-decreasing");
     }
+    if ((d->probe_omega || d->probe_delta || d->probe_phi) && (!d->cavity_on || !d->probe_omega))
+        return fail(p, GPE_EINVAL, "the probe needs cavity_on and probe_omega");
     if (d->cavity_on && (!d->eta_or_u || !d->delta || !d->kappa))
         return fail(p, GPE_EINVAL, "cavity_on needs eta_or_u, delta and kappa");
     if (d->cavity_on && d->eta_mode != 0 && d->eta_mode != 1) return fail(p, GPE_EINVAL, "eta_mode must be 0 or 1");
@@ -801,6 +808,18 @@ gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
     if ((s = upload_f64(p, &p->d_natoms, p->h_natoms)) != GPE_OK) return s;
     if ((s = upload_f64(p, &p->d_delta, p->h_delta)) != GPE_OK) return s;
     if ((s = upload_f64(p, &p->d_kappa, p->h_kappa)) != GPE_OK) return s;
+    {   // on-axis probe (upload_f64 frees and leaves nullptr for an empty vector = no probe)
+        std::vector<double> om, de, ph;
+        if (d->probe_omega) {
+            om.assign(d->probe_omega, d->probe_omega + B);
+            de.assign(B, 0.0); ph.assign(B, 0.0);
+            if (d->probe_delta) de.assign(d->probe_delta, d->probe_delta + B);
+            if (d->probe_phi) ph.assign(d->probe_phi, d->probe_phi + B);
+        }
+        if ((s = upload_f64(p, &p->d_probe_omega, om)) != GPE_OK) return s;
+        if ((s = upload_f64(p, &p->d_probe_delta, de)) != GPE_OK) return s;
+        if ((s = upload_f64(p, &p->d_probe_phi, ph)) != GPE_OK) return s;
+    }
     s = p->dtype == GPE_C64 ? set_potential_impl<float>(p, d) : set_potential_impl<double>(p, d);
     if (s != GPE_OK) return s;
     p->pot_set = true;

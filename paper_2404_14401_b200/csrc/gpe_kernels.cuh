@@ -68,21 +68,32 @@ __device__ inline double schedule_at(const FinalizeParams &f, int b, double n) {
 // The part of row a0 that does not depend on the sums: A_n and the cavity constants of step n,
 // alpha_n = N eta_n Theta_n / (Delta + i kappa) = (kre + i kim) Theta_n, C_n = 2 eta_n Re alpha_n = kc Theta_n
 // (Eqs. 13-14).
-__device__ inline void step_coefficients(const FinalizeParams &f, int b, long long n, double &A, double &kre, double &kim, double &kc) {
+// Probe (Eq. 17, real time): alpha_n += pre + i pim = Omega exp(i (Delta_p n dt + phi)) / (Delta + i kappa),
+// C_n += pc = 2 eta_n pre.
+__device__ inline void step_coefficients(const FinalizeParams &f, int b, long long n, double &A, double &kre, double &kim, double &kc,
+                                         double &pre, double &pim, double &pc) {
     A = schedule_at(f, b, (double)n);
-    kre = kim = kc = 0.0;
+    kre = kim = kc = pre = pim = pc = 0.0;
     if (f.cavity_on) {
         const double eta = f.eta_mode == 0 ? f.eta_or_u[b] : sqrt(fabs(A) * f.eta_or_u[b]);
         const double D = f.delta[b], K = f.kappa[b], den = D * D + K * K, ne = f.n_atoms[b] * eta;
         kre = ne * D / den;                       // 1 / (D + iK) = (D - iK) / (D^2 + K^2)
         kim = -ne * K / den;
         kc = 2.0 * eta * kre;
+        if (f.probe_omega && f.probe_dt != 0.0 && f.probe_omega[b] != 0.0) {
+            double sn, cs;
+            sincos(f.probe_delta[b] * ((double)n * f.probe_dt) + f.probe_phi[b], &sn, &cs);
+            const double Om = f.probe_omega[b];
+            pre = Om * (cs * D + sn * K) / den;   // (cs + i sn)(D - iK) / (D^2 + K^2)
+            pim = Om * (sn * D - cs * K) / den;
+            pc = 2.0 * eta * pre;
+        }
     }
 }
 // Called by one thread of pass B per member while step n runs: coefficients of step n + 1.
 __device__ inline void prepare_member(const FinalizeParams &f, int b) {
     MemberState &s = f.st[b];
-    step_coefficients(f, b, s.step + 1, s.nA, s.nKre, s.nKim, s.nKc);
+    step_coefficients(f, b, s.step + 1, s.nA, s.nKre, s.nKim, s.nKc, s.nPre, s.nPim, s.nPc);
 }
 
 // Called by one thread of the last block of member b with the raw sums over the stored psi.
@@ -100,11 +111,11 @@ __device__ inline void finalize_member(const FinalizeParams &f, int b, double su
     }
     double A, re_a = 0.0, im_a = 0.0, C = 0.0;
     if (f.advance && f.prepared) {
-        A = s.nA; re_a = s.nKre * theta; im_a = s.nKim * theta; C = s.nKc * theta;
+        A = s.nA; re_a = s.nKre * theta + s.nPre; im_a = s.nKim * theta + s.nPim; C = s.nKc * theta + s.nPc;
     } else {
-        double kre, kim, kc;
-        step_coefficients(f, b, n1, A, kre, kim, kc);
-        re_a = kre * theta; im_a = kim * theta; C = kc * theta;
+        double kre, kim, kc, pre, pim, pc;
+        step_coefficients(f, b, n1, A, kre, kim, kc, pre, pim, pc);
+        re_a = kre * theta + pre; im_a = kim * theta + pim; C = kc * theta + pc;
     }
     if (f.advance && f.merged) { s.A_pend = s.A; s.C_pend = s.C; s.pend = 1; } else s.pend = 0;
     s.scale = scale; s.A = A; s.C = C; s.norm = norm; s.theta = theta;

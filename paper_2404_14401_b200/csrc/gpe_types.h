@@ -22,6 +22,7 @@ struct MemberState {
     // pass B while the step runs (prepare_member), so the last block of pass C has little left to do:
     // A_{n+1}; Re alpha = nKre Theta, Im alpha = nKim Theta, C = nKc Theta
     double nA, nKre, nKim, nKc;
+    double nPre, nPim, nPc;   // probe: alpha += nPre + i nPim, C += nPc (zero without a probe)
 };
 
 // Per-gpe_evolve-call parameters kept in device memory (written by the prologue kernel), so that
@@ -44,6 +45,8 @@ struct FinalizeParams {
     int sched_batched;
     int cavity_on, eta_mode;
     const double *eta_or_u, *n_atoms, *delta, *kappa;  // [batch]
+    const double *probe_omega, *probe_delta, *probe_phi;  // [batch] or nullptr (Eq. 17)
+    double probe_dt;          // dt of the running real-time evolution; 0 = no probe (imaginary time)
     double dxdy;
     long long record_every, rec_first;  // prologue only (advance == 0): copied into *call
     double *records;          // prologue only
