@@ -26,6 +26,9 @@
  *      real time with a probe: alpha_n += Omega_c exp(i (Delta_p t_n + phi)) / (Delta + i kappa),
  *      t_n = n dt (Eq. 17; the dispersive shift of its denominator is not on
  *      this path, reading Q6)
+ *      with cav_u0 = U_0 (full cavity model): Delta above is replaced by
+ *      Delta~_n = Delta - N_at U_0 B_n, B_n = sum cos^2(kc x)|psi|^2 dx dy   [PAPER.md:188, Eq. 15]
+ *      and V_n gains the cavity lattice D_n cos^2(kc x), D_n = U_0 |alpha_n|^2 [PAPER.md:177, Eq. 12]
  *      C_n = 2 eta_n Re(alpha_n)                                 [PAPER.md:179, Eq. 13]
  *   2. V_n = V_static + A_n cos^2(k_l * (x or y)) + C_n cos(kc x)cos(kc y)   [Eqs. 9-13]
  *   3. psi <- psi * exp(-sigma (V_n + g|psi|^2) dt/2)            [PAPER.md:67,71]
@@ -79,6 +82,8 @@ typedef struct {
     const double *probe_omega; /* [batch] Omega_c */
     const double *probe_delta; /* [batch] Delta_p */
     const double *probe_phi;   /* [batch] phi */
+    /* full cavity model (Eqs. 12 and 15): U_0 per member; NULL = off */
+    const double *cav_u0;      /* [batch] */
 } oracle_params;
 
 /* ------------------------------------------------------------------ FFT */
@@ -249,23 +254,39 @@ static double sum_theta(const oracle_params *P, const axis_tables *T, const cplx
     return s * (P->Lx / P->nx) * (P->Ly / P->ny);
 }
 
+static double sum_bunch(const oracle_params *P, const axis_tables *T, const cplx_t *psi)
+{
+    double s = 0.0;
+#pragma omp parallel for reduction(+ : s) schedule(static)
+    for (int i = 0; i < P->nx; ++i)
+        for (int j = 0; j < P->ny; ++j) {
+            cplx_t z = psi[(size_t)i * P->ny + j];
+            double re = creal(z), im = cimag(z);
+            s += T->cav_x[i] * T->cav_x[i] * (re * re + im * im);
+        }
+    return s * (P->Lx / P->nx) * (P->Ly / P->ny);
+}
+
 /* step 1 of the header: per-step scalars of member b at step index n from the current psi */
 /* t < 0: no probe (imaginary time, observables) */
-static void cavity_scalars(const oracle_params *P, int b, double A, double theta, double t,
-                           double *eta, double _Complex *alpha, double *C)
+static void cavity_scalars(const oracle_params *P, int b, double A, double theta, double bunch, double t,
+                           double *eta, double _Complex *alpha, double *C, double *Dc)
 {
-    *eta = 0.0; *alpha = 0.0; *C = 0.0;
+    *eta = 0.0; *alpha = 0.0; *C = 0.0; *Dc = 0.0;
     if (!P->cavity_on) return;
     *eta = P->eta_mode == 0 ? P->eta_or_u[b] : sqrt(fabs(A) * P->eta_or_u[b]);
-    *alpha = P->n_atoms[b] * (*eta) * theta / (P->delta[b] + I * P->kappa[b]);
+    double D = P->delta[b];
+    if (P->cav_u0) D -= P->n_atoms[b] * P->cav_u0[b] * bunch;          /* Eq. 15 */
+    *alpha = P->n_atoms[b] * (*eta) * theta / (D + I * P->kappa[b]);
     if (t >= 0.0 && P->probe_omega && P->probe_omega[b] != 0.0)
-        *alpha += P->probe_omega[b] * cexp(I * (P->probe_delta[b] * t + P->probe_phi[b])) / (P->delta[b] + I * P->kappa[b]);
+        *alpha += P->probe_omega[b] * cexp(I * (P->probe_delta[b] * t + P->probe_phi[b])) / (D + I * P->kappa[b]);
+    if (P->cav_u0) *Dc = P->cav_u0[b] * (creal(*alpha) * creal(*alpha) + cimag(*alpha) * cimag(*alpha));  /* Eq. 12 */
     *C = 2.0 * (*eta) * creal(*alpha);
 }
 
 /* steps 3 / 5 of the header */
 static void potential_half_step(const oracle_params *P, const axis_tables *T, int b, cplx_t *psi, double A, double C,
-                                double dt, int imag_time)
+                                double Dc, double dt, int imag_time)
 {
     double g = P->g ? P->g[b] : 0.0;
 #pragma omp parallel for schedule(static)
@@ -274,7 +295,7 @@ static void potential_half_step(const oracle_params *P, const axis_tables *T, in
             size_t q = (size_t)i * P->ny + j;
             double re = creal(psi[q]), im = cimag(psi[q]);
             double V = v_static_at(P, b, q) + A * LATTICE_SHAPE(T, i, j);
-            if (P->cavity_on) V += C * CAVITY_MODE(T, i, j);
+            if (P->cavity_on) V += C * CAVITY_MODE(T, i, j) + Dc * T->cav_x[i] * T->cav_x[i];
             double W = (V + g * (re * re + im * im)) * dt * 0.5;
             cplx_t f = imag_time ? (cplx_t)exp(-W) : (cplx_t)cexp(-I * W);
             psi[q] = psi[q] * f;
@@ -314,11 +335,12 @@ int oracle_evolve(const oracle_params *P, cplx_t *psi, double dt, long n_steps, 
             cplx_t *w = psi + (size_t)b * npts;
             double A = oracle_schedule(P, b, (double)n);
             double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
-            double eta, C; double _Complex alpha;
-            cavity_scalars(P, b, A, theta, imag_time ? -1.0 : (double)n * dt, &eta, &alpha, &C);
-            potential_half_step(P, &T, b, w, A, C, dt, imag_time);
+            double bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
+            double eta, C, Dc; double _Complex alpha;
+            cavity_scalars(P, b, A, theta, bunch, imag_time ? -1.0 : (double)n * dt, &eta, &alpha, &C, &Dc);
+            potential_half_step(P, &T, b, w, A, C, Dc, dt, imag_time);
             kinetic_step(P, w, dt, imag_time);
-            potential_half_step(P, &T, b, w, A, C, dt, imag_time);
+            potential_half_step(P, &T, b, w, A, C, Dc, dt, imag_time);
             if (imag_time) {
                 real_t inv = (real_t)(1.0 / sqrt(sum_norm(P, w)));
 #pragma omp parallel for schedule(static)
@@ -330,8 +352,9 @@ int oracle_evolve(const oracle_params *P, cplx_t *psi, double dt, long n_steps, 
                 cplx_t *w = psi + (size_t)b * npts;
                 double A = oracle_schedule(P, b, (double)(n + 1));
                 double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
-                double eta, C; double _Complex alpha;
-                cavity_scalars(P, b, A, theta, imag_time ? -1.0 : (double)(n + 1) * dt, &eta, &alpha, &C);
+                double bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
+                double eta, C, Dc; double _Complex alpha;
+                cavity_scalars(P, b, A, theta, bunch, imag_time ? -1.0 : (double)(n + 1) * dt, &eta, &alpha, &C, &Dc);
                 double *r = records + ((size_t)nrec * P->batch + b) * ORACLE_NREC;
                 r[0] = (double)(n + 1); r[1] = sum_norm(P, w); r[2] = theta;
                 r[3] = creal(alpha); r[4] = cimag(alpha); r[5] = A;
@@ -359,8 +382,9 @@ int oracle_observables(const oracle_params *P, const cplx_t *psi, long n, double
         double g = P->g ? P->g[b] : 0.0;
         double norm = sum_norm(P, w);
         double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
-        double eta, C; double _Complex alpha;
-        cavity_scalars(P, b, A, theta, -1.0, &eta, &alpha, &C);
+        double bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
+        double eta, C, Dc; double _Complex alpha;
+        cavity_scalars(P, b, A, theta, bunch, -1.0, &eta, &alpha, &C, &Dc);
         double epot = 0.0, eint = 0.0;
         for (int i = 0; i < P->nx; ++i)
             for (int j = 0; j < P->ny; ++j) {
@@ -390,7 +414,7 @@ int oracle_observables(const oracle_params *P, const cplx_t *psi, long n, double
         double ekin = 0.5 * k2sum / ksum * norm;
         double ecav = 0.0;
         if (P->cavity_on) {
-            double D = P->delta[b], K = P->kappa[b];
+            double D = P->delta[b] - (P->cav_u0 ? P->n_atoms[b] * P->cav_u0[b] * bunch : 0.0), K = P->kappa[b];
             ecav = P->n_atoms[b] * eta * eta * theta * theta * D / (D * D + K * K);
         }
         double *o = out + (size_t)b * 8;
@@ -443,9 +467,10 @@ int oracle_potential_half_step(const oracle_params *P, cplx_t *psi, double dt, i
         cplx_t *w = psi + (size_t)b * npts;
         double A = oracle_schedule(P, b, (double)n);
         double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
-        double eta, C; double _Complex alpha;
-        cavity_scalars(P, b, A, theta, -1.0, &eta, &alpha, &C);
-        potential_half_step(P, &T, b, w, A, C, dt, imag_time);
+        double bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
+        double eta, C, Dc; double _Complex alpha;
+        cavity_scalars(P, b, A, theta, bunch, -1.0, &eta, &alpha, &C, &Dc);
+        potential_half_step(P, &T, b, w, A, C, Dc, dt, imag_time);
     }
     free_tables(&T);
     return 0;

@@ -57,6 +57,7 @@ class _Params(C.Structure):
         ("eta_or_u", C.c_void_p), ("n_atoms", C.c_void_p), ("delta", C.c_void_p),
         ("kappa", C.c_void_p),
         ("probe_omega", C.c_void_p), ("probe_delta", C.c_void_p), ("probe_phi", C.c_void_p),
+        ("cav_u0", C.c_void_p),
     ]
 
 
@@ -164,6 +165,8 @@ class Oracle:
             for name, default in (("probe_omega", 0.0), ("probe_delta", 0.0), ("probe_phi", 0.0)):
                 a = _f64(np.broadcast_to(np.asarray(p.get(name, default), dtype=np.float64), (B,)), B)
                 setattr(P, name, ptr(a))
+        if p.get("cav_u0") is not None:   # full cavity model, PAPER.md:177,188 (Eqs. 12, 15)
+            P.cav_u0 = ptr(_f64(np.broadcast_to(np.asarray(p["cav_u0"], dtype=np.float64), (B,)), B))
         self.P = P
         self.step = 0
 

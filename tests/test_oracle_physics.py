@@ -452,6 +452,57 @@ def test_probe_closed_form_and_imprint():
     assert np.linalg.norm(a - b) > 1e-6
 
 
+def test_full_cavity_model_closed_forms():
+    """Cavity lattice V_c = U0 |alpha|^2 cos^2(kx) and dispersive shift Delta~ = Delta - N U0 B,
+    B = int cos^2(kx)|psi|^2 (Eqs. 12 and 15).
+    (a) psi = c (1 + eps cos kx cos ky): Theta = c^2 L^2 eps/2, B = c^2 L^2 (1/2 + 3 eps^2/16),
+        c^2 L^2 = 1/(1 + eps^2/4), so alpha = N eta Theta/(Delta - N U0 B + i kappa) in closed form
+        -- pins the definition of B (axis x), the sign of the shift and the factor N.
+    (b) N = 0 with a probe: alpha = dalpha exactly (no shift), and one short step from a uniform
+        state imprints -dt (2 eta Re(dalpha) cos kx cos ky + U0 |dalpha|^2 cos^2 kx): pins the
+        coefficient and the axis of V_c.
+    (c) U0 = 0 is the three-term model of the hot path; real time conserves the norm."""
+    L, n, k = 4 * math.pi, 128, 4.0
+    x = W.axis(n, L)
+    cc = np.cos(k * x)[:, None] * np.cos(k * x)[None, :]
+    eps, eta, N, u0, D, K = 0.3, 1.5, 2.5, 0.8, -1.3, 0.7
+    p = W._base(n, n, L)
+    p["cavity_on"], p["cavity_k"], p["eta_mode"] = 1, k, 0
+    p["eta_or_u"], p["n_atoms"], p["delta"], p["kappa"] = np.array([eta]), np.array([N]), np.array([D]), np.array([K])
+    p["cav_u0"] = np.array([u0])
+    c2L2 = 1.0 / (1.0 + eps * eps / 4.0)
+    psi = (np.sqrt(c2L2) / L * (1.0 + eps * cc)).astype(np.complex128)
+    ob = Oracle(p).observables(psi)[0][0]
+    theta, B = c2L2 * eps / 2.0, c2L2 * (0.5 + 3.0 * eps * eps / 16.0)
+    alpha = N * eta * theta / (D - N * u0 * B + 1j * K)
+    assert ob["norm"] == pytest.approx(1.0, abs=1e-13)
+    assert ob["theta"] == pytest.approx(theta, rel=1e-12)
+    assert ob["re_alpha"] == pytest.approx(alpha.real, rel=1e-12)
+    assert ob["im_alpha"] == pytest.approx(alpha.imag, rel=1e-12)
+    # (b)
+    Om, ph = 0.8, 0.4
+    pb = dict(p); pb["n_atoms"] = np.array([0.0])
+    pb["probe_omega"], pb["probe_delta"], pb["probe_phi"] = np.array([Om]), np.array([11.0]), np.array([ph])
+    u = np.full((n, n), 1.0 / L, dtype=np.complex128)
+    tiny = 1e-6
+    Oracle(pb).evolve(u, tiny, 1, False)
+    da = Om * np.exp(1j * ph) / (D + 1j * K)
+    want = -tiny * (2.0 * eta * da.real * cc + u0 * abs(da) ** 2 * (np.cos(k * x) ** 2)[:, None] * np.ones((1, n)))
+    assert np.allclose(np.angle(u * L), want, rtol=1e-4, atol=1e-12)
+    # (c)
+    q = _cavity_small(8.0, g=5.0)
+    q0 = dict(q); q0["cav_u0"] = np.array([0.0])
+    a, b = q["psi0"].copy(), q["psi0"].copy()
+    Oracle(q0).evolve(a, 1e-3, 5, False); Oracle(q).evolve(b, 1e-3, 5, False)
+    assert np.linalg.norm(a - b) <= 1e-14 * np.linalg.norm(b)
+    q1 = dict(q); q1["cav_u0"] = np.array([3.0])
+    a = q["psi0"].copy()
+    o = Oracle(q1); o.evolve(a, 1e-3, 50, False)
+    assert o.observables(a)[0][0]["norm"] == pytest.approx(1.0, abs=1e-12)
+    b = q["psi0"].copy(); Oracle(q).evolve(b, 1e-3, 50, False)
+    assert np.linalg.norm(a - b) > 1e-6          # and U0 does act
+
+
 def test_interactions_raise_threshold():
     """repulsive interactions increase the critical pump."""
     thetas = {}
