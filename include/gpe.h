@@ -112,6 +112,11 @@ typedef struct {
     const double *probe_omega; /* HOST [batch] Omega_c                                            */
     const double *probe_delta; /* HOST [batch] Delta_p                                            */
     const double *probe_phi;   /* HOST [batch] phi                                                */
+    /* Full cavity model (Eqs. 12 and 15): with U_0 = cav_u0[b] the potential gains the
+     * cavity lattice U_0 |alpha_n|^2 cos^2(k_c x) and Delta is replaced, in alpha_n and in the probe,
+     * by Delta - N_at U_0 B_n, B_n = sum cos^2(k_c x)|psi_n|^2 dx dy (a third fused reduction).
+     * NULL = the three-term model.  Needs cavity_on. */
+    const double *cav_u0;      /* HOST [batch]                                                    */
 } gpe_potential_desc;
 
 /*
@@ -145,7 +150,7 @@ GPE_API gpe_status gpe_evolve(gpe_plan *p, void *psi_dev, double dt, long n_step
  *   e_kin = 1/2 sum (kx^2+ky^2)|psi^|^2 / sum |psi^|^2 * norm
  *   e_pot = sum (V_static + A_n cos^2) |psi|^2 dx dy          (n = the plan's step counter)
  *   e_int = g/2 sum |psi|^4 dx dy
- *   e_cav = N_at eta_n^2 Theta^2 Delta / (Delta^2 + kappa^2)  (its functional derivative is
+ *   e_cav = N_at eta_n^2 Theta^2 Delta / (Delta^2 + kappa^2)  [Delta -> Delta~ with cav_u0]  (its functional derivative is
  *           the interference potential of Eq. 13)
  *   theta, re_alpha, im_alpha as in Eq. 14.
  * out_host: HOST [batch].  density_dev (DEVICE real [batch][nx][ny], or NULL): |psi|^2.

@@ -33,6 +33,7 @@ class gpe_potential_desc(C.Structure):
         ("eta_or_u", C.c_void_p), ("n_atoms", C.c_void_p), ("delta", C.c_void_p),
         ("kappa", C.c_void_p),
         ("probe_omega", C.c_void_p), ("probe_delta", C.c_void_p), ("probe_phi", C.c_void_p),
+        ("cav_u0", C.c_void_p),
     ]
 
 
@@ -239,6 +240,8 @@ class Plan:
             for name in ("probe_omega", "probe_delta", "probe_phi"):
                 a = np.broadcast_to(np.asarray(p.get(name, 0.0), dtype=np.float64), (B,))
                 setattr(d, name, hp(a, B))
+        if p.get("cav_u0") is not None:
+            d.cav_u0 = hp(np.broadcast_to(np.asarray(p["cav_u0"], dtype=np.float64), (B,)), B)
         gpe_set_potential(self.plan, d)
         torch.cuda.current_stream().synchronize()
         self._keep = keep

@@ -54,6 +54,9 @@ struct gpe_plan {
     // device scalars
     MemberState *st = nullptr;
     double2 *partials = nullptr;
+    double *partials_b = nullptr;   // third sum (full cavity model)
+    double *d_u0 = nullptr;         // [batch] U0 of Eqs. 12, 15; nullptr = three-term model
+    std::vector<double> h_u0;
     unsigned int *counters = nullptr;
     int *nonfinite = nullptr;
     double *d_sched_step = nullptr, *d_sched_amp = nullptr;
@@ -209,10 +212,10 @@ template <typename T> gpe_status make_kinetic(gpe_plan *p, double dt, int mode) 
 template <typename T>
 __global__ void __launch_bounds__(256) k_reduce(const cx<T> *psi, int nx, int ny, const T *cavx,
                                                 const T *cavy, int cavity_on, FinalizeParams fin) {
-    __shared__ double red[64];
+    __shared__ double red[96];
     const int b = blockIdx.y;
     const cx<T> *w = psi + (size_t)b * nx * ny;
-    double sn = 0.0, st = 0.0;
+    double sn = 0.0, st = 0.0, sb = 0.0;
     for (int i = blockIdx.x; i < nx; i += gridDim.x) {
         double rn = 0.0, rt = 0.0;
         for (int j = threadIdx.x; j < ny; j += blockDim.x) {
@@ -223,8 +226,9 @@ __global__ void __launch_bounds__(256) k_reduce(const cx<T> *psi, int nx, int ny
         }
         sn += rn;
         if (cavity_on) st += rt * (double)cavx[i];
+        if (fin.cav_u0) sb += rn * ((double)cavx[i] * (double)cavx[i]);
     }
-    block_reduce_and_finalize(fin, b, blockIdx.x, sn, st, red);
+    block_reduce_and_finalize(fin, b, blockIdx.x, sn, st, sb, red);
 }
 
 // Epilogue of an imaginary-time gpe_evolve: apply the pending lazy scale (row a7).
@@ -248,7 +252,7 @@ __global__ void __launch_bounds__(256) k_pending_halfstep(cx<T> *psi, int nx, in
                                                           const MemberState *st) {
     const int b = blockIdx.y;
     if (!st[b].pend) return;
-    const T A = (T)st[b].A_pend, Cc = (T)st[b].C_pend, gg = (flags & F_HAS_G) ? g[b] : T(0);
+    const T A = (T)st[b].A_pend, Cc = (T)st[b].C_pend, Dc = (T)st[b].D_pend, gg = (flags & F_HAS_G) ? g[b] : T(0);
     const size_t npts = (size_t)nx * ny;
     cx<T> *w = psi + (size_t)b * npts;
     const T *v2 = (flags & F_HAS_V2D) ? v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * npts : 0) : nullptr;
@@ -259,6 +263,7 @@ __global__ void __launch_bounds__(256) k_pending_halfstep(cx<T> *psi, int nx, in
         if (flags & F_LAT_X) V += A * latx[i];
         if (flags & F_LAT_Y) V += A * laty[j];
         if (flags & F_CAVITY) V += Cc * cavx[i] * cavy[j];
+        if (flags & F_CAV_FULL) V += Dc * cavx[i] * cavx[i];
         if (v2) V += v2[q];
         cx<T> z = w[q];
         const T ang = (V + gg * (z.x * z.x + z.y * z.y)) * half_dt;
@@ -303,7 +308,7 @@ __global__ void __launch_bounds__(256) k_obs_real(const cx<T> *psi, int nx, int 
     const cx<T> *w = psi + (size_t)b * npts;
     const T *v2 = (flags & F_HAS_V2D) ? v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * npts : 0) : nullptr;
     const double Ab = A[b];
-    double sn = 0, sp = 0, s4 = 0, st = 0;
+    double sn = 0, sp = 0, s4 = 0, st = 0, sb = 0;
     for (int i = blockIdx.x; i < nx; i += gridDim.x)
         for (int j = threadIdx.x; j < ny; j += blockDim.x) {
             size_t q = (size_t)i * ny + j;
@@ -318,11 +323,13 @@ __global__ void __launch_bounds__(256) k_obs_real(const cx<T> *psi, int nx, int 
             if (v2) V += (double)v2[q];
             sn += d; sp += V * d; s4 += d * d;
             if (flags & F_CAVITY) st += (double)cavx[i] * (double)cavy[j] * d;
+            if (flags & F_CAV_FULL) sb += (double)cavx[i] * (double)cavx[i] * d;
         }
     block_atomic_add(sn, out + b * 8 + 0, red);
     block_atomic_add(sp, out + b * 8 + 1, red);
     block_atomic_add(s4, out + b * 8 + 2, red);
     block_atomic_add(st, out + b * 8 + 3, red);
+    if (flags & F_CAV_FULL) block_atomic_add(sb, out + b * 8 + 6, red);
 }
 
 // k-space sums: out[b][4] += sum |psi^|^2, out[b][5] += sum k^2 |psi^|^2
@@ -400,6 +407,7 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     a.kin_xr = (const T *)p->kin_x; a.kin_yr = (const T *)p->kin_y;
     a.inv_p = (T)(1.0 / ((double)p->nx * (double)p->ny));
     FinalizeParams &f = a.fin;
+    f.partials_b = p->partials_b; f.cav_u0 = p->d_u0;
     f.st = p->st; f.partials = p->partials; f.counters = p->counters; f.nonfinite = p->nonfinite;
     f.sched_len = p->sched_len; f.sched_step = p->d_sched_step; f.sched_amp = p->d_sched_amp;
     f.sched_batched = p->sched_batched;
@@ -448,7 +456,8 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     a.fin.cpm = p->nx / (paired ? oy->p_rows_per_cta : oy->rows_per_cta);
     a.fin.normalise = imag ? 1 : 0;
     a.fin.advance = 1;
-    a.fin.prepared = 1;   // pass B prepares the coefficients of the next step (prepare_member)
+    a.fin.prepared = p->d_u0 ? 0 : 1;   // pass B prepares the coefficients of the next step (prepare_member);
+                                        // with the dispersive shift they depend on the sums
     // real time: pass C leaves its half-step to the next pass A (one multiply
     // by exp(-i (V_n + V_{n+1} + 2 g |psi|^2) dt/2) instead of two; |psi|^2, hence Theta, is unchanged)
     a.fin.merged = (!imag && !getenv("GPE_NO_MERGE")) ? 1 : 0;
@@ -595,7 +604,8 @@ gpe_status observables_impl(gpe_plan *p, const void *psi, gpe_obs *out, void *de
         o.e_cav = 0.0; o.re_alpha = 0.0; o.im_alpha = 0.0;
         if (p->cavity_on) {
             double eta = p->eta_mode == 0 ? p->h_eta[b] : sqrt(fabs(A[b]) * p->h_eta[b]);
-            double D = p->h_delta[b], K = p->h_kappa[b], den = D * D + K * K;
+            double D = p->h_delta[b] - (p->h_u0.empty() ? 0.0 : p->h_natoms[b] * p->h_u0[b] * r[6] * dxdy);   // Eq. 15
+            double K = p->h_kappa[b], den = D * D + K * K;
             double num = p->h_natoms[b] * eta * o.theta;
             o.re_alpha = num * D / den;
             o.im_alpha = -num * K / den;
@@ -657,6 +667,7 @@ template <typename T> gpe_status set_potential_impl(gpe_plan *p, const gpe_poten
     }
     if (d->cavity_on) {
         flags |= F_CAVITY;
+        if (d->cav_u0) flags |= F_CAV_FULL;
         for (int i = 0; i < nx; ++i) cxv[i] = cos(d->cavity_k * coord(i, nx, p->Lx));
         for (int j = 0; j < ny; ++j) cyv[j] = cos(d->cavity_k * coord(j, ny, p->Ly));
     }
@@ -723,6 +734,7 @@ gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly,
         GPE_CUDA(p, cudaMalloc((void **)&p->st, sizeof(MemberState) * batch));
         GPE_CUDA(p, cudaMemset(p->st, 0, sizeof(MemberState) * batch));
         GPE_CUDA(p, cudaMalloc((void **)&p->partials, sizeof(double2) * (size_t)batch * kMaxCpm));
+        GPE_CUDA(p, cudaMalloc((void **)&p->partials_b, sizeof(double) * (size_t)batch * kMaxCpm));
         GPE_CUDA(p, cudaMalloc((void **)&p->counters, sizeof(unsigned int) * batch));
         GPE_CUDA(p, cudaMemset(p->counters, 0, sizeof(unsigned int) * batch));
         GPE_CUDA(p, cudaMalloc((void **)&p->d_call, sizeof(CallParams)));
@@ -753,7 +765,7 @@ gpe_status gpe_plan_destroy(gpe_plan *p) {
     if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
-                    p->ytab, p->g, p->v2d, p->st, p->partials, p->counters, p->nonfinite, p->d_sched_step,
+                    p->ytab, p->g, p->v2d, p->st, p->partials, p->partials_b, p->d_u0, p->counters, p->nonfinite, p->d_sched_step,
                     p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->d_probe_omega, p->d_probe_delta,
                     p->d_probe_phi, p->scratch, p->obs_dev,
                     p->pop_dev, p->obsA_dev};
@@ -775,6 +787,7 @@ gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
         if (i > 0 && d->sched_step[i] < d->sched_step[i - 1])
             return fail(p, GPE_EINVAL, "sched_step must be non-decreasing");
     }
+    if (d->cav_u0 && !d->cavity_on) return fail(p, GPE_EINVAL, "cav_u0 needs cavity_on");
     if ((d->probe_omega || d->probe_delta || d->probe_phi) && (!d->cavity_on || !d->probe_omega))
         return fail(p, GPE_EINVAL, "the probe needs cavity_on and probe_omega");
     if (d->cavity_on && (!d->eta_or_u || !d->delta || !d->kappa))
@@ -816,6 +829,9 @@ gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
             if (d->probe_delta) de.assign(d->probe_delta, d->probe_delta + B);
             if (d->probe_phi) ph.assign(d->probe_phi, d->probe_phi + B);
         }
+        p->h_u0.clear();
+        if (d->cav_u0) p->h_u0.assign(d->cav_u0, d->cav_u0 + B);
+        if ((s = upload_f64(p, &p->d_u0, p->h_u0)) != GPE_OK) return s;
         if ((s = upload_f64(p, &p->d_probe_omega, om)) != GPE_OK) return s;
         if ((s = upload_f64(p, &p->d_probe_delta, de)) != GPE_OK) return s;
         if ((s = upload_f64(p, &p->d_probe_phi, ph)) != GPE_OK) return s;

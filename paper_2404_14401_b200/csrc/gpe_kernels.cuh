@@ -70,13 +70,15 @@ __device__ inline double schedule_at(const FinalizeParams &f, int b, double n) {
 // (Eqs. 13-14).
 // Probe (Eq. 17, real time): alpha_n += pre + i pim = Omega exp(i (Delta_p n dt + phi)) / (Delta + i kappa),
 // C_n += pc = 2 eta_n pre.
-__device__ inline void step_coefficients(const FinalizeParams &f, int b, long long n, double &A, double &kre, double &kim, double &kc,
-                                         double &pre, double &pim, double &pc) {
+// bunch = int cos^2(k_c x)|psi|^2 (full cavity model: Delta -> Delta - N U0 bunch, Eq. 15).
+__device__ inline void step_coefficients(const FinalizeParams &f, int b, long long n, double bunch, double &A, double &kre, double &kim,
+                                         double &kc, double &pre, double &pim, double &pc) {
     A = schedule_at(f, b, (double)n);
     kre = kim = kc = pre = pim = pc = 0.0;
     if (f.cavity_on) {
         const double eta = f.eta_mode == 0 ? f.eta_or_u[b] : sqrt(fabs(A) * f.eta_or_u[b]);
-        const double D = f.delta[b], K = f.kappa[b], den = D * D + K * K, ne = f.n_atoms[b] * eta;
+        const double D = f.delta[b] - (f.cav_u0 ? f.n_atoms[b] * f.cav_u0[b] * bunch : 0.0);
+        const double K = f.kappa[b], den = D * D + K * K, ne = f.n_atoms[b] * eta;
         kre = ne * D / den;                       // 1 / (D + iK) = (D - iK) / (D^2 + K^2)
         kim = -ne * K / den;
         kc = 2.0 * eta * kre;
@@ -93,13 +95,13 @@ __device__ inline void step_coefficients(const FinalizeParams &f, int b, long lo
 // Called by one thread of pass B per member while step n runs: coefficients of step n + 1.
 __device__ inline void prepare_member(const FinalizeParams &f, int b) {
     MemberState &s = f.st[b];
-    step_coefficients(f, b, s.step + 1, s.nA, s.nKre, s.nKim, s.nKc, s.nPre, s.nPim, s.nPc);
+    step_coefficients(f, b, s.step + 1, 0.0, s.nA, s.nKre, s.nKim, s.nKc, s.nPre, s.nPim, s.nPc);
 }
 
 // Called by one thread of the last block of member b with the raw sums over the stored psi.
-__device__ inline void finalize_member(const FinalizeParams &f, int b, double sum_n, double sum_t) {
+__device__ inline void finalize_member(const FinalizeParams &f, int b, double sum_n, double sum_t, double sum_b) {
     MemberState &s = f.st[b];
-    double norm = sum_n * f.dxdy, theta = sum_t * f.dxdy;
+    double norm = sum_n * f.dxdy, theta = sum_t * f.dxdy, bunch = sum_b * f.dxdy;
     if (!(norm == norm) || norm > 1e300 || norm < 0.0 || (f.normalise && !(norm > 0.0))) *f.nonfinite = 1;
     long long n1;
     if (f.advance) n1 = s.step + 1; else n1 = f.step0;
@@ -107,6 +109,7 @@ __device__ inline void finalize_member(const FinalizeParams &f, int b, double su
     if (f.normalise) {
         scale = 1.0 / sqrt(norm);
         theta = theta / norm;
+        bunch = bunch / norm;
         norm = 1.0;
     }
     double A, re_a = 0.0, im_a = 0.0, C = 0.0;
@@ -114,10 +117,12 @@ __device__ inline void finalize_member(const FinalizeParams &f, int b, double su
         A = s.nA; re_a = s.nKre * theta + s.nPre; im_a = s.nKim * theta + s.nPim; C = s.nKc * theta + s.nPc;
     } else {
         double kre, kim, kc, pre, pim, pc;
-        step_coefficients(f, b, n1, A, kre, kim, kc, pre, pim, pc);
+        step_coefficients(f, b, n1, bunch, A, kre, kim, kc, pre, pim, pc);
         re_a = kre * theta + pre; im_a = kim * theta + pim; C = kc * theta + pc;
     }
-    if (f.advance && f.merged) { s.A_pend = s.A; s.C_pend = s.C; s.pend = 1; } else s.pend = 0;
+    const double Dc = f.cav_u0 ? f.cav_u0[b] * (re_a * re_a + im_a * im_a) : 0.0;   // Eq. 12
+    if (f.advance && f.merged) { s.A_pend = s.A; s.C_pend = s.C; s.D_pend = s.D; s.pend = 1; } else s.pend = 0;
+    s.D = Dc;
     s.scale = scale; s.A = A; s.C = C; s.norm = norm; s.theta = theta;
     s.re_alpha = re_a; s.im_alpha = im_a; s.step = n1;
     if (!f.advance && b == 0) {
@@ -140,17 +145,19 @@ __device__ __forceinline__ double warp_sum(double v) {
 // Block-level sum of (sn, st), one partial per CTA, last CTA of the member finalises.
 // `red` is shared scratch of at least 2*32 doubles.  All threads of the CTA must call this.
 __device__ inline void block_reduce_and_finalize(const FinalizeParams &f, int b, int cta_in_member,
-                                                 double sn, double st, double *red) {
+                                                 double sn, double st, double sb, double *red) {
     sn = warp_sum(sn);
     st = warp_sum(st);
+    if (f.cav_u0) sb = warp_sum(sb);
     int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    if (lane == 0) { red[w] = sn; red[32 + w] = st; }
+    if (lane == 0) { red[w] = sn; red[32 + w] = st; red[64 + w] = sb; }
     __syncthreads();
     __shared__ int is_last;
     if (threadIdx.x == 0) {
-        double a = 0.0, c = 0.0;
-        for (int i = 0; i < nw; ++i) { a += red[i]; c += red[32 + i]; }
+        double a = 0.0, c = 0.0, e = 0.0;
+        for (int i = 0; i < nw; ++i) { a += red[i]; c += red[32 + i]; e += red[64 + i]; }
         f.partials[(size_t)b * f.cpm + cta_in_member] = make_double2(a, c);
+        if (f.cav_u0) f.partials_b[(size_t)b * f.cpm + cta_in_member] = e;
         __threadfence();
         unsigned int old = atomicAdd(&f.counters[b], 1u);
         is_last = (old == (unsigned int)(f.cpm - 1));
@@ -159,12 +166,17 @@ __device__ inline void block_reduce_and_finalize(const FinalizeParams &f, int b,
     if (is_last && w == 0) {
         __threadfence();
         const volatile double2 *p = f.partials + (size_t)b * f.cpm;
-        double a = 0.0, c = 0.0;
+        double a = 0.0, c = 0.0, e = 0.0;
         for (int i = lane; i < f.cpm; i += 32) { a += p[i].x; c += p[i].y; }
+        if (f.cav_u0) {
+            const volatile double *pb = f.partials_b + (size_t)b * f.cpm;
+            for (int i = lane; i < f.cpm; i += 32) e += pb[i];
+            e = warp_sum(e);
+        }
         a = warp_sum(a);
         c = warp_sum(c);
         if (lane == 0) {
-            finalize_member(f, b, a, c);
+            finalize_member(f, b, a, c, e);
             f.counters[b] = 0u;
         }
     }
@@ -241,10 +253,10 @@ __device__ __forceinline__ void sincosm1_small(float w, float *s, float *cm1) {
 // REDUCE: also returns sum |psi_new|^2 and sum cos(k_c y) |psi_new|^2 over the 16 points.
 template <typename T, bool IMAG, bool REDUCE, int M1>
 __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<T, cx<T>> &a, int b, int i, int j,
-                                                 T scale, T fac, T A, T Cc, T &sn, T &st) {
+                                                 T scale, T fac, T A, T Cc, T vadd, T &sn, T &st) {
     using V4 = typename Vec4<T>::type;
     const int flags = a.flags;
-    T vrow = T(0);
+    T vrow = vadd;   // per-row constant supplied by the caller (cavity lattice D cos^2(k_c x_i))
     // fac = 1, or 2 when the multiply also carries the pending second half-step of the previous
     // step (real time; A, Cc are then the sums of the two steps' coefficients)
     if (flags & F_HAS_SEP) vrow += fac * a.vx[i];
@@ -397,8 +409,9 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
             const MemberState &ms = a.fin.st[b];
             T sn, st;
             const bool pend = !IMAG && ms.pend;
+            const T cx2 = (a.flags & F_CAV_FULL) ? a.cavx[i] * a.cavx[i] : T(0);
             potential_step16<T, IMAG, false, F::M1>(v, a, b, i, j, (T)ms.scale, pend ? T(2) : T(1), (T)(pend ? ms.A + ms.A_pend : ms.A),
-                                                    (T)(pend ? ms.C + ms.C_pend : ms.C), sn, st);
+                                                    (T)(pend ? ms.C + ms.C_pend : ms.C), (T)(pend ? ms.D + ms.D_pend : ms.D) * cx2, sn, st);
         }
         F::fwd(v, sm, j, a.tw_y, a.tw1_y);
         {
@@ -489,7 +502,7 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
     unsigned char *stage = smem_raw + sizeof(C) * G::RPC * F::SLOTS;
-    __shared__ double red[64];
+    __shared__ double red[96];
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     C *sm = smem + r * F::SLOTS;
     const long ngroups = (long)a.batch * a.nx / G::RPC;
@@ -530,11 +543,13 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
                 sn += d;
                 if (a.flags & F_CAVITY) st = fma(d, a.ytab[4 * (j + F::M1 * k) + 2], st);
             }
-        } else potential_step16<T, IMAG, true, F::M1>(v, a, b, i, j, T(1), T(1), (T)ms.A, (T)ms.C, sn, st);
+        } else potential_step16<T, IMAG, true, F::M1>(v, a, b, i, j, T(1), T(1), (T)ms.A, (T)ms.C,
+                                                      (a.flags & F_CAV_FULL) ? (T)ms.D * a.cavx[i] * a.cavx[i] : T(0), sn, st);
 #pragma unroll
         for (int k = 0; k < 16; ++k) dst[j + F::M1 * k] = v[k];
         double dn = (double)sn, dt_ = (a.flags & F_CAVITY) ? (double)st * (double)a.cavx[i] : 0.0;
-        block_reduce_and_finalize(a.fin, b, (int)(grp % gpm), dn, dt_, red);
+        const double db_ = (a.flags & F_CAV_FULL) ? dn * ((double)a.cavx[i] * (double)a.cavx[i]) : 0.0;
+        block_reduce_and_finalize(a.fin, b, (int)(grp % gpm), dn, dt_, db_, red);
         if constexpr (!STAGED) __syncthreads();
     }
 }

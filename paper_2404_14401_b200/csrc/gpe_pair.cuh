@@ -86,9 +86,9 @@ __device__ __forceinline__ size_t ipos(long i, int kp, size_t hy) { return ((siz
 template <bool IMAG, bool REDUCE, int M1, int H>
 __device__ __forceinline__ void potential_pair16(float2 (&p0)[16], float2 (&p1)[16], const StepArgs<float, float2> &a,
                                                  int b, int i, int j, float scale, float fac, float A, float Cc,
-                                                 float2 &sn, float2 &st) {
+                                                 float vadd, float2 &sn, float2 &st) {
     const int flags = a.flags;
-    float vrow = 0.f;
+    float vrow = vadd;   // per-row constant from the caller: cavity lattice D cos^2(k_c x_i) (Eq. 12)
     // fac = 1, or 2 when this multiply also carries the pending second half-step of the previous
     // step (then A, Cc are the sums of the two steps' coefficients): static terms and g count twice
     if (flags & F_HAS_SEP) vrow += fac * a.vx[i];
@@ -213,8 +213,10 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
         const MemberState &ms = a.fin.st[b];
         float2 sn, st;
         const bool pend = !IMAG && ms.pend;
+        const float cx2 = (a.flags & F_CAV_FULL) ? a.cavx[i] * a.cavx[i] : 0.f;
         potential_pair16<IMAG, false, M1, H>(p0, p1, a, b, i, j, (float)ms.scale, pend ? 2.f : 1.f,
-                                             (float)(pend ? ms.A + ms.A_pend : ms.A), (float)(pend ? ms.C + ms.C_pend : ms.C), sn, st);
+                                             (float)(pend ? ms.A + ms.A_pend : ms.A), (float)(pend ? ms.C + ms.C_pend : ms.C),
+                                             (float)(pend ? ms.D + ms.D_pend : ms.D) * cx2, sn, st);
     }
     // radix-2 decimation in frequency across the two halves of the row: lane 0 <- x[n] + x[n+H],
     // lane 1 <- (x[n] - x[n+H]) w_NY^n; scalar instructions, they write the split lane layout
@@ -323,7 +325,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     using F = Fft1D<G::H, 1, cpair>;
     constexpr int H = G::H, M1 = F::M1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double red[64];
+    __shared__ double red[96];
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     float2 *sm = reinterpret_cast<float2 *>(smem_raw) + r * F::TILE;
     const long row = (long)blockIdx.x * G::RPC + r;
@@ -370,7 +372,8 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     const MemberState &ms = a.fin.st[b];
     float2 sn = make_float2(0.f, 0.f), st = sn;
     if constexpr (MERGED) reduce_pair16<M1>(p0, p1, a, j, sn, st);
-    else potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, 1.f, (float)ms.A, (float)ms.C, sn, st);
+    else potential_pair16<IMAG, true, M1, H>(p0, p1, a, b, i, j, 1.f, 1.f, (float)ms.A, (float)ms.C,
+                                             (a.flags & F_CAV_FULL) ? (float)ms.D * a.cavx[i] * a.cavx[i] : 0.f, sn, st);
     float2 *dst = a.dst + row * NY;
     // Reduction first, wavefunction stores second: the partial sums of this CTA are published
     // (store, fence, counter increment) while thread 0 has no stores in flight, so the fence does
@@ -378,19 +381,23 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     // the stores.  Fixed summation order everywhere (bitwise reproducible, batch == single).
     const FinalizeParams &f = a.fin;
     const int cim = (int)(blockIdx.x % gpm);
-    double dn = warp_sum((double)sn.x + (double)sn.y);
+    const double rown = (double)sn.x + (double)sn.y;
+    double dn = warp_sum(rown);
     double dt_ = (a.flags & F_CAVITY) ? warp_sum(((double)st.x + (double)st.y) * (double)a.cavx[i]) : 0.0;
+    const bool full = a.flags & F_CAV_FULL;   // third sum: cos^2(k_c x_i) times the row's |psi|^2 (Eq. 15)
+    double db_ = full ? warp_sum(rown * ((double)a.cavx[i] * (double)a.cavx[i])) : 0.0;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     constexpr int NW = G::THREADS / 32;
     __shared__ int is_last;
-    if (lane == 0) { red[wid] = dn; red[32 + wid] = dt_; }
+    if (lane == 0) { red[wid] = dn; red[32 + wid] = dt_; red[64 + wid] = db_; }
     __syncthreads();
     unsigned int old = 0;
     if (threadIdx.x == 0) {
-        double s0 = 0.0, s1 = 0.0;
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
 #pragma unroll
-        for (int q = 0; q < NW; ++q) { s0 += red[q]; s1 += red[32 + q]; }
+        for (int q = 0; q < NW; ++q) { s0 += red[q]; s1 += red[32 + q]; s2 += red[64 + q]; }
         f.partials[(size_t)b * f.cpm + cim] = make_double2(s0, s1);
+        if (full) f.partials_b[(size_t)b * f.cpm + cim] = s2;
         __threadfence();
         old = atomicAdd(&f.counters[b], 1u);
     }
@@ -401,17 +408,22 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     if (is_last) {   // the last CTA of the member: all its threads sum the partials
         __threadfence();
         const volatile double2 *pp = f.partials + (size_t)b * f.cpm;
-        double s0 = 0.0, s1 = 0.0;
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
         for (int q = threadIdx.x; q < f.cpm; q += G::THREADS) { s0 += pp[q].x; s1 += pp[q].y; }
+        if (full) {
+            const volatile double *pb = f.partials_b + (size_t)b * f.cpm;
+            for (int q = threadIdx.x; q < f.cpm; q += G::THREADS) s2 += pb[q];
+            s2 = warp_sum(s2);
+        }
         s0 = warp_sum(s0); s1 = warp_sum(s1);
         __syncthreads();
-        if (lane == 0) { red[wid] = s0; red[32 + wid] = s1; }
+        if (lane == 0) { red[wid] = s0; red[32 + wid] = s1; red[64 + wid] = s2; }
         __syncthreads();
         if (threadIdx.x == 0) {
-            double t0 = 0.0, t1 = 0.0;
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0;
 #pragma unroll
-            for (int q = 0; q < NW; ++q) { t0 += red[q]; t1 += red[32 + q]; }
-            finalize_member(f, b, t0, t1);
+            for (int q = 0; q < NW; ++q) { t0 += red[q]; t1 += red[32 + q]; t2 += red[64 + q]; }
+            finalize_member(f, b, t0, t1, t2);
             f.counters[b] = 0u;
         }
     }

@@ -23,6 +23,9 @@ struct MemberState {
     // A_{n+1}; Re alpha = nKre Theta, Im alpha = nKim Theta, C = nKc Theta
     double nA, nKre, nKim, nKc;
     double nPre, nPim, nPc;   // probe: alpha += nPre + i nPim, C += nPc (zero without a probe)
+    // full cavity model (Eq. 12): coefficient D_n = U0 |alpha_n|^2 of cos^2(k_c x) of the
+    // upcoming step, and the one of the pending half-step
+    double D, D_pend;
 };
 
 // Per-gpe_evolve-call parameters kept in device memory (written by the prologue kernel), so that
@@ -36,6 +39,7 @@ struct CallParams {
 struct FinalizeParams {
     MemberState *st;          // [batch]
     double2 *partials;        // [batch][cpm] (sum |psi|^2, sum cos cos |psi|^2)
+    double *partials_b;       // [batch][cpm] sum cos^2(k_c x) |psi|^2 (full cavity model only)
     unsigned int *counters;   // [batch]
     int *nonfinite;           // sticky flag
     int cpm;                  // CTAs per member in the reducing pass
@@ -46,6 +50,7 @@ struct FinalizeParams {
     int cavity_on, eta_mode;
     const double *eta_or_u, *n_atoms, *delta, *kappa;  // [batch]
     const double *probe_omega, *probe_delta, *probe_phi;  // [batch] or nullptr (Eq. 17)
+    const double *cav_u0;     // [batch] U0 of Eqs. 12 and 15, or nullptr (three-term model)
     double probe_dt;          // dt of the running real-time evolution; 0 = no probe (imaginary time)
     double dxdy;
     long long record_every, rec_first;  // prologue only (advance == 0): copied into *call
@@ -67,7 +72,8 @@ enum : int {
     F_LAT_Y = 16,     // A cos^2(k_l y)
     F_CAVITY = 32,
     F_HAS_G = 64,
-    F_NO_POT = 128    // plain FFT pass (observables)
+    F_NO_POT = 128,   // plain FFT pass (observables)
+    F_CAV_FULL = 256  // cavity lattice D_n cos^2(k_c x) and dispersive shift (needs the third sum)
 };
 
 // Arguments of the three passes of one step.  T = float / double.

@@ -333,6 +333,44 @@ def test_merged_half_steps_equal_separate_ones(monkeypatch, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("mode", ["real", "imag"])
+@pytest.mark.parametrize("nx,ny", [(256, 128), (64, 64), (128, 1024)])
+def test_full_cavity_model_parity(nx, ny, mode, dtype):
+    """Cavity lattice U0|alpha|^2 cos^2(kx) and dispersive shift (Eqs. 12, 15):
+    psi, records and observables against the oracle; batch of 2 with U0 = (8, 0) -- the second
+    member is the three-term model -- plus a probe on member 0 in real time."""
+    p = _general_workload(nx, ny, batch=2)
+    p["cav_u0"] = np.array([8.0, 0.0])
+    p["probe_omega"], p["probe_delta"], p["probe_phi"] = np.array([3.0, 0.0]), np.array([30.0, 0.0]), np.array([0.2, 0.0])
+    dt = 1e-3
+    plan = _gpu_plan(p, dtype)
+    psi = _to_dev(p["psi0"], dtype)
+    ref = _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    rg = np.concatenate([plan.evolve(psi, dt, n, mode, record_every=1).cpu().numpy() for n in (3, 17)])
+    ro = np.concatenate([o.evolve(ref, dt, n, mode == "imag", record_every=1) for n in (3, 17)])
+    e = _rel(psi.cpu().numpy(), ref)
+    assert e <= 20 * PER_STEP[dtype], f"{e:.3e}"
+    tol = 1e-5 if dtype == "c64" else 1e-10
+    for c in (1, 2, 3, 4, 5):
+        assert np.all(np.abs(rg[:, :, c] - ro[:, :, c]) <= tol * np.maximum(np.abs(ro[:, :, c]), 1e-2)), c
+    og, oo = plan.observables(psi)[0], o.observables(ref)[0]
+    for b in range(2):
+        for k in ("norm", "theta", "re_alpha", "im_alpha", "e_cav"):
+            assert abs(og[b][k] - oo[b][k]) <= tol * max(abs(oo[b][k]), 1e-2), (b, k)
+    # U0 matters at the level the test resolves: the recorded field of member 0 moves by > 10 %
+    # (dispersive shift), and in real time (probe-driven field) psi itself by > 10 tolerances
+    pn = dict(p); pn["cav_u0"] = np.array([0.0, 0.0])
+    ref2 = _oracle_input(p["psi0"], dtype)
+    r2 = Oracle(pn).evolve(ref2, dt, 20, mode == "imag", record_every=1)
+    assert np.max(np.abs(r2[:, 0, 3] - ro[:, 0, 3]) / np.abs(ro[:, 0, 3])) > 0.1
+    assert np.allclose(r2[:, 1, 3], ro[:, 1, 3], rtol=1e-9, atol=1e-15)
+    if mode == "real":
+        assert _rel(ref2[0], ref[0]) > 10 * 20 * PER_STEP["c64"]
+    plan.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
 def test_probe_parity_and_records(dtype):
     """On-axis cavity probe (Eq. 17): psi and the recorded cavity field against
     the oracle over two gpe_evolve calls (the probe's time origin is the plan's step counter),
