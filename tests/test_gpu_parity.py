@@ -454,6 +454,14 @@ def test_error_behaviour():
         G.gpe_evolve(plan, psi.data_ptr(), -1e-3, 1, G.GPE_IMAG_TIME)
     assert e.value.status == 1
     G.gpe_evolve(plan, psi.data_ptr(), 1e-3, 0, G.GPE_REAL_TIME)  # empty run is fine
+    # probe / full cavity model without the cavity, probe phase without an amplitude
+    import ctypes as C
+    one = (C.c_double * 1)(1.0)
+    ptr = C.cast(one, C.c_void_p)
+    for kw in (dict(cav_u0=ptr), dict(probe_omega=ptr), dict(cavity_on=1, cavity_k=1.0, eta_or_u=ptr, delta=ptr, kappa=ptr, probe_phi=ptr)):
+        with pytest.raises(G.GpeError) as e:
+            G.gpe_set_potential(plan, G.gpe_potential_desc(lattice_axis=-1, **kw))
+        assert e.value.status == 1, kw
     # all-zero psi in imaginary time: norm 0 -> non-finite scale -> sticky flag
     G.gpe_evolve(plan, psi.data_ptr(), 1e-3, 2, G.GPE_IMAG_TIME)
     with pytest.raises(G.GpeError) as e:
