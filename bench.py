@@ -130,6 +130,41 @@ def cpu_baseline(nx: int, budget_s: float = 15.0):
                       f"({dt:.1f} s, OpenMP over rows/columns/points)"}
 
 
+def other_workloads(G, torch, peak):
+    """Short device-resident timings of the other BASELINE.json configs (parity-test workloads, not
+    the bench line): updates/s, us per split-step and the fraction of the 48 (complex64) or 96
+    (complex128) bytes/point roofline.  One warm-up call, then CUDA events around one gpe_evolve."""
+    import numpy as np
+    import workloads as W
+    out = {}
+    cases = (("config2_256_c64_real", lambda: W.config3(n=256), "c64", 1, "real", 1e-4, 2000),
+             ("config3_1024_c64_imag", lambda: W.config3(n=1024), "c64", 1, "imag", 5e-4, 400),
+             ("config4_2048_c128_real", lambda: W.config4(n=2048), "c128", 1, "real", 1e-4, 100),
+             ("config5_64x512_c64_imag", lambda: W.config5(n=512, side=8, n_steps=1), "c64", 64, "imag", 5e-4, 100))
+    for name, make, dtype, batch, mode, dt, steps in cases:
+        p = make()
+        n = p["nx"]
+        plan = G.Plan(n, n, p["Lx"], p["Ly"], dtype, batch)
+        plan.set_potential(p)
+        cd = np.complex64 if dtype == "c64" else np.complex128
+        psi = torch.from_numpy(np.ascontiguousarray(p["psi0"].astype(cd))).cuda()
+        plan.evolve(psi, dt, max(16, steps // 4), mode)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        plan.evolve(psi, dt, steps, mode)
+        e1.record()
+        torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) / steps * 1e3
+        pts = batch * n * n
+        bpp = 48.0 if dtype == "c64" else 96.0
+        out[name] = {"updates_per_s": pts / (us * 1e-6), "us_per_split_step": us,
+                     "roofline_frac": pts * bpp / (us * 1e-6) / 1e9 / peak}
+        plan.close()
+        del psi
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -298,6 +333,8 @@ def run_ours(args):
                                    "frac": step_alg / (step_ms * 1e-3) / 1e9 / peak,
                                    "algorithmic_bytes_per_step": step_alg, "us_per_split_step": step_ms * 1e3}}
     plan.close()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        extra["other_workloads"] = other_workloads(G, torch, peak)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(nx)
