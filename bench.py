@@ -165,6 +165,54 @@ def other_workloads(G, torch, peak):
     return out
 
 
+def torch_fft_comparison(torch, nx: int, steps: int = 40):
+    """Comparison point only (north_star): the paper's own design -- torch.fft (cuFFT) plus separate
+    PyTorch element-wise kernels -- written from the paper's description for the
+    bench workload (config 4, complex64, real time), all on the device with no host synchronisation
+    inside the loop.  Not part of the product and not used by it."""
+    import math
+    import numpy as np
+    import workloads as W
+    p = W.config4(n=nx)
+    L, dt, g, k = p["Lx"], 1e-4, float(p["g"][0]), float(p["cavity_k"])
+    dev = torch.device("cuda")
+    x = torch.tensor(W.axis(nx, L), dtype=torch.float32, device=dev)
+    cx_, cy_ = torch.cos(k * x)[:, None], torch.cos(k * x)[None, :]
+    vtrap = 0.5 * (x[:, None] ** 2 + x[None, :] ** 2)
+    lat, cc = (cy_ ** 2).expand(nx, nx).contiguous(), (cx_ * cy_).contiguous()
+    kk = torch.tensor(2.0 * math.pi * np.fft.fftfreq(nx, d=L / nx), dtype=torch.float32, device=dev)
+    kin = torch.exp(-0.5j * dt * (kk[:, None] ** 2 + kk[None, :] ** 2).to(torch.complex64))
+    psi = torch.from_numpy(p["psi0"].astype(np.complex64)).to(dev)
+    u, delta, kappa = float(p["eta_or_u"][0]), float(p["delta"][0]), float(p["kappa"][0])
+    dxdy = (L / nx) ** 2
+    ramp = torch.tensor([20.0 * n / 10000.0 for n in range(steps + 8)], dtype=torch.float32, device=dev)
+
+    def step(n):
+        nonlocal psi
+        dens = psi.real ** 2 + psi.imag ** 2
+        theta = (cc * dens).sum() * dxdy
+        A = ramp[n]
+        eta = torch.sqrt(A * u)
+        C = 2.0 * eta * (eta * theta * delta / (delta * delta + kappa * kappa))
+        V = vtrap + A * lat + C * cc
+        psi = psi * torch.exp(-0.5j * dt * (V + g * dens))
+        psi = torch.fft.ifft2(torch.fft.fft2(psi) * kin)
+        psi = psi * torch.exp(-0.5j * dt * (V + g * (psi.real ** 2 + psi.imag ** 2)))
+
+    for n in range(8):
+        step(n)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for n in range(8, 8 + steps):
+        step(n)
+    e1.record()
+    torch.cuda.synchronize()
+    us = e0.elapsed_time(e1) / steps * 1e3
+    return {"kind": "torch.fft (cuFFT) + separate PyTorch element-wise kernels: the paper's own design, "
+                    "comparison point only", "us_per_split_step": us, "updates_per_s": nx * nx / (us * 1e-6)}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -335,6 +383,7 @@ def run_ours(args):
     plan.close()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         extra["other_workloads"] = other_workloads(G, torch, peak)
+        extra["comparison"] = torch_fft_comparison(torch, nx)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(nx)
