@@ -308,7 +308,7 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else None
     local_ms = sum(a.elapsed_time(b) for a, b in evs)
-    launches = K * (1 + 3 * inner)
+    launches = K * (1 + 3 * inner + 2)     # prologue reduction, 3 passes per split-step, pending half-step + flag reset
 
     def rmax(x):
         if dist is None:
