@@ -41,7 +41,7 @@ struct gpe_plan {
     void *tw1_x = nullptr, *tw1_y = nullptr;
     void *tw_hy = nullptr, *tw1_hy = nullptr;  // length ny/2 (paired row passes)
     void *ytab2 = nullptr;
-    void *kin_x = nullptr, *kin_y = nullptr;
+    void *kin_x = nullptr, *kin_y = nullptr, *kin_y2 = nullptr;
     double kin_dt = 0.0;
     int kin_mode = -1;
     void *vx = nullptr, *vy = nullptr, *latx = nullptr, *laty = nullptr, *cavx = nullptr, *cavy = nullptr;
@@ -181,6 +181,7 @@ template <typename T> gpe_status make_kinetic(gpe_plan *p, double dt, int mode) 
     if (p->kin_mode != mode) {  // element size changes between real (complex table) and imaginary
         if (p->kin_x) { cudaFree(p->kin_x); p->kin_x = nullptr; }
         if (p->kin_y) { cudaFree(p->kin_y); p->kin_y = nullptr; }
+        if (p->kin_y2) { cudaFree(p->kin_y2); p->kin_y2 = nullptr; }
     }
     const double invP = 1.0 / ((double)p->nx * (double)p->ny);
     for (int ax = 0; ax < 2; ++ax) {
@@ -199,6 +200,15 @@ template <typename T> gpe_status make_kinetic(gpe_plan *p, double dt, int mode) 
         void **dev = ax == 0 ? &p->kin_x : &p->kin_y;
         gpe_status s = mode == GPE_IMAG_TIME ? upload_real<T>(p, dev, re) : upload_cplx<T>(p, dev, re, im);
         if (s != GPE_OK) return s;
+        if (ax == 1 && mode != GPE_IMAG_TIME) {   // split layout per column pair for the paired pass B (gpe_pair.cuh)
+            std::vector<double> t(4 * (size_t)n);
+            for (int c = 0; c < n / 2; ++c)
+                for (int l = 0; l < 2; ++l) {
+                    const double bx = re[2 * c + l], by = im[2 * c + l];
+                    t[8 * c + l] = 1.0 + bx; t[8 * c + 2 + l] = by; t[8 * c + 4 + l] = bx * invP; t[8 * c + 6 + l] = by * invP;
+                }
+            if ((s = upload_real<T>(p, &p->kin_y2, t)) != GPE_OK) return s;
+        }
     }
     p->kin_mode = mode;
     p->kin_dt = dt;
@@ -405,6 +415,7 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     a.ytab2 = (const T *)p->ytab2;
     a.kin_xc = (const cx<T> *)p->kin_x; a.kin_yc = (const cx<T> *)p->kin_y;
     a.kin_xr = (const T *)p->kin_x; a.kin_yr = (const T *)p->kin_y;
+    a.kin_y2 = (const T *)p->kin_y2;
     a.inv_p = (T)(1.0 / ((double)p->nx * (double)p->ny));
     FinalizeParams &f = a.fin;
     f.partials_b = p->partials_b; f.cav_u0 = p->d_u0;
@@ -764,7 +775,7 @@ gpe_status gpe_plan_destroy(gpe_plan *p) {
     cudaStreamSynchronize(p->stream);
     if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
-    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
+    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->kin_y2, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
                     p->ytab, p->g, p->v2d, p->st, p->partials, p->partials_b, p->d_u0, p->counters, p->nonfinite, p->d_sched_step,
                     p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->d_probe_omega, p->d_probe_delta,
                     p->d_probe_phi, p->scratch, p->obs_dev,

@@ -299,11 +299,10 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / Col
     } else {
         // kinetic factor (1+a)(1+b)/P applied as v/P + v*g, g = a' + b' + a'b (k_col of
         // gpe_kernels.cuh); b differs between the two columns (lanes), a is common to both
-        const float4 bq4 = *reinterpret_cast<const float4 *>(a.kin_yc + 2 * cp);
-        const float2 bqx = make_float2(bq4.x, bq4.z), bqy = make_float2(bq4.y, bq4.w);
+        // (kin_y2: the per-column constants in split lane layout, so no register shuffling is needed)
+        const float4 k0 = ldtw(reinterpret_cast<const float4 *>(a.kin_y2), 2 * cp), k1 = ldtw(reinterpret_cast<const float4 *>(a.kin_y2), 2 * cp + 1);
+        const float2 cb = make_float2(k0.x, k0.y), bqy = make_float2(k0.z, k0.w), bpx = make_float2(k1.x, k1.y), bpy = make_float2(k1.z, k1.w);
         const float invp = a.inv_p;
-        const float2 cb = radd(bqx, make_float2(1.f, 1.f));
-        const float2 bpx = rmuls(bqx, invp), bpy = rmuls(bqy, invp);
 #pragma unroll
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll

@@ -93,6 +93,7 @@ template <typename T, typename C> struct StepArgs {
     const C *tw_hy, *tw1_hy;       // the same two tables for length ny/2 (paired row passes, gpe_pair.cuh)
     const T *ytab2;                // [ny/2][8] = {vy[n], vy[n+ny/2], lat[n], lat[n+ny/2], cav[n], cav[n+ny/2], 0, 0}
     const C *kin_xc, *kin_yc;      // real time: (exp(-i kx^2 dt/2) - 1)/(nx ny), exp(-i ky^2 dt/2) - 1
+    const T *kin_y2;               // real time, paired column pass: per column pair {1+bx0, 1+bx1, by0, by1, bx0/P, bx1/P, by0/P, by1/P}, b = exp(-i ky^2 dt/2) - 1
     T inv_p;                       // 1/(nx ny)
     const T *kin_xr, *kin_yr;      // imaginary time: exp(-kx^2 dt/2)/(nx ny), exp(-ky^2 dt/2)
     FinalizeParams fin;
