@@ -1,7 +1,8 @@
 // gpe_pair.cuh -- the complex64 hot path: the three passes of gpe_kernels.cuh with every
 // thread working on TWO complex numbers in lock step (element type cpair of gpe_fft.cuh), so that
-// all butterfly and twiddle arithmetic is packed fp32x2 (FADD2 / FMUL2 / FFMA2 of sm_100) and
-// every shared-memory exchange and every access to the intermediate array is 128 bits wide.
+// all butterfly and twiddle arithmetic is packed fp32x2 (FADD2 / FMUL2 / FFMA2 of sm_100), the
+// shared-memory exchange moves whole lane pairs (two 64-bit planes) and every access to the
+// intermediate array is 128 or 256 bits wide.
 //
 //   pass B (columns): the two lanes are two ADJACENT COLUMNS (two independent transforms).
 //   pass A (rows):    the two lanes are the even and the odd half of ONE row transform: a
@@ -30,13 +31,13 @@
 #define GPE_ROWP_THREADS 64    // measured: 64 / 128 beat 128 / 256 below 2048 (more, smaller CTAs fill the 148 SMs)
 #endif
 #ifndef GPE_ROWP_MINB
-#define GPE_ROWP_MINB 4
+#define GPE_ROWP_MINB 4         // 128-thread row CTAs per SM the row passes are compiled for (3 and 5 measured slower)
 #endif
 #ifndef GPE_COLP_RESIDENT
 #define GPE_COLP_RESIDENT 512   // threads per SM the column pass is compiled for (128 registers each)
 #endif
 #ifndef GPE_COLP_THREADS
-#define GPE_COLP_THREADS 128
+#define GPE_COLP_THREADS 128   // threads per column CTA where the transform allows (2048: 256 = two column pairs)
 #endif
 
 namespace gpe {
@@ -45,7 +46,7 @@ template <int N> struct RowGeomP {
     static constexpr int H = N / 2;
     static constexpr int TPF = H / 16;                               // threads per row
     static constexpr int RPC = (GPE_ROWP_THREADS / TPF) < 2 ? 2 : (GPE_ROWP_THREADS / TPF);    // rows per CTA (>= one row pair)
-    static constexpr int THREADS = RPC * TPF;                        // 128
+    static constexpr int THREADS = RPC * TPF;                        // 128 at 2048, 64 below
     static constexpr bool NAMED = RPC > 1 && TPF % 32 == 0;          // rows own whole warps
     // outer stage pair-mapped (Fft1D::last_fwd_pair): a thread holds the same output indices of rows
     // 2m and 2m+1, i.e. 32 contiguous bytes of the row-pair-interleaved intermediate array
