@@ -117,6 +117,9 @@ typedef struct {
      * by Delta - N_at U_0 B_n, B_n = sum cos^2(k_c x)|psi_n|^2 dx dy (a third fused reduction).
      * NULL = the three-term model.  Needs cavity_on. */
     const double *cav_u0;      /* HOST [batch]                                                    */
+    /* 1: the schedule amplitude of step n is sampled at the middle of the step, A(n + 1/2), instead
+     * of its start A(n) (reading Q4); records and observables report the same sample. */
+    int sched_midpoint;
 } gpe_potential_desc;
 
 /*

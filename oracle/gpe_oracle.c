@@ -84,6 +84,9 @@ typedef struct {
     const double *probe_phi;   /* [batch] phi */
     /* full cavity model (Eqs. 12 and 15): U_0 per member; NULL = off */
     const double *cav_u0;      /* [batch] */
+    /* 1: the schedule amplitude of step n is sampled at the middle of the step, A((n + 1/2) dt),
+     * instead of its start (reading Q4) */
+    int sched_midpoint;
 } oracle_params;
 
 /* ------------------------------------------------------------------ FFT */
@@ -333,7 +336,7 @@ int oracle_evolve(const oracle_params *P, cplx_t *psi, double dt, long n_steps, 
         long n = step0 + s;
         for (int b = 0; b < P->batch; ++b) {
             cplx_t *w = psi + (size_t)b * npts;
-            double A = oracle_schedule(P, b, (double)n);
+            double A = oracle_schedule(P, b, (double)n + (P->sched_midpoint ? 0.5 : 0.0));
             double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
             double bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
             double eta, C, Dc; double _Complex alpha;
@@ -350,7 +353,7 @@ int oracle_evolve(const oracle_params *P, cplx_t *psi, double dt, long n_steps, 
         if (records && record_every > 0 && ((n + 1) % record_every) == 0) {
             for (int b = 0; b < P->batch; ++b) {
                 cplx_t *w = psi + (size_t)b * npts;
-                double A = oracle_schedule(P, b, (double)(n + 1));
+                double A = oracle_schedule(P, b, (double)(n + 1) + (P->sched_midpoint ? 0.5 : 0.0));
                 double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
                 double bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
                 double eta, C, Dc; double _Complex alpha;
@@ -378,7 +381,7 @@ int oracle_observables(const oracle_params *P, const cplx_t *psi, long n, double
     axis_tables T = make_tables(P);
     for (int b = 0; b < P->batch; ++b) {
         const cplx_t *w = psi + (size_t)b * npts;
-        double A = oracle_schedule(P, b, (double)n);
+        double A = oracle_schedule(P, b, (double)n + (P->sched_midpoint ? 0.5 : 0.0));
         double g = P->g ? P->g[b] : 0.0;
         double norm = sum_norm(P, w);
         double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
@@ -465,7 +468,7 @@ int oracle_potential_half_step(const oracle_params *P, cplx_t *psi, double dt, i
     axis_tables T = make_tables(P);
     for (int b = 0; b < P->batch; ++b) {
         cplx_t *w = psi + (size_t)b * npts;
-        double A = oracle_schedule(P, b, (double)n);
+        double A = oracle_schedule(P, b, (double)n + (P->sched_midpoint ? 0.5 : 0.0));
         double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
         double bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
         double eta, C, Dc; double _Complex alpha;

@@ -34,6 +34,7 @@ class gpe_potential_desc(C.Structure):
         ("kappa", C.c_void_p),
         ("probe_omega", C.c_void_p), ("probe_delta", C.c_void_p), ("probe_phi", C.c_void_p),
         ("cav_u0", C.c_void_p),
+        ("sched_midpoint", C.c_int),
     ]
 
 
@@ -242,6 +243,7 @@ class Plan:
                 setattr(d, name, hp(a, B))
         if p.get("cav_u0") is not None:
             d.cav_u0 = hp(np.broadcast_to(np.asarray(p["cav_u0"], dtype=np.float64), (B,)), B)
+        d.sched_midpoint = int(p.get("sched_midpoint", 0))
         gpe_set_potential(self.plan, d)
         torch.cuda.current_stream().synchronize()
         self._keep = keep

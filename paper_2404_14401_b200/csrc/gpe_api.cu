@@ -64,7 +64,7 @@ struct gpe_plan {
     double *d_probe_omega = nullptr, *d_probe_delta = nullptr, *d_probe_phi = nullptr;   // nullptr = no probe
 
     // host copies of the descriptor
-    int lattice_axis = -1, sched_len = 0, sched_batched = 0, cavity_on = 0, eta_mode = 0;
+    int lattice_axis = -1, sched_len = 0, sched_batched = 0, cavity_on = 0, eta_mode = 0, sched_midpoint = 0;
     double lattice_k = 0, cavity_k = 0;
     std::vector<double> h_sched_step, h_sched_amp, h_eta, h_natoms, h_delta, h_kappa, h_g;
 
@@ -422,6 +422,7 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     f.st = p->st; f.partials = p->partials; f.counters = p->counters; f.nonfinite = p->nonfinite;
     f.sched_len = p->sched_len; f.sched_step = p->d_sched_step; f.sched_amp = p->d_sched_amp;
     f.sched_batched = p->sched_batched;
+    f.sched_mid = p->sched_midpoint ? 0.5 : 0.0;
     f.cavity_on = p->cavity_on; f.eta_mode = p->eta_mode;
     f.eta_or_u = p->d_eta; f.n_atoms = p->d_natoms; f.delta = p->d_delta; f.kappa = p->d_kappa;
     f.probe_omega = p->d_probe_omega; f.probe_delta = p->d_probe_delta; f.probe_phi = p->d_probe_phi;
@@ -580,7 +581,7 @@ gpe_status observables_impl(gpe_plan *p, const void *psi, gpe_obs *out, void *de
     if (!p->obs_dev) GPE_CUDA(p, cudaMalloc((void **)&p->obs_dev, sizeof(double) * 8 * B));
     if (!p->obsA_dev) GPE_CUDA(p, cudaMalloc((void **)&p->obsA_dev, sizeof(double) * B));
     std::vector<double> A(B);
-    for (int b = 0; b < B; ++b) A[b] = host_schedule(p, b, (double)p->step);
+    for (int b = 0; b < B; ++b) A[b] = host_schedule(p, b, (double)p->step + (p->sched_midpoint ? 0.5 : 0.0));
     GPE_CUDA(p, cudaMemcpyAsync(p->obsA_dev, A.data(), sizeof(double) * B, cudaMemcpyHostToDevice, p->stream));
     GPE_CUDA(p, cudaMemsetAsync(p->obs_dev, 0, sizeof(double) * 8 * B, p->stream));
     dim3 grid(p->nx < 256 ? p->nx : 256, B);
@@ -812,6 +813,7 @@ gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
     p->lattice_axis = d->lattice_axis; p->lattice_k = d->lattice_k;
     p->sched_len = d->sched_len; p->sched_batched = d->sched_len > 0 ? (d->sched_batched ? 1 : 0) : 0;
     p->cavity_on = d->cavity_on ? 1 : 0; p->cavity_k = d->cavity_k; p->eta_mode = d->eta_mode;
+    p->sched_midpoint = d->sched_midpoint ? 1 : 0;
     p->h_sched_step.clear(); p->h_sched_amp.clear();
     if (d->sched_len > 0) {
         p->h_sched_step.assign(d->sched_step, d->sched_step + d->sched_len);

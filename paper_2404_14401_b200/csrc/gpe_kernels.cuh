@@ -73,7 +73,7 @@ __device__ inline double schedule_at(const FinalizeParams &f, int b, double n) {
 // bunch = int cos^2(k_c x)|psi|^2 (full cavity model: Delta -> Delta - N U0 bunch, Eq. 15).
 __device__ inline void step_coefficients(const FinalizeParams &f, int b, long long n, double bunch, double &A, double &kre, double &kim,
                                          double &kc, double &pre, double &pim, double &pc) {
-    A = schedule_at(f, b, (double)n);
+    A = schedule_at(f, b, (double)n + f.sched_mid);
     kre = kim = kc = pre = pim = pc = 0.0;
     if (f.cavity_on) {
         const double eta = f.eta_mode == 0 ? f.eta_or_u[b] : sqrt(fabs(A) * f.eta_or_u[b]);

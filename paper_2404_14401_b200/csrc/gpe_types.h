@@ -47,6 +47,7 @@ struct FinalizeParams {
     const double *sched_step; // [sched_len]
     const double *sched_amp;  // [sched_len] or [batch][sched_len]
     int sched_batched;
+    double sched_mid;         // 0, or 0.5: sample the schedule at the middle of the step
     int cavity_on, eta_mode;
     const double *eta_or_u, *n_atoms, *delta, *kappa;  // [batch]
     const double *probe_omega, *probe_delta, *probe_phi;  // [batch] or nullptr (Eq. 17)

@@ -371,6 +371,27 @@ def test_full_cavity_model_parity(nx, ny, mode, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_schedule_midpoint_parity(dtype):
+    """sched_midpoint: A_n = A(n + 1/2) on the device as in the oracle (psi, the recorded A and the
+    observables' e_pot, which uses the same sample)."""
+    p = _general_workload(128, 256)
+    p["sched_midpoint"] = 1
+    plan = _gpu_plan(p, dtype)
+    psi = _to_dev(p["psi0"], dtype)
+    ref = _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    rg = plan.evolve(psi, 1e-3, 12, "real", record_every=1).cpu().numpy()
+    ro = o.evolve(ref, 1e-3, 12, False, record_every=1)
+    assert _rel(psi.cpu().numpy(), ref) <= 12 * PER_STEP[dtype]
+    assert np.allclose(rg[:, 0, 5], ro[:, 0, 5], rtol=1e-14)
+    assert not np.allclose(ro[:, 0, 5], [W_ for W_ in Oracle({**p, "sched_midpoint": 0}).evolve(
+        _oracle_input(p["psi0"], dtype), 1e-3, 12, False, record_every=1)[:, 0, 5]])
+    eg, eo = plan.observables(psi)[0][0]["e_pot"], o.observables(ref)[0][0]["e_pot"]
+    assert abs(eg - eo) <= (1e-5 if dtype == "c64" else 1e-10) * abs(eo)
+    plan.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
 def test_probe_parity_and_records(dtype):
     """On-axis cavity probe (Eq. 17): psi and the recorded cavity field against
     the oracle over two gpe_evolve calls (the probe's time origin is the plan's step counter),

@@ -503,6 +503,34 @@ def test_full_cavity_model_closed_forms():
     assert np.linalg.norm(a - b) > 1e-6          # and U0 does act
 
 
+def test_schedule_midpoint_sampling_is_exact_for_a_linear_ramp():
+    """sched_midpoint (reading Q4).  A uniform state under a lattice whose amplitude
+    ramps linearly in time: over a short run the kinetic term mixes the imprinted grating only at
+    O(k^2 t) of an already small phase, so the accumulated phase is -cos^2(kx) int A dt.  Sampling
+    at the middle of each step gives that integral exactly, sampling at the start misses
+    (A(T) - A(0)) dt / 2: pins the +1/2 and that nothing else moved."""
+    L, n, k = 4 * math.pi, 64, 0.5          # k small: the kinetic mixing of the imprinted grating is O(k^2 t phase)
+    p = W._base(n, n, L)
+    p["lattice_axis"], p["lattice_k"] = 0, k
+    nst, dt = 10, 1e-5
+    p["sched_step"], p["sched_amp"] = np.array([0.0, float(nst)]), np.array([2.0, 12.0])
+    x = W.axis(n, L)
+    c2 = (np.cos(k * x) ** 2)[:, None] * np.ones((1, n))
+    out = {}
+    for mid in (0, 1):
+        q = dict(p); q["sched_midpoint"] = mid
+        psi = np.full((n, n), 1.0 / L, dtype=np.complex128)
+        rec = Oracle(q).evolve(psi, dt, nst, False, record_every=1)
+        out[mid] = (np.angle(psi * L), rec[:, 0, 5])
+    integral = 0.5 * (2.0 + 12.0) * nst * dt
+    assert np.allclose(out[1][0], -c2 * integral, rtol=0, atol=2e-9)
+    assert np.allclose(out[0][0], -c2 * (integral - 0.5 * (12.0 - 2.0) * dt), rtol=0, atol=2e-9)
+    assert np.max(np.abs(out[1][0] - out[0][0])) > 1e-5 * 0.9 * 5.0          # the two differ by 5 dt cos^2
+    # records report the sample of the upcoming step: A(n + 1/2) against A(n), clamped after the last knot
+    assert np.allclose(out[1][1][:-1], 2.0 + (np.arange(1, nst) + 0.5))
+    assert np.allclose(out[0][1], 2.0 + np.arange(1, nst + 1))
+
+
 def test_interactions_raise_threshold():
     """repulsive interactions increase the critical pump."""
     thetas = {}
