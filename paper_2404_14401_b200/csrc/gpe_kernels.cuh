@@ -369,32 +369,6 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
     }
 }
 
-// ---------------------------------------------------------------- row staging (passes A and C)
-// The row passes are persistent: a CTA walks over groups of RPC rows (group g, g + gridDim.x, ...)
-// and fetches the NEXT group into a shared-memory stage with cp.async (16-byte chunks, L1
-// bypassed) while it computes the current one, so the L2 latency of the row loads -- half of
-// every warp's lifetime in the first version (profiles/r01_baseline.md) -- is off the critical
-// path.  STAGED = false keeps the direct register loads (complex128: the stage would halve the
-// occupancy of an ALU-bound kernel).
-#ifndef GPE_ROW_STAGE
-#define GPE_ROW_STAGE 0
-#endif
-template <typename T> struct RowStage { static constexpr bool on = GPE_ROW_STAGE && sizeof(T) == 4; };
-
-__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-
-// copies the `bytes` (multiple of 16) at gsrc into the stage, all threads of the CTA
-__device__ __forceinline__ void stage_fetch(unsigned char *stage, const void *gsrc, int bytes) {
-    const unsigned char *g = reinterpret_cast<const unsigned char *>(gsrc);
-    for (int q = threadIdx.x * 16; q < bytes; q += blockDim.x * 16) cp_async16(stage + q, g + q);
-    cp_async_commit();
-}
-
 // ---------------------------------------------------------------- pass A
 // complex128 rows: two 256-thread CTAs per SM (128 registers) from 512 points up -- measured on B200:
 // 2048^2 real time 185 -> 157 us per step, 1024^2 53 -> 45; below 512 one CTA with all registers wins.
@@ -403,35 +377,21 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
-    constexpr bool STAGED = RowStage<T>::on;
-    constexpr int GROUP_BYTES = (int)sizeof(C) * G::RPC * NY;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
-    unsigned char *stage = smem_raw + sizeof(C) * G::RPC * F::SLOTS;
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     C *sm = smem + r * F::SLOTS;
-    const long ngroups = (long)a.batch * a.nx / G::RPC;
     pdl_launch_dependents();
     pdl_wait();
-    if (STAGED && (long)blockIdx.x < ngroups) stage_fetch(stage, a.src + (long)blockIdx.x * G::RPC * NY, GROUP_BYTES);
-    for (long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    {   // one group of RPC rows per CTA
+        const long grp = blockIdx.x;
         const long row = grp * G::RPC + r;
         const int b = (int)(row / a.nx), i = (int)(row % a.nx);
         C *dst = a.dst + row * NY;
         C v[16];
-        if constexpr (STAGED) {
-            cp_async_wait_all();
-            __syncthreads();
-            const C *st_row = reinterpret_cast<const C *>(stage) + r * NY;
+        const C *src = a.src + row * NY;
 #pragma unroll
-            for (int k = 0; k < 16; ++k) v[k] = st_row[j + F::M1 * k];
-            __syncthreads();
-            if (grp + gridDim.x < ngroups) stage_fetch(stage, a.src + (grp + gridDim.x) * G::RPC * NY, GROUP_BYTES);
-        } else {
-            const C *src = a.src + row * NY;
-#pragma unroll
-            for (int k = 0; k < 16; ++k) v[k] = __ldcg(src + j + F::M1 * k);
-        }
+        for (int k = 0; k < 16; ++k) v[k] = __ldcg(src + j + F::M1 * k);
         if (!(a.flags & F_NO_POT)) {
             const MemberState &ms = a.fin.st[b];
             T sn, st;
@@ -447,7 +407,6 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
 #pragma unroll
             for (int rr = 0; rr < F::RL; ++rr) dst[F::nat(j, ii, rr)] = v[ii * F::RL + rr];
         }
-        if constexpr (!STAGED) __syncthreads();
     }
 }
 
@@ -524,41 +483,25 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
-    constexpr bool STAGED = RowStage<T>::on;
-    constexpr int GROUP_BYTES = (int)sizeof(C) * G::RPC * NY;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
-    unsigned char *stage = smem_raw + sizeof(C) * G::RPC * F::SLOTS;
     __shared__ double red[96];
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     C *sm = smem + r * F::SLOTS;
-    const long ngroups = (long)a.batch * a.nx / G::RPC;
     const int gpm = a.nx / G::RPC;  // groups per member: all rows of a group belong to one member
     pdl_launch_dependents();
     pdl_wait();
-    if (STAGED && (long)blockIdx.x < ngroups) stage_fetch(stage, a.src + (long)blockIdx.x * G::RPC * NY, GROUP_BYTES);
-    for (long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    {   // one group of RPC rows per CTA
+        const long grp = blockIdx.x;
         const long row = grp * G::RPC + r;
         const int b = (int)(row / a.nx), i = (int)(row % a.nx);
         C *dst = a.dst + row * NY;
         C v[16];
-        if constexpr (STAGED) {
-            cp_async_wait_all();
-            __syncthreads();
-            const C *st_row = reinterpret_cast<const C *>(stage) + r * NY;
+        const C *src = a.src + row * NY;
 #pragma unroll
-            for (int ii = 0; ii < F::GL; ++ii)
+        for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
-                for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = st_row[F::nat(j, ii, rr)];
-            __syncthreads();
-            if (grp + gridDim.x < ngroups) stage_fetch(stage, a.src + (grp + gridDim.x) * G::RPC * NY, GROUP_BYTES);
-        } else {
-            const C *src = a.src + row * NY;
-#pragma unroll
-            for (int ii = 0; ii < F::GL; ++ii)
-#pragma unroll
-                for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = __ldcg(src + F::nat(j, ii, rr));
-        }
+            for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = __ldcg(src + F::nat(j, ii, rr));
         F::inv(v, sm, j, a.tw_y, a.tw1_y);
         const MemberState &ms = a.fin.st[b];
         T sn, st;
@@ -577,7 +520,6 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
         double dn = (double)sn, dt_ = (a.flags & F_CAVITY) ? (double)st * (double)a.cavx[i] : 0.0;
         const double db_ = (a.flags & F_CAV_FULL) ? dn * ((double)a.cavx[i] * (double)a.cavx[i]) : 0.0;
         block_reduce_and_finalize(a.fin, b, (int)(grp % gpm), dn, dt_, db_, red);
-        if constexpr (!STAGED) __syncthreads();
     }
 }
 
@@ -586,20 +528,12 @@ template <typename T, int N> struct Launch {
     using C = cx<T>;
     using A = StepArgs<T, C>;
     static size_t row_smem() {
-        return sizeof(C) * RowGeom<N>::RPC * Fft1D<N, 1, cx<T>>::SLOTS + (RowStage<T>::on ? sizeof(C) * RowGeom<N>::RPC * N : 0);
+        return sizeof(C) * RowGeom<N>::RPC * Fft1D<N, 1, cx<T>>::SLOTS;
     }
     // Measured on B200: overlapping the next pass's launch with the tail of
     // the current one pays for launch-bound grids (<= 256^2 points) and costs 1-4 us per step above.
     static bool use_pdl(const A &a) { return (long)a.batch * a.nx * a.ny <= 65536L; }
-    // persistent when staged: GPE_ROW_MINB CTAs per SM walk over the row groups
-    static unsigned row_grid(const A &a) {
-        long groups = (long)a.batch * a.nx / RowGeom<N>::RPC;
-        if (!RowStage<T>::on) return (unsigned)groups;
-        static int sms = 0;
-        if (!sms) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev); if (sms <= 0) sms = 148; }
-        long cap = (long)sms * GPE_ROW_MINB;
-        return (unsigned)(groups < cap ? groups : cap);
-    }
+    static unsigned row_grid(const A &a) { return (unsigned)((long)a.batch * a.nx / RowGeom<N>::RPC); }
     static size_t col_smem() { return sizeof(C) * ColGeom<T, N>::W * Fft1D<N, 1, cx<T>>::SLOTS; }
 
     // opt in to > 48 KB of dynamic shared memory once per kernel (not on every launch: the
