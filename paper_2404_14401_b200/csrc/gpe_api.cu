@@ -440,6 +440,8 @@ struct PassProfile {
     std::vector<int> which;
 };
 
+gpe_status ensure_scratch(gpe_plan *p);
+
 template <typename T>
 gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode mode, long record_every,
                        double *records, PassProfile *prof = nullptr) {
@@ -474,15 +476,22 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     // by exp(-i (V_n + V_{n+1} + 2 g |psi|^2) dt/2) instead of two; |psi|^2, hence Theta, is unchanged)
     a.fin.merged = (!imag && !getenv("GPE_NO_MERGE")) ? 1 : 0;
     a.fin.record_every = 0; a.fin.rec_first = 0; a.fin.records = nullptr;  // step kernels read *call
+    // four-row-interleaved intermediate array (gpe_types.h): psi -> scratch -> scratch -> psi
+    const bool oop = paired && p->nx >= GPE_IL4_MIN_N && p->ny >= GPE_IL4_MIN_N && p->batch == 1;
+    if (oop && (s = ensure_scratch(p)) != GPE_OK) return s;
     auto one_step = [&](cudaStream_t st, int w, cudaEvent_t e0, cudaEvent_t e1) -> gpe_status {
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, st));
+        if (oop) a.dst = (cx<T> *)p->scratch;
         GPE_CUDA(p, paired ? oy->p_row_fwd(a, imag, st) : oy->row_fwd(a, imag, st));
+        if (oop) a.src = (const cx<T> *)p->scratch;
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e1, st));
         if (w == 1) GPE_CUDA(p, cudaEventRecord(e0, st));
         GPE_CUDA(p, paired ? ox->p_col(a, imag, st) : ox->col(a, imag, 0, st));
         if (w == 1) GPE_CUDA(p, cudaEventRecord(e1, st));
         if (w == 2) GPE_CUDA(p, cudaEventRecord(e0, st));
+        if (oop) a.dst = (cx<T> *)psi;
         GPE_CUDA(p, paired ? oy->p_row_inv(a, imag, st) : oy->row_inv(a, imag, st));
+        if (oop) a.src = (const cx<T> *)psi;
         if (w == 2) GPE_CUDA(p, cudaEventRecord(e1, st));
         return GPE_OK;
     };

@@ -142,6 +142,34 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
+// Last CTA of member b: thread t adds partials t, t + blockDim.x, ... in that order.  The loads go out
+// four at a time (ld.global.cg: L2, where the other CTAs' partials are after their fence) -- one
+// dependent L2 round trip per partial, as a volatile loop does, left a 3 us serial tail after pass C
+// at 2048^2 (1024 partials, 8 per thread) and 10 us in complex128 (32 per lane of one warp).
+__device__ __forceinline__ void sum_partials(const FinalizeParams &f, int b, double &s0, double &s1, double &s2) {
+    __threadfence();
+    const double2 *pp = f.partials + (size_t)b * f.cpm;
+    const int nt = blockDim.x;
+    s0 = 0.0; s1 = 0.0; s2 = 0.0;
+    for (int q0 = threadIdx.x; q0 < f.cpm; q0 += 4 * nt) {
+        double2 t[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { const int q = q0 + k * nt; t[k] = q < f.cpm ? __ldcg(pp + q) : make_double2(0.0, 0.0); }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { s0 += t[k].x; s1 += t[k].y; }
+    }
+    if (f.cav_u0) {
+        const double *pb = f.partials_b + (size_t)b * f.cpm;
+        for (int q0 = threadIdx.x; q0 < f.cpm; q0 += 4 * nt) {
+            double u[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { const int q = q0 + k * nt; u[k] = q < f.cpm ? __ldcg(pb + q) : 0.0; }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) s2 += u[k];
+        }
+    }
+}
+
 // Block-level sum of (sn, st), one partial per CTA, last CTA of the member finalises.
 // `red` is shared scratch of at least 2*32 doubles.  All threads of the CTA must call this.
 __device__ inline void block_reduce_and_finalize(const FinalizeParams &f, int b, int cta_in_member,
@@ -163,20 +191,17 @@ __device__ inline void block_reduce_and_finalize(const FinalizeParams &f, int b,
         is_last = (old == (unsigned int)(f.cpm - 1));
     }
     __syncthreads();
-    if (is_last && w == 0) {
-        __threadfence();
-        const volatile double2 *p = f.partials + (size_t)b * f.cpm;
-        double a = 0.0, c = 0.0, e = 0.0;
-        for (int i = lane; i < f.cpm; i += 32) { a += p[i].x; c += p[i].y; }
-        if (f.cav_u0) {
-            const volatile double *pb = f.partials_b + (size_t)b * f.cpm;
-            for (int i = lane; i < f.cpm; i += 32) e += pb[i];
-            e = warp_sum(e);
-        }
-        a = warp_sum(a);
-        c = warp_sum(c);
-        if (lane == 0) {
-            finalize_member(f, b, a, c, e);
+    if (is_last) {   // uniform over the CTA: all its threads sum the partials of the member
+        double a, c, e;
+        sum_partials(f, b, a, c, e);
+        a = warp_sum(a); c = warp_sum(c); e = warp_sum(e);
+        __syncthreads();
+        if (lane == 0) { red[w] = a; red[32 + w] = c; red[64 + w] = e; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+            for (int i = 0; i < nw; ++i) { t0 += red[i]; t1 += red[32 + i]; t2 += red[64 + i]; }
+            finalize_member(f, b, t0, t1, t2);
             f.counters[b] = 0u;
         }
     }

@@ -56,10 +56,32 @@ template <int N> struct RowGeomP {
 template <int N> struct ColGeomP {
     static constexpr int TPF = N / 16;                               // threads per column pair
     static constexpr int CPW0 = GPE_COLP_THREADS / TPF;
-    static constexpr int CPW = CPW0 < 2 ? 2 : CPW0;                  // column pairs per CTA
+    // column pairs per CTA; 2048: ONE (128 threads, 1024 CTAs: 6.92 per SM, at most 7 -- two pairs per
+    // CTA gave 512 CTAs, 3 on 80 SMs and 4 on 68, and the pass waited for the 68: 27.4 against 21 us)
+    static constexpr int CPW = CPW0 < 2 ? (N >= GPE_IL4_MIN_N ? 1 : 2) : CPW0;
     static constexpr int THREADS = CPW * TPF;
 };
 
+#ifdef GPE_TRACE
+struct TraceScope {
+    unsigned long long *slot, t0;
+    __device__ TraceScope(unsigned long long *base, int pass) {
+        slot = nullptr;
+        if (base && threadIdx.x == 0) {
+            slot = base + ((size_t)pass * 4096 + blockIdx.x + gridDim.x * blockIdx.y) * 4;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+        }
+    }
+    __device__ void mark(int k) { if (slot) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); slot[k] = t; } }
+    __device__ ~TraceScope() {
+        if (slot) { unsigned long long t1; unsigned sm; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+                    slot[0] = sm; slot[1] = t0; slot[3] = t1; }
+    }
+};
+#define GPE_TRACE_SCOPE(pass) TraceScope trace_scope(a.trace, pass)
+#else
+#define GPE_TRACE_SCOPE(pass)
+#endif
 __device__ __forceinline__ void bar_named(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -83,7 +105,11 @@ __device__ __forceinline__ void ldcg_pair2(const cpair *p, cpair &v0, cpair &v1)
 
 // position of element (row i, column pair kp) of the intermediate array, hy = ny/2 (rows counted
 // through the whole batch: nx is even, so a row pair never straddles two members)
-__device__ __forceinline__ size_t ipos(long i, int kp, size_t hy) { return ((size_t)(i >> 1) * hy + kp) * 2 + (i & 1); }
+// il = log2 of the number of interleaved rows: 1, or 2 when nx and ny >= GPE_IL4_MIN_N (il_of)
+__device__ __forceinline__ size_t ipos(long i, int kp, size_t hy, int il) { return (((size_t)(i >> il) * hy + kp) << il) + (i & ((1 << il) - 1)); }
+// N = the kernel's own compile-time axis length, other = the other one: both must reach GPE_IL4_MIN_N
+// single grids only: the out-of-place passes double the footprint, and two 2048^2 grids no longer fit in L2
+template <int N> __device__ __forceinline__ int il_of(int other, int batch) { return (N >= GPE_IL4_MIN_N && other >= GPE_IL4_MIN_N && batch == 1) ? 2 : 1; }
 
 // Potential half-step (rows a1 / a5) on the 32 points of one thread: p0[k] at y = j + M1 k,
 // p1[k] at y + H, same row i.  ytab2[n] = {vy[n], vy[n+H], cos^2(k_l y_n), cos^2(k_l y_{n+H})},
@@ -198,7 +224,7 @@ __device__ __forceinline__ void reduce_pair16(const float2 (&p0)[16], const floa
 }
 
 // ---------------------------------------------------------------- pass A (rows, forward)
-template <int NY, bool IMAG>
+template <int NY, bool IMAG, bool LATE>
 __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) / RowGeomP<NY>::THREADS) k_row_fwd_p(const StepArgs<float, float2> a) {
     using G = RowGeomP<NY>;
     using F = Fft1D<G::H, 1, cpair>;
@@ -207,10 +233,11 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     float2 *sm = reinterpret_cast<float2 *>(smem_raw) + r * F::TILE;
     const long row = (long)blockIdx.x * G::RPC + r;
-    const int b = (int)(row / a.nx), i = (int)(row % a.nx);
+    const int b = (int)(row / a.nx), i = (int)(row % a.nx), il = il_of<NY>(a.nx, a.batch);
     const float2 *src = a.src + row * NY;
-    pdl_launch_dependents();
+    if constexpr (!LATE) pdl_launch_dependents();
     pdl_wait();
+    GPE_TRACE_SCOPE(0);
     float2 p0[16], p1[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
@@ -248,7 +275,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
         for (int ii = 0; ii < F::GL / 2; ++ii)
 #pragma unroll
             for (int rr = 0; rr < F::RL; ++rr) {
-                const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H);
+                const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H, il);
                 st_pair2(dst + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
             }
     } else {
@@ -259,12 +286,15 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
 #pragma unroll
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
-            for (int rr = 0; rr < F::RL; ++rr) st_pair(dst + ipos(row, F::nat(j, ii, rr), H), v[ii * F::RL + rr]);
+            for (int rr = 0; rr < F::RL; ++rr) st_pair(dst + ipos(row, F::nat(j, ii, rr), H, il), v[ii * F::RL + rr]);
     }
+    // after the CTA's last store, and only when asked for: even without the launch attribute the
+    // instruction is not free after a burst of stores (measured: config 5 +6 us, 16 x 1024^2 +13 us per step)
+    if constexpr (LATE) pdl_launch_dependents();
 }
 
 // ---------------------------------------------------------------- pass B (columns)
-template <int NX, bool IMAG>
+template <int NX, bool IMAG, bool LATE>
 __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / ColGeomP<NX>::THREADS) k_col_p(const StepArgs<float, float2> a) {
     using G = ColGeomP<NX>;
     using F = Fft1D<NX, G::CPW, cpair>;
@@ -274,13 +304,14 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / Col
     const int b = blockIdx.y;
     const size_t hy = a.ny / 2;
     // rows j + M1 k, k = 0..15 (M1 even): ipos(j + M1 k, cp) = ipos(j, cp) + k * M1 * hy
-    const size_t base = (size_t)b * NX * hy + ipos(j, cp, hy), kstr = (size_t)F::M1 * hy;
+    const size_t base = (size_t)b * NX * hy + ipos(j, cp, hy, il_of<NX>(a.ny, a.batch)), kstr = (size_t)F::M1 * hy;
     const cpair *src = reinterpret_cast<const cpair *>(a.src) + base;
     cpair *dst = reinterpret_cast<cpair *>(a.dst) + base;
     float2 *sm = reinterpret_cast<float2 *>(smem_raw) + c;
     cpair v[16];
-    pdl_launch_dependents();
+    if constexpr (!LATE) pdl_launch_dependents();
     pdl_wait();
+    GPE_TRACE_SCOPE(1);
     if (blockIdx.x == 0 && threadIdx.x == 0 && a.fin.prepared) prepare_member(a.fin, b);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
@@ -322,10 +353,11 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / Col
     for (int k = 0; k < 16; ++k) {
         st_pair(dst + k * kstr, v[k]);
     }
+    if constexpr (LATE) pdl_launch_dependents();
 }
 
 // ---------------------------------------------------------------- pass C (rows, inverse)
-template <int NY, bool IMAG, bool MERGED>
+template <int NY, bool IMAG, bool MERGED, bool LATE>
 __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) / RowGeomP<NY>::THREADS) k_row_inv_p(const StepArgs<float, float2> a) {
     using G = RowGeomP<NY>;
     using F = Fft1D<G::H, 1, cpair>;
@@ -335,11 +367,12 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     float2 *sm = reinterpret_cast<float2 *>(smem_raw) + r * F::TILE;
     const long row = (long)blockIdx.x * G::RPC + r;
-    const int b = (int)(row / a.nx), i = (int)(row % a.nx);
+    const int b = (int)(row / a.nx), i = (int)(row % a.nx), il = il_of<NY>(a.nx, a.batch);
     const int gpm = a.nx / G::RPC;
     const cpair *src = reinterpret_cast<const cpair *>(a.src);
-    pdl_launch_dependents();
+    if constexpr (!LATE) pdl_launch_dependents();
     pdl_wait();
+    GPE_TRACE_SCOPE(2);
     cpair v[16];
     if constexpr (G::PAIRMAP) {
         // mirror of pass A: 32 contiguous bytes (rows 2m, 2m+1, same column pair) per thread and index
@@ -350,7 +383,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
         for (int ii = 0; ii < F::GL / 2; ++ii)
 #pragma unroll
             for (int rr = 0; rr < F::RL; ++rr) {
-                const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H);
+                const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H, il);
                 ldcg_pair2(src + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
             }
         auto sync_row = [r] { if constexpr (G::NAMED) bar_named(1 + r, G::TPF); else __syncthreads(); };
@@ -361,7 +394,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
             for (int rr = 0; rr < F::RL; ++rr) {
-                v[ii * F::RL + rr] = ldcg_pair(src + ipos(row, F::nat(j, ii, rr), H));
+                v[ii * F::RL + rr] = ldcg_pair(src + ipos(row, F::nat(j, ii, rr), H, il));
             }
         if constexpr (G::NAMED) F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
         else F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
@@ -409,6 +442,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     }
 #pragma unroll
     for (int k = 0; k < 16; ++k) { dst[j + M1 * k] = p0[k]; dst[H + j + M1 * k] = p1[k]; }
+    if constexpr (LATE) pdl_launch_dependents();
     if (threadIdx.x == 0) is_last = (old == (unsigned int)(f.cpm - 1));
     __syncthreads();
     if (is_last) {   // the last CTA of the member: all its threads sum the partials
@@ -444,24 +478,48 @@ template <int N> struct LaunchP {
         static const long lim = getenv("GPE_PDL_MAX_POINTS") ? atol(getenv("GPE_PDL_MAX_POINTS")) : 65536L;   // tuning knob
         return (long)a.batch * a.nx * a.ny <= lim;
     }
+    // Where a pass releases its dependent launch (programmatic dependent launch, gpe_kernels.cuh):
+    // at the top for launch-bound grids (<= 256^2 points), after its last store -- a compile-time
+    // variant, LATE -- for single grids of a wave or two (measured on B200, us per step: 512^2 17.4 -> 16.3,
+    // 1024^2 23.0 -> 22.1, 2048^2 57.2 -> 56.4; released at the top these sizes lose 4-5 us), and not at
+    // all for batches of many waves.  The instruction after the stores is not free even when predicated
+    // off at run time (config 5: +6 us per step), hence the template parameter.
+    static bool late(const A &a) {
+        static const long lo = getenv("GPE_PDL_LATE_MIN_POINTS") ? atol(getenv("GPE_PDL_LATE_MIN_POINTS")) : 65537L;   // tuning knobs
+        static const long hi = getenv("GPE_PDL_LATE_MAX_POINTS") ? atol(getenv("GPE_PDL_LATE_MAX_POINTS")) : (1L << 23) - 1;
+        const long pts = (long)a.batch * a.nx * a.ny;
+        return pts >= lo && pts <= hi;
+    }
     template <typename K> static cudaError_t go(K kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, const A &a) {
         cudaError_t e = Launch<float, N>::prep(kern, smem);
         if (e != cudaSuccess) return e;
-        e = launch_pdl(kern, grid, block, smem, s, use_pdl(a), a);
+#ifdef GPE_TRACE
+        A a2 = a;
+        a2.trace = getenv("GPE_TRACE_PTR") ? (unsigned long long *)strtoull(getenv("GPE_TRACE_PTR"), nullptr, 0) : nullptr;
+        e = launch_pdl(kern, grid, block, smem, s, use_pdl(a) || late(a), a2);
+#else
+        e = launch_pdl(kern, grid, block, smem, s, use_pdl(a) || late(a), a);
+#endif
         return e != cudaSuccess ? e : cudaGetLastError();
     }
     static cudaError_t row_fwd(const A &a, bool imag, cudaStream_t s) {   // ny == N
         dim3 grid((unsigned)((long)a.batch * a.nx / RowGeomP<N>::RPC)), block(RowGeomP<N>::THREADS);
-        return imag ? go(k_row_fwd_p<N, true>, grid, block, row_smem(), s, a) : go(k_row_fwd_p<N, false>, grid, block, row_smem(), s, a);
+        if (late(a)) return imag ? go(k_row_fwd_p<N, true, true>, grid, block, row_smem(), s, a) : go(k_row_fwd_p<N, false, true>, grid, block, row_smem(), s, a);
+        return imag ? go(k_row_fwd_p<N, true, false>, grid, block, row_smem(), s, a) : go(k_row_fwd_p<N, false, false>, grid, block, row_smem(), s, a);
     }
     static cudaError_t row_inv(const A &a, bool imag, cudaStream_t s) {   // ny == N
         dim3 grid((unsigned)((long)a.batch * a.nx / RowGeomP<N>::RPC)), block(RowGeomP<N>::THREADS);
-        if (imag) return go(k_row_inv_p<N, true, false>, grid, block, row_smem(), s, a);
-        return a.fin.merged ? go(k_row_inv_p<N, false, true>, grid, block, row_smem(), s, a) : go(k_row_inv_p<N, false, false>, grid, block, row_smem(), s, a);
+        if (late(a)) {
+            if (imag) return go(k_row_inv_p<N, true, false, true>, grid, block, row_smem(), s, a);
+            return a.fin.merged ? go(k_row_inv_p<N, false, true, true>, grid, block, row_smem(), s, a) : go(k_row_inv_p<N, false, false, true>, grid, block, row_smem(), s, a);
+        }
+        if (imag) return go(k_row_inv_p<N, true, false, false>, grid, block, row_smem(), s, a);
+        return a.fin.merged ? go(k_row_inv_p<N, false, true, false>, grid, block, row_smem(), s, a) : go(k_row_inv_p<N, false, false, false>, grid, block, row_smem(), s, a);
     }
     static cudaError_t col(const A &a, bool imag, cudaStream_t s) {       // nx == N
         dim3 grid((unsigned)(a.ny / 2 / ColGeomP<N>::CPW), (unsigned)a.batch), block(ColGeomP<N>::THREADS);
-        return imag ? go(k_col_p<N, true>, grid, block, col_smem(), s, a) : go(k_col_p<N, false>, grid, block, col_smem(), s, a);
+        if (late(a)) return imag ? go(k_col_p<N, true, true>, grid, block, col_smem(), s, a) : go(k_col_p<N, false, true>, grid, block, col_smem(), s, a);
+        return imag ? go(k_col_p<N, true, false>, grid, block, col_smem(), s, a) : go(k_col_p<N, false, false>, grid, block, col_smem(), s, a);
     }
 };
 

@@ -2,6 +2,13 @@
 #pragma once
 #include <cuda_runtime.h>
 
+// Paired complex64 passes (gpe_pair.cuh): from this nx on, FOUR rows (not two) are interleaved in the
+// intermediate array, so that a column CTA with one column pair still moves 64 contiguous bytes.  A row
+// CTA owns two rows, so the passes can then no longer work in place: pass A writes the plan's scratch
+// buffer, pass B works inside it, pass C writes psi (gpe_api.cu, evolve_impl).
+#ifndef GPE_IL4_MIN_N
+#define GPE_IL4_MIN_N 2048
+#endif
 namespace gpe {
 
 // Per-member device scalars: written by the last block of the
@@ -98,6 +105,9 @@ template <typename T, typename C> struct StepArgs {
     T inv_p;                       // 1/(nx ny)
     const T *kin_xr, *kin_yr;      // imaginary time: exp(-kx^2 dt/2)/(nx ny), exp(-ky^2 dt/2)
     FinalizeParams fin;
+#ifdef GPE_TRACE
+    unsigned long long *trace;     // debug builds: per-CTA {smid, t0, -, t1}
+#endif
 };
 
 }  // namespace gpe
