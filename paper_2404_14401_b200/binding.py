@@ -54,6 +54,14 @@ def load_library() -> C.CDLL:
         return _LIB
     path = library_path()
     if not os.path.exists(path):
+        # a checkout without built artefacts (libgpe.so is git-ignored): compile it once with nvcc.
+        # Still no fallback of any kind -- if the build fails the import fails.
+        try:
+            from . import build as _build
+            _build.build()
+        except Exception as exc:  # noqa: BLE001
+            raise ImportError(f"{path} is missing and could not be built: {exc}") from exc
+    if not os.path.exists(path):
         raise ImportError(f"{path} is missing: run `python -m paper_2404_14401_b200.build` "
                           "(or __graft_entry__.build()); there is no CPU fallback")
     lib = C.CDLL(path)
