@@ -36,6 +36,10 @@
  *   5. psi <- psi * exp(-sigma (V_n + g|psi|^2) dt/2), |psi|^2 from the psi entering
  *      this line ("most up-to-date wave function")
  *   6. imaginary time only: psi <- psi / sqrt(sum |psi|^2 dx dy)  [PAPER.md:116]
+ * With ordering = 1 (T/2 V T/2, the form the paper prints, Eqs. 3-4) steps 3-5 become:
+ * half of step 4 (dt/4 in its exponent), steps 1-2 evaluated on the psi at that point, one full
+ * potential factor exp(-sigma (V_n + g|psi|^2) dt), half of step 4 again.  Oracle only so far: the
+ * CUDA path does not have this ordering yet.
  *
  * Pins: tests/test_oracle_*.py (direct DFT, numpy.fft, Parseval, shift theorem, exact
  * composition of kinetic steps, free Gaussian expansion, Jacobi-Anger/Bessel, the Gaussian
@@ -87,6 +91,12 @@ typedef struct {
     /* 1: the schedule amplitude of step n is sampled at the middle of the step, A((n + 1/2) dt),
      * instead of its start (reading Q4) */
     int sched_midpoint;
+    /* 0: V/2 T V/2 (steps 3-5 above, north_star); 1: T/2 V T/2, the ordering the paper prints
+     * (Eqs. 3-4; reading Q1): half a kinetic step,
+     * the scalars of step 1 from the psi that ENTERS the potential factor, one full potential
+     * factor exp(-sigma (V_n + g|psi|^2) dt) with |psi|^2 of that same psi, half a kinetic step,
+     * then step 6 */
+    int ordering;
 } oracle_params;
 
 /* ------------------------------------------------------------------ FFT */
@@ -340,10 +350,22 @@ int oracle_evolve(const oracle_params *P, cplx_t *psi, double dt, long n_steps, 
             double theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
             double bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
             double eta, C, Dc; double _Complex alpha;
+            if (P->ordering == 1) {
+                /* T/2 V T/2: kinetic_step(dt') multiplies by exp(-sigma k^2 dt'/2), so dt' = dt/2 is
+                 * half a kinetic step; potential_half_step(dt') multiplies by exp(-sigma (V + g|psi|^2) dt'/2),
+                 * so dt' = 2 dt is the full potential factor */
+                kinetic_step(P, w, 0.5 * dt, imag_time);
+                theta = P->cavity_on ? sum_theta(P, &T, w) : 0.0;
+                bunch = (P->cavity_on && P->cav_u0) ? sum_bunch(P, &T, w) : 0.0;
+                cavity_scalars(P, b, A, theta, bunch, imag_time ? -1.0 : (double)n * dt, &eta, &alpha, &C, &Dc);
+                potential_half_step(P, &T, b, w, A, C, Dc, 2.0 * dt, imag_time);
+                kinetic_step(P, w, 0.5 * dt, imag_time);
+            } else {
             cavity_scalars(P, b, A, theta, bunch, imag_time ? -1.0 : (double)n * dt, &eta, &alpha, &C, &Dc);
             potential_half_step(P, &T, b, w, A, C, Dc, dt, imag_time);
             kinetic_step(P, w, dt, imag_time);
             potential_half_step(P, &T, b, w, A, C, Dc, dt, imag_time);
+            }
             if (imag_time) {
                 real_t inv = (real_t)(1.0 / sqrt(sum_norm(P, w)));
 #pragma omp parallel for schedule(static)

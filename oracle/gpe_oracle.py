@@ -59,6 +59,7 @@ class _Params(C.Structure):
         ("probe_omega", C.c_void_p), ("probe_delta", C.c_void_p), ("probe_phi", C.c_void_p),
         ("cav_u0", C.c_void_p),
         ("sched_midpoint", C.c_int),
+        ("ordering", C.c_int),
     ]
 
 
@@ -169,6 +170,7 @@ class Oracle:
         if p.get("cav_u0") is not None:   # full cavity model, PAPER.md:177,188 (Eqs. 12, 15)
             P.cav_u0 = ptr(_f64(np.broadcast_to(np.asarray(p["cav_u0"], dtype=np.float64), (B,)), B))
         P.sched_midpoint = int(p.get("sched_midpoint", 0))
+        P.ordering = int(p.get("ordering", 0))   # 0: V/2 T V/2; 1: T/2 V T/2
         self.P = P
         self.step = 0
 

@@ -4,7 +4,7 @@ markdown table: relative L2 error of psi, error of the order parameter Theta, an
 the method's own fp32 floor (the oracle's statements in complex64 against complex128 on the same
 input) next to them.
 
-    python tests/full_size_report.py [--quick] > gpurun_out/full_size_parity.md
+    python tests/full_size_report.py [--quick] [--only 3,4c64] > gpurun_out/full_size_parity.md
 
 Needs a B200 and the host cores for the oracle (about an hour without --quick).
 """
@@ -80,26 +80,33 @@ def run(name, p, dtype, mode, dt, checkpoints, floor=True):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--quick", action="store_true", help="a tenth of the steps")
+    ap.add_argument("--only", default="1,2,3,5,4c128,4c64", help="comma-separated subset of 1,2,3,5,4c128,4c64")
     a = ap.parse_args()
     s = 10 if a.quick else 1
+    only = set(a.only.split(","))
     print("| config | dtype | mode | steps | rel L2 err of psi (GPU vs oracle) | fp32 floor of the method | max abs err of Theta | "
           "fp32 floor of Theta | max rel err of the energy | wall s GPU / oracle |")
     print("|---|---|---|---|---|---|---|---|---|---|", flush=True)
-    for g in (0.0, 10.0):
-        run(f"1 (g={g:g})", W.config1(g=g), "c128", "imag", 1e-3, [1, 2000 // s])
-    for dtype in ("c64", "c128"):
-        p = W.config2(V0=10.0, dtype=dtype)
-        p["sched_step"], p["sched_amp"] = None, None           # the ground-state phase has no lattice
-        run("2 ground state", p, dtype, "imag", 1e-3, [1, 1000 // s, 5000 // s])
-    p = W.config3()
-    run("3", p, "c64", "imag", 5e-4, [1, 10, 100, 1000 // s, 5000 // s] if s == 1 else [1, 10, 100, 500])
-    p = W.config5(n_steps=1)
-    run("5 (64 x 512^2)", p, "c64", "imag", 5e-4, [1, 100, 1000 // s])
-    p = W.config4(dtype="c128")
-    run("4", p, "c128", "real", 1e-4, [1, 100, 1000 // s])
-    p = W.config4()
-    run("4", p, "c64", "real", 1e-4, [1, 10, 100, 1000, 5000, 10000] if s == 1 else [1, 10, 100, 1000])
-
+    if "1" in only:
+        for g in (0.0, 10.0):
+            run(f"1 (g={g:g})", W.config1(g=g), "c128", "imag", 1e-3, [1, 2000 // s])
+    if "2" in only:
+        for dtype in ("c64", "c128"):
+            p = W.config2(V0=10.0, dtype=dtype)
+            p["sched_step"], p["sched_amp"] = None, None           # the ground-state phase has no lattice
+            run("2 ground state", p, dtype, "imag", 1e-3, [1, 1000 // s, 5000 // s])
+    if "3" in only:
+        p = W.config3()
+        run("3", p, "c64", "imag", 5e-4, [1, 10, 100, 1000 // s, 5000 // s] if s == 1 else [1, 10, 100, 500])
+    if "5" in only:
+        p = W.config5(n_steps=1)
+        run("5 (64 x 512^2)", p, "c64", "imag", 5e-4, [1, 100, 1000 // s])
+    if "4c128" in only:
+        p = W.config4(dtype="c128")
+        run("4", p, "c128", "real", 1e-4, [1, 100, 1000 // s])
+    if "4c64" in only:
+        p = W.config4()
+        run("4", p, "c64", "real", 1e-4, [1, 10, 100, 1000, 5000, 10000] if s == 1 else [1, 10, 100, 1000])
 
 if __name__ == "__main__":
     main()

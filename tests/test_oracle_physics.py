@@ -574,3 +574,107 @@ def test_f32_build_tracks_f64():
     Oracle(p, "f64").evolve(b, 1e-3, 10, True)
     err = np.linalg.norm(a.astype(np.complex128) - b) / np.linalg.norm(b)
     assert 1e-9 < err < 5e-6
+
+
+# ------------------------------------------------------------------ T/2 V T/2 ordering
+def test_tvt_gaussian_recurrence_closed_form():
+    """ordering = 1, the form the paper prints (Eqs. 3-4).  Same Gaussian algebra as
+    the V/2.T.V/2 pin, in the other order: half a kinetic step 1/a <- 1/a + dt/2,
+    the full potential factor a <- a + dt, half a kinetic step again; renormalisation leaves a alone.
+    Pins the dt/4 in the kinetic exponents, the full dt in the potential factor and their order: after
+    2000 steps the V/2.T.V/2 recurrence gives an a that differs by 2.4e-7, four orders of magnitude
+    above the tolerance (checked below)."""
+    p = W.config1(g=0.0, noise=0.0)
+    p["ordering"] = 1
+    psi = p["psi0"].copy()
+    dt, nsteps = 1e-3, 2000
+    o = Oracle(p)
+    o.evolve(psi, dt, nsteps, True)
+    a = a_vtv = 1.0 / 1.5 ** 2
+    for _ in range(nsteps):
+        a = a / (1 + a * dt / 2)
+        a = a + dt
+        a = a / (1 + a * dt / 2)
+        b = a_vtv + dt / 2
+        a_vtv = b / (1 + b * dt) + dt / 2
+    assert abs(a - a_vtv) > 1e-7
+    obs, _, _ = o.observables(psi)
+    assert obs[0]["norm"] == pytest.approx(1.0, abs=1e-13)
+    assert obs[0]["e_kin"] + obs[0]["e_pot"] == pytest.approx(2 * (a / 4 + 1 / (4 * a)), abs=2e-11)
+    mx, my = _moments(psi, p)
+    assert mx == pytest.approx(1 / (2 * a), abs=2e-11)
+    assert my == pytest.approx(1 / (2 * a), abs=2e-11)
+
+
+def test_tvt_is_the_vtv_propagator_conjugated_by_half_steps():
+    """For a linear, time-independent Hamiltonian (g = 0, static trap + constant lattice, real time)
+    (T/2 V T/2)^n = T/2 V/2 (V/2 T V/2)^(n-1) V/2 T/2 exactly (adjacent half factors of the same
+    operator merge).  The right-hand side is built from the V/2.T.V/2 loop and the single factors,
+    which have their own pins above."""
+    n, L = 64, 16.0
+    p = W._with_trap(W._base(n, n, L))
+    p["lattice_axis"], p["lattice_k"] = 0, 2 * math.pi * 4 / L
+    p["sched_step"], p["sched_amp"] = np.array([0.0]), np.array([3.0])
+    psi0 = W.noisy_gaussian(n, n, L, L, 1.3, 11)
+    dt, ns = 2e-3, 25
+    a = psi0.copy()
+    Oracle({**p, "ordering": 1}).evolve(a, dt, ns, False)
+    b = psi0.copy()
+    o = Oracle(p)
+    o.kinetic_step(b, dt / 2, False)
+    o.potential_half_step(b, dt, False)
+    o.evolve(b, dt, ns - 1, False)
+    o.potential_half_step(b, dt, False)
+    o.kinetic_step(b, dt / 2, False)
+    assert np.linalg.norm(a - b) / np.linalg.norm(b) <= 1e-12
+    c = psi0.copy()
+    Oracle(p).evolve(c, dt, ns, False)
+    assert np.linalg.norm(a - c) / np.linalg.norm(c) > 1e-7      # and the two orderings do differ (1e-6 here)
+
+
+def test_tvt_time_reversal_and_second_order():
+    """The step is symmetric, so running it with -dt undoes it exactly (g != 0 included: a phase factor
+    leaves |psi|^2 alone); and both orderings are second-order approximations of the same flow, so
+    they converge to one another as dt^2."""
+    p = W.config1(g=10.0)
+    psi0 = p["psi0"].copy()
+    q = {**p, "ordering": 1}
+    a = psi0.copy()
+    o = Oracle(q)
+    o.evolve(a, 1e-3, 40, False)
+    assert np.linalg.norm(a - psi0) / np.linalg.norm(psi0) > 1e-2
+    o.evolve(a, -1e-3, 40, False)
+    assert np.linalg.norm(a - psi0) / np.linalg.norm(psi0) <= 1e-12
+
+    def gap(dt, ns):
+        u, v = psi0.copy(), psi0.copy()
+        Oracle(q).evolve(u, dt, ns, False)
+        Oracle(p).evolve(v, dt, ns, False)
+        return np.linalg.norm(u - v) / np.linalg.norm(v)
+    g1, g2 = gap(4e-3, 50), gap(2e-3, 100)
+    assert 3.5 < g1 / g2 < 4.5
+
+
+def test_tvt_cavity_scalars_come_from_the_psi_entering_the_potential_factor():
+    """One T/2 V T/2 step with the cavity, contact interaction and a lattice equals: half a kinetic
+    step, the single potential factor evaluated (Theta, alpha, |psi|^2) on that intermediate psi over
+    2 x dt/2, half a kinetic step, normalisation.  Evaluating Theta on the psi at the start of the
+    step instead gives a different result (checked), so the cadence is pinned."""
+    p = _cavity_small(8.0, g=5.0)
+    psi0 = p["psi0"].copy()
+    dt = 5e-3
+    a = psi0.copy()
+    Oracle({**p, "ordering": 1}).evolve(a, dt, 1, True)
+    b = psi0.copy()
+    o = Oracle(p)
+    o.kinetic_step(b, dt / 2, True)
+    o.potential_half_step(b, 2 * dt, True)
+    o.kinetic_step(b, dt / 2, True)
+    b /= math.sqrt(o.observables(b)[0][0]["norm"])
+    assert np.linalg.norm(a - b) / np.linalg.norm(b) <= 1e-13
+    # the other cadence: Theta of the starting psi, held through the step
+    th0 = o.observables(psi0)[0][0]["theta"]
+    c = psi0.copy()
+    o.kinetic_step(c, dt / 2, True)
+    th_mid = o.observables(c)[0][0]["theta"]
+    assert abs(th_mid - th0) > 1e-6 * abs(th0)
