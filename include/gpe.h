@@ -120,6 +120,15 @@ typedef struct {
     /* 1: the schedule amplitude of step n is sampled at the middle of the step, A(n + 1/2), instead
      * of its start A(n) (reading Q4); records and observables report the same sample. */
     int sched_midpoint;
+    /* Order of the factors of one step (reading Q1).  0 (default): V/2 T V/2 as north_star
+     * spells out.  1: T/2 V T/2, the form the paper prints (Eqs. 3-4): half a kinetic
+     * step, then A_n, Theta_n, alpha_n and |psi|^2 taken from the psi that ENTERS the potential factor,
+     * one full factor exp(-sigma (V_n + g|psi|^2) dt), half a kinetic step, and in imaginary time the
+     * renormalisation.  Real time runs the same three fused passes per step (adjacent kinetic halves
+     * merge; one extra kinetic-only unit per call and per record boundary); imaginary time runs the
+     * unmerged form, two units of three passes per step.  With ordering = 1 gpe_evolve uploads a
+     * second set of kinetic tables the first time a (dt, mode) pair is seen. */
+    int ordering;
 } gpe_potential_desc;
 
 /*

@@ -38,8 +38,7 @@
  *   6. imaginary time only: psi <- psi / sqrt(sum |psi|^2 dx dy)  [PAPER.md:116]
  * With ordering = 1 (T/2 V T/2, the form the paper prints, Eqs. 3-4) steps 3-5 become:
  * half of step 4 (dt/4 in its exponent), steps 1-2 evaluated on the psi at that point, one full
- * potential factor exp(-sigma (V_n + g|psi|^2) dt), half of step 4 again.  Oracle only so far: the
- * CUDA path does not have this ordering yet.
+ * potential factor exp(-sigma (V_n + g|psi|^2) dt), half of step 4 again.
  *
  * Pins: tests/test_oracle_*.py (direct DFT, numpy.fft, Parseval, shift theorem, exact
  * composition of kinetic steps, free Gaussian expansion, Jacobi-Anger/Bessel, the Gaussian

@@ -35,6 +35,7 @@ class gpe_potential_desc(C.Structure):
         ("probe_omega", C.c_void_p), ("probe_delta", C.c_void_p), ("probe_phi", C.c_void_p),
         ("cav_u0", C.c_void_p),
         ("sched_midpoint", C.c_int),
+        ("ordering", C.c_int),
     ]
 
 
@@ -252,6 +253,7 @@ class Plan:
         if p.get("cav_u0") is not None:
             d.cav_u0 = hp(np.broadcast_to(np.asarray(p["cav_u0"], dtype=np.float64), (B,)), B)
         d.sched_midpoint = int(p.get("sched_midpoint", 0))
+        d.ordering = int(p.get("ordering", 0))
         gpe_set_potential(self.plan, d)
         torch.cuda.current_stream().synchronize()
         self._keep = keep

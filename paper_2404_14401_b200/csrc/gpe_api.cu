@@ -65,6 +65,11 @@ struct gpe_plan {
 
     // host copies of the descriptor
     int lattice_axis = -1, sched_len = 0, sched_batched = 0, cavity_on = 0, eta_mode = 0, sched_midpoint = 0;
+    int ordering = 0;          // 0: V/2 T V/2, 1: T/2 V T/2 (gpe.h)
+    // T/2 V T/2: second set of kinetic tables, for half a kinetic step (dt/2)
+    void *kinh_x = nullptr, *kinh_y = nullptr, *kinh_y2 = nullptr;
+    double kinh_dt = 0.0;
+    int kinh_mode = -1;
     double lattice_k = 0, cavity_k = 0;
     std::vector<double> h_sched_step, h_sched_amp, h_eta, h_natoms, h_delta, h_kappa, h_g;
 
@@ -214,6 +219,23 @@ template <typename T> gpe_status make_kinetic(gpe_plan *p, double dt, int mode) 
     p->kin_dt = dt;
     p->epoch++;
     return GPE_OK;
+}
+
+// T/2 V T/2: tables of half a kinetic step (dt/2) in kinh_*, those of a whole one (dt) in kin_*.
+// make_kinetic writes kin_*, so the half set is generated there and swapped out.
+template <typename T> gpe_status make_kinetic_pair(gpe_plan *p, double dt, int mode) {
+    if (!(p->kinh_mode == mode && p->kinh_dt == 0.5 * dt)) {
+        std::swap(p->kin_x, p->kinh_x); std::swap(p->kin_y, p->kinh_y); std::swap(p->kin_y2, p->kinh_y2);
+        std::swap(p->kin_mode, p->kinh_mode);
+        p->kin_dt = -1.0;   // force regeneration (a mode change also reallocates)
+        gpe_status s = make_kinetic<T>(p, 0.5 * dt, mode);
+        if (s != GPE_OK) return s;
+        std::swap(p->kin_x, p->kinh_x); std::swap(p->kin_y, p->kinh_y); std::swap(p->kin_y2, p->kinh_y2);
+        std::swap(p->kin_mode, p->kinh_mode);
+        p->kinh_dt = 0.5 * dt;
+        p->kin_dt = -1.0;
+    }
+    return make_kinetic<T>(p, dt, mode);
 }
 
 // ------------------------------------------------------------------ small kernels
@@ -446,7 +468,8 @@ template <typename T>
 gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode mode, long record_every,
                        double *records, PassProfile *prof = nullptr) {
     const bool imag = mode == GPE_IMAG_TIME;
-    gpe_status s = make_kinetic<T>(p, dt, (int)mode);
+    const bool tvt = p->ordering == 1;
+    gpe_status s = tvt ? make_kinetic_pair<T>(p, dt, (int)mode) : make_kinetic<T>(p, dt, (int)mode);
     if (s != GPE_OK) return s;
     const Ops<T> *oy = get_ops<T>(p->ny), *ox = get_ops<T>(p->nx);
     StepArgs<T, cx<T>> a = base_args<T>(p, psi, psi);
@@ -495,6 +518,76 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
         if (w == 2) GPE_CUDA(p, cudaEventRecord(e1, st));
         return GPE_OK;
     };
+    if (tvt) {
+        // T/2 V T/2 (gpe.h `ordering`, Eqs. 3-4).  A "unit" is the three passes with the
+        // potential factors of pass A and pass C given separately (0 = none: the multiply is exact).
+        if (prof) return fail(p, GPE_EUNSUPPORTED, "per-pass profiling is for the V/2 T V/2 ordering");
+        StepArgs<T, cx<T>> ah = a;   // the same passes on the tables of half a kinetic step
+        ah.kin_xc = (const cx<T> *)p->kinh_x; ah.kin_yc = (const cx<T> *)p->kinh_y;
+        ah.kin_xr = (const T *)p->kinh_x; ah.kin_yr = (const T *)p->kinh_y;
+        ah.kin_y2 = (const T *)p->kinh_y2;
+        auto unit = [&](StepArgs<T, cx<T>> u, T hdt_a, T hdt_c) -> gpe_status {
+            u.src = (const cx<T> *)psi; u.dst = (cx<T> *)psi;
+            u.half_dt = hdt_a;
+            if (oop) u.dst = (cx<T> *)p->scratch;
+            GPE_CUDA(p, paired ? oy->p_row_fwd(u, imag, p->stream) : oy->row_fwd(u, imag, p->stream));
+            if (oop) u.src = (const cx<T> *)p->scratch;
+            GPE_CUDA(p, paired ? ox->p_col(u, imag, p->stream) : ox->col(u, imag, 0, p->stream));
+            u.half_dt = hdt_c;
+            if (oop) u.dst = (cx<T> *)psi;
+            GPE_CUDA(p, paired ? oy->p_row_inv(u, imag, p->stream) : oy->row_inv(u, imag, p->stream));
+            return GPE_OK;
+        };
+        // half a kinetic step, then the scalars of step `stepnow` from the psi it leaves (no advance)
+        auto half_kinetic = [&](long stepnow, int real_tvt) -> gpe_status {
+            StepArgs<T, cx<T>> u = ah;
+            u.fin.advance = 0; u.fin.step0 = stepnow; u.fin.normalise = 0; u.fin.prepared = 0;
+            u.fin.merged = real_tvt; u.fin.tvt = real_tvt;
+            u.fin.record_every = records ? record_every : 0;
+            u.fin.rec_first = record_every > 0 ? p->step / record_every : 0;
+            u.fin.records = records;
+            return unit(u, (T)0, (T)0);
+        };
+        if (!imag) {
+            // T/2 (V T)^(c-1) V T/2 per chunk of c steps: adjacent kinetic halves merge, the full
+            // potential factor is the merged multiply of pass A with both halves on the coefficients
+            // of the psi that enters it (finalize_member, f.tvt).  A chunk ends where a record is due,
+            // because only there is the stored psi the psi_{n+1} the record is taken from.
+            for (long done = 0; done < n_steps;) {
+                const long stepnow = p->step + done;
+                long chunk = n_steps - done;
+                if (records && record_every > 0) {
+                    const long to_rec = record_every - (stepnow % record_every);
+                    if (to_rec < chunk) chunk = to_rec;
+                }
+                if ((s = half_kinetic(stepnow, 1)) != GPE_OK) return s;
+                for (long i = 0; i < chunk; ++i) {
+                    StepArgs<T, cx<T>> u = (i == chunk - 1) ? ah : a;
+                    u.fin = a.fin; u.fin.merged = 1; u.fin.tvt = 1;
+                    if ((s = unit(u, (T)(0.5 * dt), (T)(0.5 * dt))) != GPE_OK) return s;
+                }
+                k_clear_pend<<<(p->batch + 127) / 128, 128, 0, p->stream>>>(p->st, p->batch);
+                GPE_CUDA(p, cudaGetLastError());
+                done += chunk;
+            }
+        } else {
+            // unmerged: the norm is taken after the second kinetic half, so the halves of
+            // consecutive steps cannot merge without a k-space sum in pass B (not built)
+            for (long i = 0; i < n_steps; ++i) {
+                if ((s = half_kinetic(p->step + i, 0)) != GPE_OK) return s;
+                StepArgs<T, cx<T>> u = ah;
+                u.fin = a.fin; u.fin.merged = 0; u.fin.tvt = 0; u.fin.prepared = 0;
+                if ((s = unit(u, (T)dt, (T)0)) != GPE_OK) return s;
+            }
+            dim3 grid(256, p->batch);
+            k_rescale<T><<<grid, 256, 0, p->stream>>>((cx<T> *)psi, (size_t)p->nx * p->ny, p->st);
+            GPE_CUDA(p, cudaGetLastError());
+            k_reset_scale<<<(p->batch + 127) / 128, 128, 0, p->stream>>>(p->st, p->batch);
+            GPE_CUDA(p, cudaGetLastError());
+        }
+        p->step += n_steps;
+        return GPE_OK;
+    }
     long n = 0;
     if (!prof && n_steps >= 2 * kStepsPerGraph) {
         // The arguments of the three passes do not depend on the step (all per-step state is on the
@@ -785,7 +878,7 @@ gpe_status gpe_plan_destroy(gpe_plan *p) {
     cudaStreamSynchronize(p->stream);
     if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
-    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->kin_y2, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
+    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->kin_y2, p->kinh_x, p->kinh_y, p->kinh_y2, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
                     p->ytab, p->g, p->v2d, p->st, p->partials, p->partials_b, p->d_u0, p->counters, p->nonfinite, p->d_sched_step,
                     p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->d_probe_omega, p->d_probe_delta,
                     p->d_probe_phi, p->scratch, p->obs_dev,
@@ -823,6 +916,8 @@ gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
     p->sched_len = d->sched_len; p->sched_batched = d->sched_len > 0 ? (d->sched_batched ? 1 : 0) : 0;
     p->cavity_on = d->cavity_on ? 1 : 0; p->cavity_k = d->cavity_k; p->eta_mode = d->eta_mode;
     p->sched_midpoint = d->sched_midpoint ? 1 : 0;
+    if (d->ordering != 0 && d->ordering != 1) return fail(p, GPE_EINVAL, "ordering must be 0 (V/2 T V/2) or 1 (T/2 V T/2)");
+    p->ordering = d->ordering;
     p->h_sched_step.clear(); p->h_sched_amp.clear();
     if (d->sched_len > 0) {
         p->h_sched_step.assign(d->sched_step, d->sched_step + d->sched_len);

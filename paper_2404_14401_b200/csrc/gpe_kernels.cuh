@@ -121,7 +121,10 @@ __device__ inline void finalize_member(const FinalizeParams &f, int b, double su
         re_a = kre * theta + pre; im_a = kim * theta + pim; C = kc * theta + pc;
     }
     const double Dc = f.cav_u0 ? f.cav_u0[b] * (re_a * re_a + im_a * im_a) : 0.0;   // Eq. 12
-    if (f.advance && f.merged) { s.A_pend = s.A; s.C_pend = s.C; s.D_pend = s.D; s.pend = 1; } else s.pend = 0;
+    // T/2 V T/2 (gpe.h `ordering`): the stored psi is the one that enters the potential factor, so both
+    // halves of the merged multiply of the next pass A take the coefficients computed right here
+    if (f.tvt) { s.A_pend = A; s.C_pend = C; s.D_pend = Dc; s.pend = 1; }
+    else if (f.advance && f.merged) { s.A_pend = s.A; s.C_pend = s.C; s.D_pend = s.D; s.pend = 1; } else s.pend = 0;
     s.D = Dc;
     s.scale = scale; s.A = A; s.C = C; s.norm = norm; s.theta = theta;
     s.re_alpha = re_a; s.im_alpha = im_a; s.step = n1;

@@ -69,6 +69,7 @@ struct FinalizeParams {
     int advance;              // 1: a step was taken (step += 1); 0: prologue reduction
     int prepared;             // 1: pass B has run prepare_member for the step being finalised
     int merged;               // 1: pass C left the second half-step pending (real time, paired passes)
+    int tvt;                  // 1: T/2 V T/2 ordering in real time: the pending factor takes the coefficients of THIS psi
     long long step0;          // used when advance == 0: sets the step counter
 };
 

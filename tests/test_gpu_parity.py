@@ -392,6 +392,53 @@ def test_schedule_midpoint_parity(dtype):
 
 
 @pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("mode", ["real", "imag"])
+@pytest.mark.parametrize("nx,ny,batch", [(64, 64, 1), (256, 128, 2), (128, 1024, 1), (2048, 2048, 1)])
+def test_tvt_ordering_parity(nx, ny, batch, mode, dtype):
+    """ordering = 1 (T/2 V T/2, Eqs. 3-4) against the oracle's
+    ordering = 1: psi after one step and after a run whose length is not a multiple of the record
+    cadence, over two gpe_evolve calls; records (norm, Theta, alpha, A) taken from psi_{n+1}; both
+    kernel families, the out-of-place 2048^2 path, a batch; and the result differs from ordering 0."""
+    p = _general_workload(nx, ny, batch=batch, mode=mode)
+    p["ordering"] = 1
+    dt = 1e-3
+    imag = mode == "imag"
+    plan = _gpu_plan(p, dtype)
+    psi = _to_dev(p["psi0"], dtype)
+    ref = _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    plan.evolve(psi, dt, 1, mode)
+    o.evolve(ref, dt, 1, imag)
+    e1 = _rel(psi.cpu().numpy(), ref)
+    assert e1 <= PER_STEP[dtype], f"1 step: {e1:.3e}"
+    big = nx * ny >= 2048 * 2048
+    n2, every = (5, 2) if big else (10, 4)
+    rg = plan.evolve(psi, dt, n2, mode, record_every=every).cpu().numpy()
+    ro = o.evolve(ref, dt, n2, imag, record_every=every)
+    e = _rel(psi.cpu().numpy(), ref)
+    assert e <= (n2 + 1) * PER_STEP[dtype], f"{n2 + 1} steps: {e:.3e}"
+    assert plan.step == n2 + 1
+    assert rg.shape == ro.shape and rg.shape[0] == (n2 + 1) // every
+    tol = 1e-5 if dtype == "c64" else 1e-10
+    assert np.array_equal(rg[:, :, 0], ro[:, :, 0])
+    for c in (1, 2, 3, 4, 5):
+        assert np.all(np.abs(rg[:, :, c] - ro[:, :, c]) <= tol * np.maximum(np.abs(ro[:, :, c]), 1e-2)), c
+    if not big:
+        other = _oracle_input(p["psi0"], dtype)
+        Oracle({**p, "ordering": 0}).evolve(other, dt, n2 + 1, imag)
+        assert _rel(other, ref) > 1e-7     # the two orderings differ far above the c128 bar
+        # back to the default ordering on the same plan: the V/2 T V/2 path still matches
+        p0 = {**p, "ordering": 0}
+        plan.set_potential(p0)
+        o0 = Oracle(p0)
+        o0.step = o.step
+        plan.evolve(psi, dt, 3, mode)
+        o0.evolve(ref, dt, 3, imag)
+        assert _rel(psi.cpu().numpy(), ref) <= (n2 + 4) * PER_STEP[dtype]
+    plan.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
 def test_probe_parity_and_records(dtype):
     """On-axis cavity probe (Eq. 17): psi and the recorded cavity field against
     the oracle over two gpe_evolve calls (the probe's time origin is the plan's step counter),
@@ -479,7 +526,8 @@ def test_error_behaviour():
     import ctypes as C
     one = (C.c_double * 1)(1.0)
     ptr = C.cast(one, C.c_void_p)
-    for kw in (dict(cav_u0=ptr), dict(probe_omega=ptr), dict(cavity_on=1, cavity_k=1.0, eta_or_u=ptr, delta=ptr, kappa=ptr, probe_phi=ptr)):
+    for kw in (dict(cav_u0=ptr), dict(probe_omega=ptr), dict(cavity_on=1, cavity_k=1.0, eta_or_u=ptr, delta=ptr, kappa=ptr, probe_phi=ptr),
+               dict(ordering=2)):
         with pytest.raises(G.GpeError) as e:
             G.gpe_set_potential(plan, G.gpe_potential_desc(lattice_axis=-1, **kw))
         assert e.value.status == 1, kw
