@@ -20,7 +20,10 @@
  *   Theta_n = sum cos(k_c x) cos(k_c y) |psi_n|^2 dx dy
  *   alpha_n = N_at eta_n Theta_n / (Delta + i kappa),  C_n = 2 eta_n Re(alpha_n),
  *   eta_n = eta (eta_mode 0) or sqrt(|A_n| u) (eta_mode 1; eta = sqrt(V0 U0) in Eq. 13).
- * V_c (Eq. 12) and the dispersive shift (Eq. 15) are not applied (reading Q6).
+ * Optional (gpe_potential_desc.cav_u0, off in BASELINE.json's configs, reading Q6): the full
+ * cavity model adds the cavity lattice U_0 |alpha_n|^2 cos^2(k_c x) (Eq. 12) and the dispersive shift
+ * Delta -> Delta - N_at U_0 sum cos^2(k_c x)|psi_n|^2 dx dy (Eq. 15; the printed equation has no N_at:
+ * with psi normalised to 1 the atom number is explicit, reading Q5).
  *
  * Grid: x_i = -Lx/2 + i Lx/nx, i = 0..nx-1 (periodic), likewise y_j; psi is stored
  * [batch][nx][ny], y fastest, interleaved (re, im); integrals are sums times dx dy.
@@ -34,6 +37,8 @@
  */
 #ifndef GPE_H
 #define GPE_H
+
+#include <stddef.h>
 
 #ifdef __cplusplus
 extern "C" {
@@ -60,6 +65,10 @@ typedef enum {
 } gpe_status;
 
 #define GPE_NREC 6 /* doubles per record: {step, norm, theta, re_alpha, im_alpha, A} */
+
+/* Bumped whenever a struct layout or a signature below changes; the Python binding refuses to run
+ * against a library whose gpe_abi_version() or gpe_sizeof_potential_desc() differ from its own. */
+#define GPE_ABI_VERSION 3
 
 /*
  * gpe_plan_create -- the discretised problem of Eq. 1: an nx x ny periodic grid
@@ -134,7 +143,10 @@ typedef struct {
 /*
  * gpe_set_potential -- copies everything it needs (the caller may free all arrays on return;
  * the device array v_static is copied device-to-device on the plan's stream).  May be called
- * again at any time between gpe_evolve calls.  GPE_EINVAL on inconsistent fields.
+ * again at any time between gpe_evolve calls.  GPE_EINVAL on inconsistent fields: all of them are
+ * checked before the plan is touched, so the previous potential stays in force.  A CUDA failure while
+ * the new one is being uploaded leaves the plan without a potential (GPE_ESTATE until the next
+ * successful call).  Synchronises the plan's stream.
  */
 GPE_API gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d);
 
@@ -149,8 +161,10 @@ GPE_API gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d);
  * records: DEVICE [n_rec][batch][GPE_NREC] = {step, norm, Theta, Re alpha, Im alpha, A}, evaluated on
  * the wavefunction after that step (after the renormalisation in imaginary time), with
  * n_rec = floor((n0+n_steps)/record_every) - floor(n0/record_every).  record_every = 0: none.
- * The call only ENQUEUES work on the plan's stream: no host synchronisation, no host round
- * trip of the per-step scalars (norm, Theta, alpha live in device memory; north_star (3)).
+ * The call only ENQUEUES work on the plan's stream: no host synchronisation (the kinetic tables of a
+ * new (dt, mode) pair are written by a kernel on the same stream, nothing is allocated), no host
+ * round trip of the per-step scalars (norm, Theta, alpha live in device memory; north_star (3)).
+ * The plan's device must be current (GPE_EINVAL otherwise; this holds for every call on a plan).
  * GPE_ESTATE before gpe_set_potential; GPE_EINVAL on bad arguments; GPE_ECUDA on launch errors.
  */
 GPE_API gpe_status gpe_evolve(gpe_plan *p, void *psi_dev, double dt, long n_steps, gpe_mode mode,
@@ -169,7 +183,8 @@ GPE_API gpe_status gpe_evolve(gpe_plan *p, void *psi_dev, double dt, long n_step
  * kdensity_dev (DEVICE real [batch][nx][ny], or NULL): |psi^|^2 / sum |psi^|^2 in FFT order
  * ("directly from the wave-function amplitude in reciprocal space").
  * Synchronises the plan's stream (it returns host values).  psi is not modified.
- * Returns GPE_ENONFINITE if an earlier gpe_evolve on this plan produced a non-finite norm.
+ * Returns GPE_ENONFINITE if an earlier gpe_evolve on this plan produced a non-finite norm: reported
+ * ONCE (the flag is then cleared); out_host and the density buffers are filled all the same.
  */
 typedef struct {
     double norm, e_kin, e_pot, e_int, e_cav, theta, re_alpha, im_alpha;
@@ -207,7 +222,8 @@ GPE_API gpe_status gpe_fft2_forward(gpe_plan *p, const void *src_dev, void *dst_
 GPE_API gpe_status gpe_profile_passes(gpe_plan *p, void *psi_dev, double dt, long n_steps, gpe_mode mode,
                               double *ms_out_host);
 
-/* Step counter n (schedule time origin); see gpe_evolve. */
+/* Step counter n (schedule time origin); see gpe_evolve.  n >= 0: gpe_set_step returns GPE_EINVAL for a
+ * negative value (shift the schedule knots instead). */
 GPE_API gpe_status gpe_get_step(const gpe_plan *p, long *step);
 GPE_API gpe_status gpe_set_step(gpe_plan *p, long step);
 
@@ -217,6 +233,10 @@ GPE_API const char *gpe_last_error(const gpe_plan *p);
 
 /* Library build information: "libgpe <version> sm_100a". */
 GPE_API const char *gpe_version(void);
+
+/* GPE_ABI_VERSION and sizeof(gpe_potential_desc) of the built library (checked by the binding on load). */
+GPE_API int gpe_abi_version(void);
+GPE_API size_t gpe_sizeof_potential_desc(void);
 
 #ifdef __cplusplus
 }

@@ -24,8 +24,8 @@
  *      eta_n = eta (mode 0) or sqrt(|A_n| u) (mode 1).
  *      alpha_n = N_at eta_n Theta_n / (Delta + i kappa)          [PAPER.md:183, Eq. 14]
  *      real time with a probe: alpha_n += Omega_c exp(i (Delta_p t_n + phi)) / (Delta + i kappa),
- *      t_n = n dt (Eq. 17; the dispersive shift of its denominator is not on
- *      this path, reading Q6)
+ *      t_n = n dt (Eq. 17; with cav_u0 its denominator carries the dispersive
+ *      shift of the next line, Delta~_n + i kappa)
  *      with cav_u0 = U_0 (full cavity model): Delta above is replaced by
  *      Delta~_n = Delta - N_at U_0 B_n, B_n = sum cos^2(kc x)|psi|^2 dx dy   [PAPER.md:188, Eq. 15]
  *      and V_n gains the cavity lattice D_n cos^2(kc x), D_n = U_0 |alpha_n|^2 [PAPER.md:177, Eq. 12]

@@ -12,6 +12,7 @@ _LIB = None
 GPE_C64, GPE_C128 = 0, 1
 GPE_REAL_TIME, GPE_IMAG_TIME = 0, 1
 GPE_NREC = 6
+GPE_ABI_VERSION = 3   # include/gpe.h
 _STATUS = {0: "GPE_OK", 1: "GPE_EINVAL", 2: "GPE_EUNSUPPORTED", 3: "GPE_ENOMEM", 4: "GPE_ECUDA",
            5: "GPE_ESTATE", 6: "GPE_ENONFINITE"}
 
@@ -54,17 +55,17 @@ def load_library() -> C.CDLL:
     if _LIB is not None:
         return _LIB
     path = library_path()
-    if not os.path.exists(path):
-        # a checkout without built artefacts (libgpe.so is git-ignored): compile it once with nvcc.
-        # Still no fallback of any kind -- if the build fails the import fails.
+    # libgpe.so is git-ignored: a fresh checkout, or one whose csrc/ or include/gpe.h is newer than the
+    # library, compiles it with nvcc first (build.build() returns at once when it is up to date).  Still
+    # no fallback of any kind -- if the build fails and no library exists, the import fails.
+    from . import build as _build
+    if not _build.up_to_date():
         try:
-            from . import build as _build
             _build.build()
         except Exception as exc:  # noqa: BLE001
-            raise ImportError(f"{path} is missing and could not be built: {exc}") from exc
-    if not os.path.exists(path):
-        raise ImportError(f"{path} is missing: run `python -m paper_2404_14401_b200.build` "
-                          "(or __graft_entry__.build()); there is no CPU fallback")
+            if not os.path.exists(path):
+                raise ImportError(f"{path} is missing and could not be built: {exc}") from exc
+            raise ImportError(f"{path} is older than its sources and could not be rebuilt: {exc}") from exc
     lib = C.CDLL(path)
     vp, i, d, l = C.c_void_p, C.c_int, C.c_double, C.c_long
     lib.gpe_plan_create.restype = i
@@ -93,6 +94,15 @@ def load_library() -> C.CDLL:
     lib.gpe_last_error.argtypes = [vp]
     lib.gpe_version.restype = C.c_char_p
     lib.gpe_version.argtypes = []
+    lib.gpe_abi_version.restype = i
+    lib.gpe_abi_version.argtypes = []
+    lib.gpe_sizeof_potential_desc.restype = C.c_size_t
+    lib.gpe_sizeof_potential_desc.argtypes = []
+    # layout drift between this file and the built library must fail loudly, not corrupt a descriptor
+    if lib.gpe_abi_version() != GPE_ABI_VERSION or lib.gpe_sizeof_potential_desc() != C.sizeof(gpe_potential_desc):
+        raise ImportError(f"{path}: ABI {lib.gpe_abi_version()} / descriptor of {lib.gpe_sizeof_potential_desc()} bytes, "
+                          f"the binding expects ABI {GPE_ABI_VERSION} / {C.sizeof(gpe_potential_desc)} bytes: rebuild "
+                          "with `python -m paper_2404_14401_b200.build --force`")
     _LIB = lib
     return lib
 

@@ -35,6 +35,10 @@ struct gpe_plan {
     bool pot_set = false;
     long step = 0;
     std::string err;
+    int device = 0;            // the device the plan was created on; every call checks it is current
+    // test hooks, read ONCE at gpe_plan_create from the environment (tests/test_gpu_parity.py):
+    // GPE_NO_PAIR = one-number-per-element kernels for complex64 too, GPE_NO_MERGE = separate half-steps
+    bool no_pair = false, no_merge = false;
 
     // device tables (typed by dtype)
     void *tw_x = nullptr, *tw_y = nullptr;
@@ -106,6 +110,21 @@ gpe_status cuda_fail(gpe_plan *p, cudaError_t e, const char *what) {
     do {                                                               \
         cudaError_t e__ = (call);                                      \
         if (e__ != cudaSuccess) return cuda_fail((p), e__, #call);     \
+    } while (0)
+
+// every call must run with the plan's device current: device pointers, the kernels' shared-memory
+// opt-in (cudaFuncSetAttribute is per device) and the plan's buffers all belong to it
+gpe_status check_device(gpe_plan *p) {
+    int dev = -1;
+    GPE_CUDA(p, cudaGetDevice(&dev));
+    if (dev != p->device) return fail(p, GPE_EINVAL, "the plan was created on device " + std::to_string(p->device) +
+                                                      " but device " + std::to_string(dev) + " is current");
+    return GPE_OK;
+}
+#define GPE_CHECK_DEVICE(p)                                            \
+    do {                                                               \
+        gpe_status s__ = check_device(p);                              \
+        if (s__ != GPE_OK) return s__;                                 \
     } while (0)
 
 bool pow2_in_range(int n) { return n >= 64 && n <= 2048 && (n & (n - 1)) == 0; }
@@ -180,60 +199,62 @@ template <typename T> gpe_status make_twiddles(gpe_plan *p) {
     return GPE_OK;
 }
 
-// kinetic tables for (dt, mode) (row a3); 1/(nx ny) of the inverse transform folded into x
-template <typename T> gpe_status make_kinetic(gpe_plan *p, double dt, int mode) {
-    if (p->kin_mode == mode && p->kin_dt == dt) return GPE_OK;
-    if (p->kin_mode != mode) {  // element size changes between real (complex table) and imaginary
-        if (p->kin_x) { cudaFree(p->kin_x); p->kin_x = nullptr; }
-        if (p->kin_y) { cudaFree(p->kin_y); p->kin_y = nullptr; }
-        if (p->kin_y2) { cudaFree(p->kin_y2); p->kin_y2 = nullptr; }
-    }
-    const double invP = 1.0 / ((double)p->nx * (double)p->ny);
+// kinetic tables for (dt, mode) (row a3); 1/(nx ny) of the inverse transform folded into x.
+// Written by a kernel on the plan's stream (fp64 arithmetic, rounded to T once), so that gpe_evolve
+// never synchronises with the host (include/gpe.h: "only ENQUEUES").  One thread per table entry.
+//   imaginary time: kin_x[q] = exp(-kx^2 dt/2)/P, kin_y[q] = exp(-ky^2 dt/2)                  (real tables)
+//   real time:      kin_x[q] = (exp(-i kx^2 dt/2) - 1)/P, kin_y[q] = exp(-i ky^2 dt/2) - 1    (complex),
+//                   exp(-i w) - 1 = -2 sin^2(w/2) - i sin w  (see sincosm1_t in gpe_kernels.cuh)
+//                   kin_y2 = the y table in split layout per column pair for the paired pass B
+template <typename T>
+__global__ void k_make_kinetic(T *kin_x, T *kin_y, T *kin_y2, int nx, int ny, double Lx, double Ly, double dt, int imag) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    const double invP = 1.0 / ((double)nx * (double)ny);
     for (int ax = 0; ax < 2; ++ax) {
-        int n = ax == 0 ? p->nx : p->ny;
-        double L = ax == 0 ? p->Lx : p->Ly;
-        double sc = ax == 0 ? invP : 1.0;
-        std::vector<double> re(n), im(n);
-        for (int q = 0; q < n; ++q) {
-            double k = wavenumber(q, n, L), w = k * k * dt * 0.5;
-            if (mode == GPE_IMAG_TIME) { re[q] = exp(-w) * sc; im[q] = 0.0; }
-            else {  // exp(-i w) - 1 = -2 sin^2(w/2) - i sin w  (see sincosm1_t in gpe_kernels.cuh)
-                double sh = sin(0.5 * w);
-                re[q] = -2.0 * sh * sh * sc; im[q] = -sin(w) * sc;
+        const int n = ax == 0 ? nx : ny;
+        if (q >= n) continue;
+        const double L = ax == 0 ? Lx : Ly, sc = ax == 0 ? invP : 1.0;
+        const double k = 2.0 * kPi * (double)(q < n / 2 ? q : q - n) / L, w = k * k * dt * 0.5;
+        T *dst = ax == 0 ? kin_x : kin_y;
+        if (imag) {
+            dst[q] = (T)(exp(-w) * sc);
+        } else {
+            const double sh = sin(0.5 * w);
+            const double re = -2.0 * sh * sh * sc, im = -sin(w) * sc;
+            dst[2 * q] = (T)re; dst[2 * q + 1] = (T)im;
+            if (ax == 1) {
+                const int c = q >> 1, l = q & 1;
+                kin_y2[8 * c + l] = (T)(1.0 + re); kin_y2[8 * c + 2 + l] = (T)im;
+                kin_y2[8 * c + 4 + l] = (T)(re * invP); kin_y2[8 * c + 6 + l] = (T)(im * invP);
             }
         }
-        void **dev = ax == 0 ? &p->kin_x : &p->kin_y;
-        gpe_status s = mode == GPE_IMAG_TIME ? upload_real<T>(p, dev, re) : upload_cplx<T>(p, dev, re, im);
-        if (s != GPE_OK) return s;
-        if (ax == 1 && mode != GPE_IMAG_TIME) {   // split layout per column pair for the paired pass B (gpe_pair.cuh)
-            std::vector<double> t(4 * (size_t)n);
-            for (int c = 0; c < n / 2; ++c)
-                for (int l = 0; l < 2; ++l) {
-                    const double bx = re[2 * c + l], by = im[2 * c + l];
-                    t[8 * c + l] = 1.0 + bx; t[8 * c + 2 + l] = by; t[8 * c + 4 + l] = bx * invP; t[8 * c + 6 + l] = by * invP;
-                }
-            if ((s = upload_real<T>(p, &p->kin_y2, t)) != GPE_OK) return s;
-        }
     }
+}
+// The buffers are allocated once (gpe_plan_create / gpe_set_potential) at their largest (complex) size.
+template <typename T> gpe_status make_kinetic_into(gpe_plan *p, void *kx, void *ky, void *ky2, double dt, int mode) {
+    const int n = p->nx > p->ny ? p->nx : p->ny;
+    k_make_kinetic<T><<<(n + 127) / 128, 128, 0, p->stream>>>((T *)kx, (T *)ky, (T *)ky2, p->nx, p->ny, p->Lx, p->Ly, dt,
+                                                              mode == GPE_IMAG_TIME ? 1 : 0);
+    GPE_CUDA(p, cudaGetLastError());
+    return GPE_OK;
+}
+template <typename T> gpe_status make_kinetic(gpe_plan *p, double dt, int mode) {
+    if (p->kin_mode == mode && p->kin_dt == dt) return GPE_OK;
+    gpe_status s = make_kinetic_into<T>(p, p->kin_x, p->kin_y, p->kin_y2, dt, mode);
+    if (s != GPE_OK) return s;
     p->kin_mode = mode;
     p->kin_dt = dt;
-    p->epoch++;
     return GPE_OK;
 }
 
-// T/2 V T/2: tables of half a kinetic step (dt/2) in kinh_*, those of a whole one (dt) in kin_*.
-// make_kinetic writes kin_*, so the half set is generated there and swapped out.
+// T/2 V T/2: tables of half a kinetic step (dt/2) in kinh_* (allocated by gpe_set_potential when
+// ordering = 1), those of a whole one (dt) in kin_*.
 template <typename T> gpe_status make_kinetic_pair(gpe_plan *p, double dt, int mode) {
     if (!(p->kinh_mode == mode && p->kinh_dt == 0.5 * dt)) {
-        std::swap(p->kin_x, p->kinh_x); std::swap(p->kin_y, p->kinh_y); std::swap(p->kin_y2, p->kinh_y2);
-        std::swap(p->kin_mode, p->kinh_mode);
-        p->kin_dt = -1.0;   // force regeneration (a mode change also reallocates)
-        gpe_status s = make_kinetic<T>(p, 0.5 * dt, mode);
+        gpe_status s = make_kinetic_into<T>(p, p->kinh_x, p->kinh_y, p->kinh_y2, 0.5 * dt, mode);
         if (s != GPE_OK) return s;
-        std::swap(p->kin_x, p->kinh_x); std::swap(p->kin_y, p->kinh_y); std::swap(p->kin_y2, p->kinh_y2);
-        std::swap(p->kin_mode, p->kinh_mode);
+        p->kinh_mode = mode;
         p->kinh_dt = 0.5 * dt;
-        p->kin_dt = -1.0;
     }
     return make_kinetic<T>(p, dt, mode);
 }
@@ -489,7 +510,7 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
         GPE_CUDA(p, cudaGetLastError());
     }
     // complex64 hot path: paired passes (gpe_pair.cuh) when built for both axis lengths
-    const bool paired = oy->p_row_fwd && ox->p_col && !getenv("GPE_NO_PAIR");
+    const bool paired = oy->p_row_fwd && ox->p_col && !p->no_pair;
     a.fin.cpm = p->nx / (paired ? oy->p_rows_per_cta : oy->rows_per_cta);
     a.fin.normalise = imag ? 1 : 0;
     a.fin.advance = 1;
@@ -497,7 +518,7 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
                                         // with the dispersive shift they depend on the sums
     // real time: pass C leaves its half-step to the next pass A (one multiply
     // by exp(-i (V_n + V_{n+1} + 2 g |psi|^2) dt/2) instead of two; |psi|^2, hence Theta, is unchanged)
-    a.fin.merged = (!imag && !getenv("GPE_NO_MERGE")) ? 1 : 0;
+    a.fin.merged = (!imag && !p->no_merge) ? 1 : 0;
     a.fin.record_every = 0; a.fin.rec_first = 0; a.fin.records = nullptr;  // step kernels read *call
     // four-row-interleaved intermediate array (gpe_types.h): psi -> scratch -> scratch -> psi
     const bool oop = paired && p->nx >= GPE_IL4_MIN_N && p->ny >= GPE_IL4_MIN_N && p->batch == 1;
@@ -726,7 +747,10 @@ gpe_status observables_impl(gpe_plan *p, const void *psi, gpe_obs *out, void *de
             o.e_cav = p->h_natoms[b] * eta * eta * o.theta * o.theta * D / den;
         }
     }
-    if (nonfinite) return fail(p, GPE_ENONFINITE, "a non-finite norm was seen during gpe_evolve");
+    if (nonfinite) {   // reported once: the flag is cleared so that a later, valid run is not blamed for it
+        GPE_CUDA(p, cudaMemsetAsync(p->nonfinite, 0, sizeof(int), p->stream));
+        return fail(p, GPE_ENONFINITE, "a non-finite norm was seen during an earlier gpe_evolve (out_host is filled)");
+    }
     return GPE_OK;
 }
 
@@ -826,7 +850,10 @@ template <typename T> gpe_status set_potential_impl(gpe_plan *p, const gpe_poten
 // ------------------------------------------------------------------ C ABI
 extern "C" {
 
-const char *gpe_version(void) { return "libgpe 0.1 sm_100a"; }
+const char *gpe_version(void) { return "libgpe 0.2 sm_100a"; }
+
+int gpe_abi_version(void) { return GPE_ABI_VERSION; }
+size_t gpe_sizeof_potential_desc(void) { return sizeof(gpe_potential_desc); }
 
 const char *gpe_last_error(const gpe_plan *p) { return p ? p->err.c_str() : g_create_error.c_str(); }
 
@@ -845,6 +872,18 @@ gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly,
         int dev_count = 0;
         GPE_CUDA(p, cudaGetDeviceCount(&dev_count));
         if (dev_count <= 0) return fail(p, GPE_ECUDA, "no CUDA device");
+        GPE_CUDA(p, cudaGetDevice(&p->device));
+        p->no_pair = getenv("GPE_NO_PAIR") != nullptr;     // test hooks, read once (see struct gpe_plan)
+        p->no_merge = getenv("GPE_NO_MERGE") != nullptr;
+        // kinetic tables at their largest (complex) size: gpe_evolve fills them with a kernel and never
+        // allocates (an allocation may synchronise the device)
+        const size_t rb = dtype == GPE_C64 ? 4 : 8;
+        GPE_CUDA(p, cudaMalloc(&p->kin_x, 2 * rb * (size_t)nx));
+        GPE_CUDA(p, cudaMalloc(&p->kin_y, 2 * rb * (size_t)ny));
+        GPE_CUDA(p, cudaMalloc(&p->kin_y2, 4 * rb * (size_t)ny));
+        // out-of-place intermediate array of the paired complex64 passes at 2048^2 (gpe_types.h)
+        if (dtype == GPE_C64 && nx >= GPE_IL4_MIN_N && ny >= GPE_IL4_MIN_N && batch == 1 && !p->no_pair)
+            GPE_CUDA(p, cudaMalloc(&p->scratch, 2 * rb * (size_t)batch * nx * ny));
         GPE_CUDA(p, cudaMalloc((void **)&p->st, sizeof(MemberState) * batch));
         GPE_CUDA(p, cudaMemset(p->st, 0, sizeof(MemberState) * batch));
         GPE_CUDA(p, cudaMalloc((void **)&p->partials, sizeof(double2) * (size_t)batch * kMaxCpm));
@@ -892,6 +931,7 @@ gpe_status gpe_plan_destroy(gpe_plan *p) {
 gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
     if (!p) return GPE_EINVAL;
     if (!d) return fail(p, GPE_EINVAL, "descriptor is NULL");
+    GPE_CHECK_DEVICE(p);
     const int B = p->batch;
     if (d->lattice_axis < -1 || d->lattice_axis > 1) return fail(p, GPE_EINVAL, "lattice_axis must be -1, 0 or 1");
     if (d->sched_len < 0 || (d->sched_len > 0 && (!d->sched_step || !d->sched_amp)))
@@ -912,12 +952,23 @@ gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d) {
             if (d->delta[b] == 0.0 && d->kappa[b] == 0.0) return fail(p, GPE_EINVAL, "Delta + i kappa is zero");
     if (d->v_static && ((uintptr_t)d->v_static % real_bytes(p)) != 0) return fail(p, GPE_EINVAL, "v_static misaligned");
 
+    if (d->ordering != 0 && d->ordering != 1) return fail(p, GPE_EINVAL, "ordering must be 0 (V/2 T V/2) or 1 (T/2 V T/2)");
+    // ---- every check has passed: from here on the plan is rewritten.  A failure below (a CUDA error
+    // during an upload) leaves it WITHOUT a potential (GPE_ESTATE on the next gpe_evolve) rather than
+    // with a mixture of the old and the new descriptor.
+    p->pot_set = false;
+    p->epoch++;
     p->lattice_axis = d->lattice_axis; p->lattice_k = d->lattice_k;
     p->sched_len = d->sched_len; p->sched_batched = d->sched_len > 0 ? (d->sched_batched ? 1 : 0) : 0;
     p->cavity_on = d->cavity_on ? 1 : 0; p->cavity_k = d->cavity_k; p->eta_mode = d->eta_mode;
     p->sched_midpoint = d->sched_midpoint ? 1 : 0;
-    if (d->ordering != 0 && d->ordering != 1) return fail(p, GPE_EINVAL, "ordering must be 0 (V/2 T V/2) or 1 (T/2 V T/2)");
     p->ordering = d->ordering;
+    if (p->ordering == 1 && !p->kinh_x) {   // second set of kinetic tables (dt/2), filled by gpe_evolve
+        const size_t rb = real_bytes(p);
+        GPE_CUDA(p, cudaMalloc(&p->kinh_x, 2 * rb * (size_t)p->nx));
+        GPE_CUDA(p, cudaMalloc(&p->kinh_y, 2 * rb * (size_t)p->ny));
+        GPE_CUDA(p, cudaMalloc(&p->kinh_y2, 4 * rb * (size_t)p->ny));
+    }
     p->h_sched_step.clear(); p->h_sched_amp.clear();
     if (d->sched_len > 0) {
         p->h_sched_step.assign(d->sched_step, d->sched_step + d->sched_len);
@@ -964,6 +1015,7 @@ gpe_status gpe_evolve(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode 
                       double *records) {
     if (!p) return GPE_EINVAL;
     if (!p->pot_set) return fail(p, GPE_ESTATE, "gpe_evolve before gpe_set_potential");
+    GPE_CHECK_DEVICE(p);
     if (!psi || ((uintptr_t)psi % 16) != 0) return fail(p, GPE_EINVAL, "psi is NULL or not 16-byte aligned");
     if (mode != GPE_REAL_TIME && mode != GPE_IMAG_TIME) return fail(p, GPE_EINVAL, "unknown mode");
     if (!std::isfinite(dt) || dt == 0.0 || (mode == GPE_IMAG_TIME && dt < 0.0))
@@ -979,6 +1031,7 @@ gpe_status gpe_fft2_forward(gpe_plan *p, const void *src, void *dst) {
     if (!p) return GPE_EINVAL;
     if (!src || !dst || ((uintptr_t)src % 16) != 0 || ((uintptr_t)dst % 16) != 0)
         return fail(p, GPE_EINVAL, "src/dst NULL or misaligned");
+    GPE_CHECK_DEVICE(p);
     void *keep = p->scratch;
     p->scratch = dst;
     gpe_status s = p->dtype == GPE_C64 ? fft_to_scratch<float>(p, src) : fft_to_scratch<double>(p, src);
@@ -989,6 +1042,7 @@ gpe_status gpe_fft2_forward(gpe_plan *p, const void *src, void *dst) {
 gpe_status gpe_profile_passes(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode mode, double *ms_out) {
     if (!p) return GPE_EINVAL;
     if (!p->pot_set) return fail(p, GPE_ESTATE, "gpe_profile_passes before gpe_set_potential");
+    GPE_CHECK_DEVICE(p);
     if (!psi || !ms_out || ((uintptr_t)psi % 16) != 0) return fail(p, GPE_EINVAL, "psi/ms_out NULL or misaligned");
     if (!std::isfinite(dt) || dt == 0.0 || (mode == GPE_IMAG_TIME && dt < 0.0) || n_steps < 3 || n_steps > 30000)
         return fail(p, GPE_EINVAL, "dt invalid or n_steps outside [3, 30000]");
@@ -1016,6 +1070,7 @@ gpe_status gpe_profile_passes(gpe_plan *p, void *psi, double dt, long n_steps, g
 gpe_status gpe_observables(gpe_plan *p, const void *psi, gpe_obs *out, void *density, void *kdensity) {
     if (!p) return GPE_EINVAL;
     if (!p->pot_set) return fail(p, GPE_ESTATE, "gpe_observables before gpe_set_potential");
+    GPE_CHECK_DEVICE(p);
     if (!psi || !out || ((uintptr_t)psi % 16) != 0) return fail(p, GPE_EINVAL, "psi/out NULL or psi misaligned");
     return p->dtype == GPE_C64 ? observables_impl<float>(p, psi, out, density, kdensity)
                                : observables_impl<double>(p, psi, out, density, kdensity);
@@ -1026,6 +1081,7 @@ gpe_status gpe_populations(gpe_plan *p, const void *psi, int axis, double k_l, i
     if (!psi || !out || ((uintptr_t)psi % 16) != 0) return fail(p, GPE_EINVAL, "psi/out NULL or psi misaligned");
     if ((axis != 0 && axis != 1) || !(k_l > 0) || m_max < 0 || m_max > 64)
         return fail(p, GPE_EINVAL, "axis in {0,1}, k_l > 0, 0 <= m_max <= 64");
+    GPE_CHECK_DEVICE(p);
     return p->dtype == GPE_C64 ? populations_impl<float>(p, psi, axis, k_l, m_max, out)
                                : populations_impl<double>(p, psi, axis, k_l, m_max, out);
 }
@@ -1038,6 +1094,9 @@ gpe_status gpe_get_step(const gpe_plan *p, long *step) {
 
 gpe_status gpe_set_step(gpe_plan *p, long step) {
     if (!p) return GPE_EINVAL;
+    // the record index floor(n / record_every) - floor(n0 / record_every) - 1 and the T/2 V T/2 chunking are
+    // written for n >= 0 (C division truncates); shift the schedule knots instead of the counter
+    if (step < 0) return fail(p, GPE_EINVAL, "the step counter must be >= 0");
     p->step = step;
     return GPE_OK;
 }

@@ -564,15 +564,20 @@ template <typename T, int N> struct Launch {
     static unsigned row_grid(const A &a) { return (unsigned)((long)a.batch * a.nx / RowGeom<N>::RPC); }
     static size_t col_smem() { return sizeof(C) * ColGeom<T, N>::W * Fft1D<N, 1, cx<T>>::SLOTS; }
 
-    // opt in to > 48 KB of dynamic shared memory once per kernel (not on every launch: the
-    // attribute call costs microseconds of host time and the launch path is latency critical)
+    // opt in to > 48 KB of dynamic shared memory once per (device, kernel) -- the attribute is per
+    // device -- and not on every launch: the call costs microseconds of host time on a latency
+    // critical path.  When the table is full the attribute is simply set again (slow but correct).
     template <typename K> static cudaError_t prep(K kern, size_t smem) {
-        static thread_local K done_for[16] = {};
+        struct Slot { K k; int dev; };
+        static thread_local Slot done_for[48] = {};
         if (smem <= 48 * 1024) return cudaSuccess;
-        for (K k : done_for) if (k == kern) return cudaSuccess;
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        for (const Slot &sl : done_for) if (sl.k == kern && sl.dev == dev) return cudaSuccess;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess)
-            for (K &k : done_for) if (k == nullptr) { k = kern; break; }
+            for (Slot &sl : done_for) if (sl.k == nullptr) { sl.k = kern; sl.dev = dev; break; }
         return e;
     }
     // ny == N

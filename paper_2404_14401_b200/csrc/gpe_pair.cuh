@@ -62,26 +62,6 @@ template <int N> struct ColGeomP {
     static constexpr int THREADS = CPW * TPF;
 };
 
-#ifdef GPE_TRACE
-struct TraceScope {
-    unsigned long long *slot, t0;
-    __device__ TraceScope(unsigned long long *base, int pass) {
-        slot = nullptr;
-        if (base && threadIdx.x == 0) {
-            slot = base + ((size_t)pass * 4096 + blockIdx.x + gridDim.x * blockIdx.y) * 4;
-            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
-        }
-    }
-    __device__ void mark(int k) { if (slot) { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); slot[k] = t; } }
-    __device__ ~TraceScope() {
-        if (slot) { unsigned long long t1; unsigned sm; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
-                    slot[0] = sm; slot[1] = t0; slot[3] = t1; }
-    }
-};
-#define GPE_TRACE_SCOPE(pass) TraceScope trace_scope(a.trace, pass)
-#else
-#define GPE_TRACE_SCOPE(pass)
-#endif
 __device__ __forceinline__ void bar_named(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -237,7 +217,6 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     const float2 *src = a.src + row * NY;
     if constexpr (!LATE) pdl_launch_dependents();
     pdl_wait();
-    GPE_TRACE_SCOPE(0);
     float2 p0[16], p1[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
@@ -311,7 +290,6 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / Col
     cpair v[16];
     if constexpr (!LATE) pdl_launch_dependents();
     pdl_wait();
-    GPE_TRACE_SCOPE(1);
     if (blockIdx.x == 0 && threadIdx.x == 0 && a.fin.prepared) prepare_member(a.fin, b);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
@@ -372,7 +350,6 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     const cpair *src = reinterpret_cast<const cpair *>(a.src);
     if constexpr (!LATE) pdl_launch_dependents();
     pdl_wait();
-    GPE_TRACE_SCOPE(2);
     cpair v[16];
     if constexpr (G::PAIRMAP) {
         // mirror of pass A: 32 contiguous bytes (rows 2m, 2m+1, same column pair) per thread and index
@@ -474,10 +451,8 @@ template <int N> struct LaunchP {
     using A = StepArgs<float, float2>;
     static size_t row_smem() { return sizeof(float2) * RowGeomP<N>::RPC * Fft1D<N / 2, 1, cpair>::TILE; }
     static size_t col_smem() { return sizeof(float2) * Fft1D<N, ColGeomP<N>::CPW, cpair>::TILE; }
-    static bool use_pdl(const A &a) {
-        static const long lim = getenv("GPE_PDL_MAX_POINTS") ? atol(getenv("GPE_PDL_MAX_POINTS")) : 65536L;   // tuning knob
-        return (long)a.batch * a.nx * a.ny <= lim;
-    }
+    // launch-bound grids (<= 256^2 points): release the dependent launch at the top (measured on B200)
+    static bool use_pdl(const A &a) { return (long)a.batch * a.nx * a.ny <= 65536L; }
     // Where a pass releases its dependent launch (programmatic dependent launch, gpe_kernels.cuh):
     // at the top for launch-bound grids (<= 256^2 points), after its last store -- a compile-time
     // variant, LATE -- for single grids of a wave or two (measured on B200, us per step: 512^2 17.4 -> 16.3,
@@ -485,21 +460,13 @@ template <int N> struct LaunchP {
     // all for batches of many waves.  The instruction after the stores is not free even when predicated
     // off at run time (config 5: +6 us per step), hence the template parameter.
     static bool late(const A &a) {
-        static const long lo = getenv("GPE_PDL_LATE_MIN_POINTS") ? atol(getenv("GPE_PDL_LATE_MIN_POINTS")) : 65537L;   // tuning knobs
-        static const long hi = getenv("GPE_PDL_LATE_MAX_POINTS") ? atol(getenv("GPE_PDL_LATE_MAX_POINTS")) : (1L << 23) - 1;
         const long pts = (long)a.batch * a.nx * a.ny;
-        return pts >= lo && pts <= hi;
+        return pts > 65536L && pts < (1L << 23);
     }
     template <typename K> static cudaError_t go(K kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, const A &a) {
         cudaError_t e = Launch<float, N>::prep(kern, smem);
         if (e != cudaSuccess) return e;
-#ifdef GPE_TRACE
-        A a2 = a;
-        a2.trace = getenv("GPE_TRACE_PTR") ? (unsigned long long *)strtoull(getenv("GPE_TRACE_PTR"), nullptr, 0) : nullptr;
-        e = launch_pdl(kern, grid, block, smem, s, use_pdl(a) || late(a), a2);
-#else
         e = launch_pdl(kern, grid, block, smem, s, use_pdl(a) || late(a), a);
-#endif
         return e != cudaSuccess ? e : cudaGetLastError();
     }
     static cudaError_t row_fwd(const A &a, bool imag, cudaStream_t s) {   // ny == N

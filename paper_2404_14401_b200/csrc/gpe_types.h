@@ -106,9 +106,6 @@ template <typename T, typename C> struct StepArgs {
     T inv_p;                       // 1/(nx ny)
     const T *kin_xr, *kin_yr;      // imaginary time: exp(-kx^2 dt/2)/(nx ny), exp(-ky^2 dt/2)
     FinalizeParams fin;
-#ifdef GPE_TRACE
-    unsigned long long *trace;     // debug builds: per-CTA {smid, t0, -, t1}
-#endif
 };
 
 }  // namespace gpe
