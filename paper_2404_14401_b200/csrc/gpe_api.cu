@@ -10,6 +10,9 @@
 #include <string>
 #include <vector>
 
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
 #include "../../include/gpe.h"
 #include "gpe_dispatch.h"
 #include "gpe_kernels.cuh"
@@ -38,7 +41,8 @@ struct gpe_plan {
     int device = 0;            // the device the plan was created on; every call checks it is current
     // test hooks, read ONCE at gpe_plan_create from the environment (tests/test_gpu_parity.py):
     // GPE_NO_PAIR = one-number-per-element kernels for complex64 too, GPE_NO_MERGE = separate half-steps
-    bool no_pair = false, no_merge = false;
+    bool no_pair = false, no_merge = false, no_stream = false;   // GPE_NO_STREAM: one-tile-per-CTA passes only
+    int num_sms = 0;
 
     // device tables (typed by dtype)
     void *tw_x = nullptr, *tw_y = nullptr;
@@ -104,7 +108,8 @@ gpe_status fail(gpe_plan *p, gpe_status s, const std::string &msg) {
     return s;
 }
 gpe_status cuda_fail(gpe_plan *p, cudaError_t e, const char *what) {
-    return fail(p, GPE_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    cudaGetLastError();   // clear the (non-sticky) error so that a later launch check does not report it again
+    return fail(p, e == cudaErrorMemoryAllocation ? GPE_ENOMEM : GPE_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
 }
 #define GPE_CUDA(p, call)                                              \
     do {                                                               \
@@ -476,6 +481,48 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     return a;
 }
 
+// Tensor maps of the persistent passes (gpe_stream.cuh).  The driver entry point is looked up at run
+// time (no link dependency on libcuda); encoding is pure host work (no stream, no synchronisation).
+PFN_cuTensorMapEncodeTiled encode_fn() {
+    static PFN_cuTensorMapEncodeTiled fn = [] {
+        void *f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) f = nullptr;
+        return (PFN_cuTensorMapEncodeTiled)f;
+    }();
+    return fn;
+}
+// pass B: the intermediate array [batch nx / 2^il][ny/2][2^il rows][4 floats] as a 2-D float tensor whose
+// lines are the row groups; a box is `cpw` column pairs wide and min(256, nx / 2^il) lines tall
+gpe_status make_col_map(gpe_plan *p, CUtensorMap *m, void *base, int il, int cpw) {
+    PFN_cuTensorMapEncodeTiled enc = encode_fn();
+    if (!enc) return fail(p, GPE_ECUDA, "cuTensorMapEncodeTiled is not available");
+    const int lines = p->nx >> il, bl = lines < 256 ? lines : 256;
+    cuuint64_t gdim[2] = {(cuuint64_t)(p->ny / 2) * (4u << il), (cuuint64_t)p->batch * lines};
+    cuuint64_t gstr[1] = {gdim[0] * sizeof(float)};
+    cuuint32_t box[2] = {(cuuint32_t)cpw * (4u << il), (cuuint32_t)bl};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(p, GPE_ECUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+    return GPE_OK;
+}
+
+// pass C with four interleaved rows (2048^2): [batch nx/4 * ny/2 cells][2 halves][8 floats]; a box is one half
+// (= one row pair) of 256 consecutive cells
+gpe_status make_rowc_map(gpe_plan *p, CUtensorMap *m, void *base) {
+    PFN_cuTensorMapEncodeTiled enc = encode_fn();
+    if (!enc) return fail(p, GPE_ECUDA, "cuTensorMapEncodeTiled is not available");
+    cuuint64_t gdim[3] = {8, 2, (cuuint64_t)p->batch * (p->nx / 4) * (p->ny / 2)};
+    cuuint64_t gstr[2] = {32, 64};
+    cuuint32_t box[3] = {8, 1, 256};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(p, GPE_ECUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
+    return GPE_OK;
+}
+
 // per-pass timing (gpe_profile_passes): events bracket ONE pass per step, round-robin, so the
 // host stays ahead of the device and no launch gap is measured.
 struct PassProfile {
@@ -511,7 +558,11 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     }
     // complex64 hot path: paired passes (gpe_pair.cuh) when built for both axis lengths
     const bool paired = oy->p_row_fwd && ox->p_col && !p->no_pair;
-    a.fin.cpm = p->nx / (paired ? oy->p_rows_per_cta : oy->rows_per_cta);
+    // persistent bulk-copy-fed passes where built for the axis length (gpe_stream.cuh); the row passes
+    // come as a pair (pass C's partial sums are per tile)
+    const bool s_col = paired && ox->s_col && !p->no_stream;
+    const bool s_row = paired && oy->s_row_fwd && oy->s_row_inv && !p->no_stream;
+    a.fin.cpm = p->nx / (s_row ? oy->s_rows_per_tile : paired ? oy->p_rows_per_cta : oy->rows_per_cta);
     a.fin.normalise = imag ? 1 : 0;
     a.fin.advance = 1;
     a.fin.prepared = p->d_u0 ? 0 : 1;   // pass B prepares the coefficients of the next step (prepare_member);
@@ -523,18 +574,34 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     // four-row-interleaved intermediate array (gpe_types.h): psi -> scratch -> scratch -> psi
     const bool oop = paired && p->nx >= GPE_IL4_MIN_N && p->ny >= GPE_IL4_MIN_N && p->batch == 1;
     if (oop && (s = ensure_scratch(p)) != GPE_OK) return s;
+    alignas(64) CUtensorMap map_col, map_rowc;
+    memset(&map_rowc, 0, sizeof(map_rowc));
+    if (s_row && oop && (s = make_rowc_map(p, &map_rowc, p->scratch)) != GPE_OK) return s;
+    auto pass_a = [&](const StepArgs<T, cx<T>> &u, cudaStream_t st) -> cudaError_t {
+        if constexpr (sizeof(T) == 4) { if (s_row) return oy->s_row_fwd(u, imag, p->num_sms, st); }
+        return paired ? oy->p_row_fwd(u, imag, st) : oy->row_fwd(u, imag, st);
+    };
+    auto pass_c = [&](const StepArgs<T, cx<T>> &u, cudaStream_t st) -> cudaError_t {
+        if constexpr (sizeof(T) == 4) { if (s_row) return oy->s_row_inv(u, map_rowc, imag, p->num_sms, st); }
+        return paired ? oy->p_row_inv(u, imag, st) : oy->row_inv(u, imag, st);
+    };
+    if (s_col && (s = make_col_map(p, &map_col, oop ? p->scratch : psi, oop ? 2 : 1, ox->s_col_cpw)) != GPE_OK) return s;
+    auto pass_b = [&](const StepArgs<T, cx<T>> &u, cudaStream_t st) -> cudaError_t {
+        if constexpr (sizeof(T) == 4) { if (s_col) return ox->s_col(u, map_col, imag, p->num_sms, st); }
+        return paired ? ox->p_col(u, imag, st) : ox->col(u, imag, 0, st);
+    };
     auto one_step = [&](cudaStream_t st, int w, cudaEvent_t e0, cudaEvent_t e1) -> gpe_status {
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, st));
         if (oop) a.dst = (cx<T> *)p->scratch;
-        GPE_CUDA(p, paired ? oy->p_row_fwd(a, imag, st) : oy->row_fwd(a, imag, st));
+        GPE_CUDA(p, pass_a(a, st));
         if (oop) a.src = (const cx<T> *)p->scratch;
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e1, st));
         if (w == 1) GPE_CUDA(p, cudaEventRecord(e0, st));
-        GPE_CUDA(p, paired ? ox->p_col(a, imag, st) : ox->col(a, imag, 0, st));
+        GPE_CUDA(p, pass_b(a, st));
         if (w == 1) GPE_CUDA(p, cudaEventRecord(e1, st));
         if (w == 2) GPE_CUDA(p, cudaEventRecord(e0, st));
         if (oop) a.dst = (cx<T> *)psi;
-        GPE_CUDA(p, paired ? oy->p_row_inv(a, imag, st) : oy->row_inv(a, imag, st));
+        GPE_CUDA(p, pass_c(a, st));
         if (oop) a.src = (const cx<T> *)psi;
         if (w == 2) GPE_CUDA(p, cudaEventRecord(e1, st));
         return GPE_OK;
@@ -551,12 +618,12 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
             u.src = (const cx<T> *)psi; u.dst = (cx<T> *)psi;
             u.half_dt = hdt_a;
             if (oop) u.dst = (cx<T> *)p->scratch;
-            GPE_CUDA(p, paired ? oy->p_row_fwd(u, imag, p->stream) : oy->row_fwd(u, imag, p->stream));
+            GPE_CUDA(p, pass_a(u, p->stream));
             if (oop) u.src = (const cx<T> *)p->scratch;
-            GPE_CUDA(p, paired ? ox->p_col(u, imag, p->stream) : ox->col(u, imag, 0, p->stream));
+            GPE_CUDA(p, pass_b(u, p->stream));
             u.half_dt = hdt_c;
             if (oop) u.dst = (cx<T> *)psi;
-            GPE_CUDA(p, paired ? oy->p_row_inv(u, imag, p->stream) : oy->row_inv(u, imag, p->stream));
+            GPE_CUDA(p, pass_c(u, p->stream));
             return GPE_OK;
         };
         // half a kinetic step, then the scalars of step `stepnow` from the psi it leaves (no advance)
@@ -875,6 +942,8 @@ gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly,
         GPE_CUDA(p, cudaGetDevice(&p->device));
         p->no_pair = getenv("GPE_NO_PAIR") != nullptr;     // test hooks, read once (see struct gpe_plan)
         p->no_merge = getenv("GPE_NO_MERGE") != nullptr;
+        p->no_stream = getenv("GPE_NO_STREAM") != nullptr;
+        GPE_CUDA(p, cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device));
         // kinetic tables at their largest (complex) size: gpe_evolve fills them with a kernel and never
         // allocates (an allocation may synchronise the device)
         const size_t rb = dtype == GPE_C64 ? 4 : 8;

@@ -174,15 +174,15 @@ def test_config3_cavity_imag_reduced():
     assert rec.shape == rref.shape
     assert np.array_equal(rec[:, :, 0], rref[:, :, 0])
     assert np.allclose(rec[:, :, 1], 1.0, atol=1e-12)
-    # order parameter: |dTheta| <= 1e-5 max(|Theta|, 1e-2)  (reading Q17), or within
-    # 3x the fp32 floor of the method itself where the instability amplifies round-off (R2):
-    # the floor is the oracle's own statements run in complex64 (float build) vs complex128.
+    # order parameter: |dTheta| <= 1e-5 max(|Theta|, 1e-2)  (reading Q17), alone.  The fp32 floor of
+    # the method (the oracle's own statements in complex64 against complex128) is printed next to it; the
+    # floor rule itself is only used at full size (tests/test_gpu_fullsize.py), where it is needed.
     f32 = p["psi0"].astype(np.complex64)
     rfloor = Oracle(p, "f32").evolve(f32, 5e-4, 400, True, record_every=50)
     floor = np.abs(rfloor[:, :, 2] - rref[:, :, 2])
     dth = np.abs(rec[:, :, 2] - rref[:, :, 2])
     print("theta err gpu", dth.ravel(), "fp32 floor", floor.ravel())
-    assert np.all(dth <= np.maximum(1e-5 * np.maximum(np.abs(rref[:, :, 2]), 1e-2), 3 * floor))
+    assert np.all(dth <= 1e-5 * np.maximum(np.abs(rref[:, :, 2]), 1e-2))
     go = plan.observables(psi)[0][0]
     ro = o.observables(ref)[0][0]
     for k in ("e_kin", "e_pot", "e_int"):
@@ -203,8 +203,8 @@ def test_config4_ramp_reduced(dtype):
     assert _rel(psi.cpu().numpy(), ref) <= FULL_RUN[dtype]
     tol = 1e-5 if dtype == "c64" else 1e-10
     assert np.allclose(rec[:, :, 1], rref[:, :, 1], rtol=tol)
-    # order parameter and field: 1e-5 relative (reading Q17), or 3x the fp32 floor of the method
-    # itself (the oracle's statements in complex64 vs complex128) where that is larger (R2)
+    # order parameter and field: 1e-5 relative (reading Q17) alone; the fp32 floor of the method (the
+    # oracle's statements in complex64 vs complex128) is printed for context only
     floor = np.zeros_like(rref)
     if dtype == "c64":
         f32 = p["psi0"].astype(np.complex64)
@@ -212,9 +212,9 @@ def test_config4_ramp_reduced(dtype):
         floor = np.abs(rfl - rref)
     err = np.abs(rec - rref)
     print("theta err", err[:, 0, 2], "fp32 floor", floor[:, 0, 2])
-    assert np.all(err[:, :, 2] <= np.maximum(tol * np.maximum(np.abs(rref[:, :, 2]), 1e-2), 3 * floor[:, :, 2]))
+    assert np.all(err[:, :, 2] <= tol * np.maximum(np.abs(rref[:, :, 2]), 1e-2))
     amax = np.abs(rref[:, :, 3:5]).max()
-    assert np.all(err[:, :, 3:5] <= np.maximum(tol * max(amax, 1e-2), 3 * floor[:, :, 3:5]))
+    assert np.all(err[:, :, 3:5] <= tol * max(amax, 1e-2))
     assert np.allclose(rec[:, :, 5], rref[:, :, 5], rtol=1e-14)
     plan.close()
 
