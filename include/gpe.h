@@ -222,6 +222,18 @@ GPE_API gpe_status gpe_fft2_forward(gpe_plan *p, const void *src_dev, void *dst_
 GPE_API gpe_status gpe_profile_passes(gpe_plan *p, void *psi_dev, double dt, long n_steps, gpe_mode mode,
                               double *ms_out_host);
 
+/*
+ * gpe_measure_roofs -- the denominators of the roofline report, measured on the current device
+ * ("L2 peak is not in MEASURED_PEAKS.json -- the builder measures it"; plain-ALU rates
+ * "to be replaced by a measured FMA-loop probe").  Not part of the method.  out_host[5] =
+ *   [0] GB/s of an in-place read + write (128-bit accesses, persistent CTAs) over a 32 MiB buffer --
+ *       the size of the 2048^2 complex64 wavefunction, resident in L2 --, [1] the same over 64 MiB
+ *       (2048^2 complex128), [2] the same over 1 GiB (HBM),
+ *   [3] Tflop/s of independent fp32 fused multiply-add chains, [4] the same in fp64.
+ * Runs on cuda_stream and synchronises it.  GPE_ENOMEM if the 1 GiB scratch buffer cannot be had.
+ */
+GPE_API gpe_status gpe_measure_roofs(void *cuda_stream, double *out_host);
+
 /* Step counter n (schedule time origin); see gpe_evolve.  n >= 0: gpe_set_step returns GPE_EINVAL for a
  * negative value (shift the schedule knots instead). */
 GPE_API gpe_status gpe_get_step(const gpe_plan *p, long *step);

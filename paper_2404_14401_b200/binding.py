@@ -86,6 +86,8 @@ def load_library() -> C.CDLL:
     lib.gpe_fft2_forward.argtypes = [vp, vp, vp]
     lib.gpe_profile_passes.restype = i
     lib.gpe_profile_passes.argtypes = [vp, vp, d, l, i, C.POINTER(C.c_double)]
+    lib.gpe_measure_roofs.restype = i
+    lib.gpe_measure_roofs.argtypes = [vp, C.POINTER(C.c_double)]
     lib.gpe_get_step.restype = i
     lib.gpe_get_step.argtypes = [vp, C.POINTER(l)]
     lib.gpe_set_step.restype = i
@@ -171,6 +173,13 @@ def gpe_profile_passes(plan, psi_ptr: int, dt: float, n_steps: int, mode: int):
     _check(load_library().gpe_profile_passes(plan, C.c_void_p(psi_ptr), float(dt), int(n_steps), int(mode), out),
            plan)
     return [out[0], out[1], out[2]]
+
+
+def gpe_measure_roofs(cuda_stream: int = 0) -> dict:
+    out = (C.c_double * 5)()
+    _check(load_library().gpe_measure_roofs(C.c_void_p(cuda_stream), out), None)
+    return {"l2_rw_32MiB_gbs": out[0], "l2_rw_64MiB_gbs": out[1], "hbm_rw_1GiB_gbs": out[2],
+            "fp32_fma_tflops": out[3], "fp64_fma_tflops": out[4]}
 
 
 def gpe_get_step(plan) -> int:

@@ -10,9 +10,6 @@
 #include <string>
 #include <vector>
 
-#include <cuda.h>
-#include <cudaTypedefs.h>
-
 #include "../../include/gpe.h"
 #include "gpe_dispatch.h"
 #include "gpe_kernels.cuh"
@@ -41,8 +38,7 @@ struct gpe_plan {
     int device = 0;            // the device the plan was created on; every call checks it is current
     // test hooks, read ONCE at gpe_plan_create from the environment (tests/test_gpu_parity.py):
     // GPE_NO_PAIR = one-number-per-element kernels for complex64 too, GPE_NO_MERGE = separate half-steps
-    bool no_pair = false, no_merge = false, no_stream = false;   // GPE_NO_STREAM: one-tile-per-CTA passes only
-    int num_sms = 0;
+    bool no_pair = false, no_merge = false;
 
     // device tables (typed by dtype)
     void *tw_x = nullptr, *tw_y = nullptr;
@@ -444,6 +440,33 @@ __global__ void __launch_bounds__(256) k_populations(const cx<T> *hat, int nx, i
     for (int m = threadIdx.x; m < nm; m += blockDim.x) atomicAdd(&pop[(size_t)b * nm + m], spop[m]);
 }
 
+// ------------------------------------------------------------------ roofline denominators (gpe_measure_roofs)
+// in-place read + write of a buffer with 128-bit accesses by persistent CTAs: the traffic pattern of one
+// fused pass (every byte read once and written once), nothing else
+__global__ void __launch_bounds__(256) k_roof_rw(float4 *buf, size_t n4, float add) {
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n4; q += (size_t)gridDim.x * blockDim.x) {
+        float4 v = __ldcg(buf + q);
+        v.x += add; v.y += add; v.z += add; v.w += add;
+        buf[q] = v;
+    }
+}
+// dependent-free fused multiply-add chains, 8 independent accumulators per thread: the plain-ALU peak
+template <typename T> __global__ void __launch_bounds__(256) k_roof_fma(T *out, T a, T b, int iters) {
+    T acc[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = (T)(threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) acc[i] = acc[i] * a + b;
+    }
+    T sum = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) sum += acc[i];
+    if (sum == (T)123456789) out[blockIdx.x * blockDim.x + threadIdx.x] = sum;   // never true: keeps the chains alive
+}
+
 // ------------------------------------------------------------------ typed implementations
 template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src, void *dst) {
     StepArgs<T, cx<T>> a;
@@ -481,48 +504,6 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     return a;
 }
 
-// Tensor maps of the persistent passes (gpe_stream.cuh).  The driver entry point is looked up at run
-// time (no link dependency on libcuda); encoding is pure host work (no stream, no synchronisation).
-PFN_cuTensorMapEncodeTiled encode_fn() {
-    static PFN_cuTensorMapEncodeTiled fn = [] {
-        void *f = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) f = nullptr;
-        return (PFN_cuTensorMapEncodeTiled)f;
-    }();
-    return fn;
-}
-// pass B: the intermediate array [batch nx / 2^il][ny/2][2^il rows][4 floats] as a 2-D float tensor whose
-// lines are the row groups; a box is `cpw` column pairs wide and min(256, nx / 2^il) lines tall
-gpe_status make_col_map(gpe_plan *p, CUtensorMap *m, void *base, int il, int cpw) {
-    PFN_cuTensorMapEncodeTiled enc = encode_fn();
-    if (!enc) return fail(p, GPE_ECUDA, "cuTensorMapEncodeTiled is not available");
-    const int lines = p->nx >> il, bl = lines < 256 ? lines : 256;
-    cuuint64_t gdim[2] = {(cuuint64_t)(p->ny / 2) * (4u << il), (cuuint64_t)p->batch * lines};
-    cuuint64_t gstr[1] = {gdim[0] * sizeof(float)};
-    cuuint32_t box[2] = {(cuuint32_t)cpw * (4u << il), (cuuint32_t)bl};
-    cuuint32_t estr[2] = {1, 1};
-    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(p, GPE_ECUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
-    return GPE_OK;
-}
-
-// pass C with four interleaved rows (2048^2): [batch nx/4 * ny/2 cells][2 halves][8 floats]; a box is one half
-// (= one row pair) of 256 consecutive cells
-gpe_status make_rowc_map(gpe_plan *p, CUtensorMap *m, void *base) {
-    PFN_cuTensorMapEncodeTiled enc = encode_fn();
-    if (!enc) return fail(p, GPE_ECUDA, "cuTensorMapEncodeTiled is not available");
-    cuuint64_t gdim[3] = {8, 2, (cuuint64_t)p->batch * (p->nx / 4) * (p->ny / 2)};
-    cuuint64_t gstr[2] = {32, 64};
-    cuuint32_t box[3] = {8, 1, 256};
-    cuuint32_t estr[3] = {1, 1, 1};
-    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return fail(p, GPE_ECUDA, "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")");
-    return GPE_OK;
-}
-
 // per-pass timing (gpe_profile_passes): events bracket ONE pass per step, round-robin, so the
 // host stays ahead of the device and no launch gap is measured.
 struct PassProfile {
@@ -558,11 +539,7 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     }
     // complex64 hot path: paired passes (gpe_pair.cuh) when built for both axis lengths
     const bool paired = oy->p_row_fwd && ox->p_col && !p->no_pair;
-    // persistent bulk-copy-fed passes where built for the axis length (gpe_stream.cuh); the row passes
-    // come as a pair (pass C's partial sums are per tile)
-    const bool s_col = paired && ox->s_col && !p->no_stream;
-    const bool s_row = paired && oy->s_row_fwd && oy->s_row_inv && !p->no_stream;
-    a.fin.cpm = p->nx / (s_row ? oy->s_rows_per_tile : paired ? oy->p_rows_per_cta : oy->rows_per_cta);
+    a.fin.cpm = p->nx / (paired ? oy->p_rows_per_cta : oy->rows_per_cta);
     a.fin.normalise = imag ? 1 : 0;
     a.fin.advance = 1;
     a.fin.prepared = p->d_u0 ? 0 : 1;   // pass B prepares the coefficients of the next step (prepare_member);
@@ -574,21 +551,14 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
     // four-row-interleaved intermediate array (gpe_types.h): psi -> scratch -> scratch -> psi
     const bool oop = paired && p->nx >= GPE_IL4_MIN_N && p->ny >= GPE_IL4_MIN_N && p->batch == 1;
     if (oop && (s = ensure_scratch(p)) != GPE_OK) return s;
-    alignas(64) CUtensorMap map_col, map_rowc;
-    memset(&map_rowc, 0, sizeof(map_rowc));
-    if (s_row && oop && (s = make_rowc_map(p, &map_rowc, p->scratch)) != GPE_OK) return s;
     auto pass_a = [&](const StepArgs<T, cx<T>> &u, cudaStream_t st) -> cudaError_t {
-        if constexpr (sizeof(T) == 4) { if (s_row) return oy->s_row_fwd(u, imag, p->num_sms, st); }
         return paired ? oy->p_row_fwd(u, imag, st) : oy->row_fwd(u, imag, st);
     };
-    auto pass_c = [&](const StepArgs<T, cx<T>> &u, cudaStream_t st) -> cudaError_t {
-        if constexpr (sizeof(T) == 4) { if (s_row) return oy->s_row_inv(u, map_rowc, imag, p->num_sms, st); }
-        return paired ? oy->p_row_inv(u, imag, st) : oy->row_inv(u, imag, st);
-    };
-    if (s_col && (s = make_col_map(p, &map_col, oop ? p->scratch : psi, oop ? 2 : 1, ox->s_col_cpw)) != GPE_OK) return s;
     auto pass_b = [&](const StepArgs<T, cx<T>> &u, cudaStream_t st) -> cudaError_t {
-        if constexpr (sizeof(T) == 4) { if (s_col) return ox->s_col(u, map_col, imag, p->num_sms, st); }
         return paired ? ox->p_col(u, imag, st) : ox->col(u, imag, 0, st);
+    };
+    auto pass_c = [&](const StepArgs<T, cx<T>> &u, cudaStream_t st) -> cudaError_t {
+        return paired ? oy->p_row_inv(u, imag, st) : oy->row_inv(u, imag, st);
     };
     auto one_step = [&](cudaStream_t st, int w, cudaEvent_t e0, cudaEvent_t e1) -> gpe_status {
         if (w == 0) GPE_CUDA(p, cudaEventRecord(e0, st));
@@ -942,8 +912,6 @@ gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly,
         GPE_CUDA(p, cudaGetDevice(&p->device));
         p->no_pair = getenv("GPE_NO_PAIR") != nullptr;     // test hooks, read once (see struct gpe_plan)
         p->no_merge = getenv("GPE_NO_MERGE") != nullptr;
-        p->no_stream = getenv("GPE_NO_STREAM") != nullptr;
-        GPE_CUDA(p, cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, p->device));
         // kinetic tables at their largest (complex) size: gpe_evolve fills them with a kernel and never
         // allocates (an allocation may synchronise the device)
         const size_t rb = dtype == GPE_C64 ? 4 : 8;
@@ -1153,6 +1121,63 @@ gpe_status gpe_populations(gpe_plan *p, const void *psi, int axis, double k_l, i
     GPE_CHECK_DEVICE(p);
     return p->dtype == GPE_C64 ? populations_impl<float>(p, psi, axis, k_l, m_max, out)
                                : populations_impl<double>(p, psi, axis, k_l, m_max, out);
+}
+
+gpe_status gpe_measure_roofs(void *cuda_stream, double *out) {
+    if (!out) return GPE_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        g_create_error = "no CUDA device";
+        return GPE_ECUDA;
+    }
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return GPE_ECUDA;
+    gpe_status rc = GPE_OK;
+    void *buf = nullptr;
+    const size_t sizes[3] = {32u << 20, 64u << 20, 1024u << 20};
+    if (cudaMalloc(&buf, sizes[2]) != cudaSuccess) { cudaGetLastError(); cudaEventDestroy(e0); cudaEventDestroy(e1); g_create_error = "cudaMalloc failed"; return GPE_ENOMEM; }
+    cudaMemsetAsync(buf, 0, sizes[2], st);
+    for (int k = 0; k < 3; ++k) {
+        const size_t n4 = sizes[k] / 16;
+        const int reps = k < 2 ? 200 : 10;
+        double best = 0.0;
+        for (int trial = 0; trial < 3; ++trial) {
+            for (int w = 0; w < 3; ++w) k_roof_rw<<<nsm * 8, 256, 0, st>>>((float4 *)buf, n4, 0.f);
+            cudaEventRecord(e0, st);
+            for (int r = 0; r < reps; ++r) k_roof_rw<<<nsm * 8, 256, 0, st>>>((float4 *)buf, n4, 0.f);
+            cudaEventRecord(e1, st);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = GPE_ECUDA; break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            const double gbs = 2.0 * (double)sizes[k] * reps / (ms * 1e-3) / 1e9;
+            if (gbs > best) best = gbs;
+        }
+        out[k] = best;
+    }
+    for (int k = 0; k < 2 && rc == GPE_OK; ++k) {
+        const int iters = 4096, blocks = nsm * 8;
+        double best = 0.0;
+        for (int trial = 0; trial < 3; ++trial) {
+            if (k == 0) k_roof_fma<float><<<blocks, 256, 0, st>>>((float *)buf, 1.0000001f, 1e-9f, 64);
+            else k_roof_fma<double><<<blocks, 256, 0, st>>>((double *)buf, 1.0000001, 1e-9, 64);
+            cudaEventRecord(e0, st);
+            if (k == 0) k_roof_fma<float><<<blocks, 256, 0, st>>>((float *)buf, 1.0000001f, 1e-9f, iters);
+            else k_roof_fma<double><<<blocks, 256, 0, st>>>((double *)buf, 1.0000001, 1e-9, iters);
+            cudaEventRecord(e1, st);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = GPE_ECUDA; break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            const double tf = 2.0 * 32.0 * iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
+            if (tf > best) best = tf;
+        }
+        out[3 + k] = best;
+    }
+    if (cudaGetLastError() != cudaSuccess) rc = GPE_ECUDA;
+    cudaFree(buf);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return rc;
 }
 
 gpe_status gpe_get_step(const gpe_plan *p, long *step) {

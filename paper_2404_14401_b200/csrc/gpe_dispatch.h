@@ -1,7 +1,6 @@
 // gpe_dispatch.h -- table of per-(dtype, N) launchers.  Each (T, N) pair is compiled in its own
 // translation unit (gpe_inst.cu with -DGPE_T/-DGPE_N/-DGPE_TAG) so the build parallelises.
 #pragma once
-#include <cuda.h>
 #include "gpe_fft.cuh"
 #include "gpe_types.h"
 
@@ -18,12 +17,6 @@ template <typename T> struct Ops {
     cudaError_t (*p_row_inv)(const A &, bool imag, cudaStream_t);
     cudaError_t (*p_col)(const A &, bool imag, cudaStream_t);
     int p_rows_per_cta;
-    // persistent bulk-copy-fed passes (gpe_stream.cuh); null when not built for this (dtype, N)
-    cudaError_t (*s_col)(const A &, const CUtensorMap &, bool imag, int nsm, cudaStream_t);
-    int s_col_cpw;   // column pairs per tile (box width of the tensor map)
-    cudaError_t (*s_row_fwd)(const A &, bool imag, int nsm, cudaStream_t);
-    cudaError_t (*s_row_inv)(const A &, const CUtensorMap &, bool imag, int nsm, cudaStream_t);
-    int s_rows_per_tile;
 };
 
 #define GPE_DECL_OPS(N)                    \

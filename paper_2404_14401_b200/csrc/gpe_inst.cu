@@ -1,6 +1,6 @@
 // gpe_inst.cu -- one translation unit per (dtype, N): compile with
 //   -DGPE_T=float|double -DGPE_N=<64..2048> -DGPE_TAG=f|d
-#include "gpe_stream.cuh"
+#include "gpe_pair.cuh"
 #include "gpe_dispatch.h"
 
 #define GPE_CAT3_(a, b, c) a##b##_##c
@@ -19,23 +19,6 @@ template <int N> struct PairOps<float, N, true> {
     static constexpr auto col = &LaunchP<N>::col;
     static constexpr int rpc = RowGeomP<N>::RPC;
 };
-#ifndef GPE_STREAM_MIN_N
-#define GPE_STREAM_MIN_N 4096   // persistent passes (gpe_stream.cuh) off until validated on the GPU
-#endif
-template <typename T, int N, bool ON = (sizeof(T) == 4 && N >= GPE_STREAM_MIN_N)> struct StreamOps {
-    static constexpr decltype(Ops<T>::s_col) col = nullptr;
-    static constexpr int col_cpw = 0;
-    static constexpr decltype(Ops<T>::s_row_fwd) row_fwd = nullptr;
-    static constexpr decltype(Ops<T>::s_row_inv) row_inv = nullptr;
-    static constexpr int rpt = 0;
-};
-template <int N> struct StreamOps<float, N, true> {
-    static constexpr auto col = &LaunchS<N>::col;
-    static constexpr int col_cpw = ColGeomS<N>::CPW;
-    static constexpr auto row_fwd = &LaunchS<N>::row_fwd;
-    static constexpr auto row_inv = &LaunchS<N>::row_inv;
-    static constexpr int rpt = RowGeomS<N>::RPG;
-};
 extern const Ops<GPE_T> GPE_CAT3(ops_, GPE_TAG, GPE_N) = {
     &Launch<GPE_T, GPE_N>::row_fwd,
     &Launch<GPE_T, GPE_N>::row_inv,
@@ -45,10 +28,5 @@ extern const Ops<GPE_T> GPE_CAT3(ops_, GPE_TAG, GPE_N) = {
     PairOps<GPE_T, GPE_N>::row_inv,
     PairOps<GPE_T, GPE_N>::col,
     PairOps<GPE_T, GPE_N>::rpc,
-    StreamOps<GPE_T, GPE_N>::col,
-    StreamOps<GPE_T, GPE_N>::col_cpw,
-    StreamOps<GPE_T, GPE_N>::row_fwd,
-    StreamOps<GPE_T, GPE_N>::row_inv,
-    StreamOps<GPE_T, GPE_N>::rpt,
 };
 }  // namespace gpe

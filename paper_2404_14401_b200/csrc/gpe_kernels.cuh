@@ -149,13 +149,12 @@ __device__ __forceinline__ double warp_sum(double v) {
 // four at a time (ld.global.cg: L2, where the other CTAs' partials are after their fence) -- one
 // dependent L2 round trip per partial, as a volatile loop does, left a 3 us serial tail after pass C
 // at 2048^2 (1024 partials, 8 per thread) and 10 us in complex128 (32 per lane of one warp).
-// tid / nt: index of the calling thread among the nt threads that share the sum (a CTA, or one group of a
-// persistent CTA, gpe_stream.cuh)
-__device__ __forceinline__ void sum_partials_n(const FinalizeParams &f, int b, int tid, int nt, double &s0, double &s1, double &s2) {
+__device__ __forceinline__ void sum_partials(const FinalizeParams &f, int b, double &s0, double &s1, double &s2) {
     __threadfence();
     const double2 *pp = f.partials + (size_t)b * f.cpm;
+    const int nt = blockDim.x;
     s0 = 0.0; s1 = 0.0; s2 = 0.0;
-    for (int q0 = tid; q0 < f.cpm; q0 += 4 * nt) {
+    for (int q0 = threadIdx.x; q0 < f.cpm; q0 += 4 * nt) {
         double2 t[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) { const int q = q0 + k * nt; t[k] = q < f.cpm ? __ldcg(pp + q) : make_double2(0.0, 0.0); }
@@ -164,7 +163,7 @@ __device__ __forceinline__ void sum_partials_n(const FinalizeParams &f, int b, i
     }
     if (f.cav_u0) {
         const double *pb = f.partials_b + (size_t)b * f.cpm;
-        for (int q0 = tid; q0 < f.cpm; q0 += 4 * nt) {
+        for (int q0 = threadIdx.x; q0 < f.cpm; q0 += 4 * nt) {
             double u[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) { const int q = q0 + k * nt; u[k] = q < f.cpm ? __ldcg(pb + q) : 0.0; }
@@ -172,10 +171,6 @@ __device__ __forceinline__ void sum_partials_n(const FinalizeParams &f, int b, i
             for (int k = 0; k < 4; ++k) s2 += u[k];
         }
     }
-}
-
-__device__ __forceinline__ void sum_partials(const FinalizeParams &f, int b, double &s0, double &s1, double &s2) {
-    sum_partials_n(f, b, threadIdx.x, blockDim.x, s0, s1, s2);
 }
 
 // Block-level sum of (sn, st), one partial per CTA, last CTA of the member finalises.
