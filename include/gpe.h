@@ -57,7 +57,7 @@ typedef enum { GPE_REAL_TIME = 0, GPE_IMAG_TIME = 1 } gpe_mode; /* PAPER.md:112-
 typedef enum {
     GPE_OK = 0,
     GPE_EINVAL = 1,       /* bad argument (NULL, non-finite, misaligned, wrong size) */
-    GPE_EUNSUPPORTED = 2, /* nx or ny not a power of two in [64, 2048] */
+    GPE_EUNSUPPORTED = 2, /* nx or ny outside the supported sizes (see gpe_plan_create) */
     GPE_ENOMEM = 3,       /* host or device allocation failed */
     GPE_ECUDA = 4,        /* a CUDA runtime call failed (text in gpe_last_error) */
     GPE_ESTATE = 5,       /* call order: gpe_evolve / gpe_observables before gpe_set_potential */
@@ -73,8 +73,11 @@ typedef enum {
 /*
  * gpe_plan_create -- the discretised problem of Eq. 1: an nx x ny periodic grid
  * over the box [-Lx/2, Lx/2) x [-Ly/2, Ly/2), `batch` independent wavefunctions (parameter
- * sweeps, north_star (4)).  nx, ny powers of two in [64, 2048] (the paper benchmarks powers of
- * two), else GPE_EUNSUPPORTED; Lx, Ly > 0 and finite, batch >= 1, else GPE_EINVAL.
+ * sweeps, north_star (4)).  nx, ny in [64, 2048], even, with no prime factor above 5, else
+ * GPE_EUNSUPPORTED.  Powers of two run the fast kernels (the paper benchmarks powers of two and notes
+ * only that other sizes are slower); any other allowed size runs mixed-radix passes
+ * (radices 8, 5, 4, 3, 2), about an order of magnitude slower per point, without ordering = 1 and
+ * without gpe_profile_passes.  Lx, Ly > 0 and finite, batch >= 1, else GPE_EINVAL.
  * Allocates the twiddle / wavenumber tables and the per-member device scalars on the current
  * device.  *out is set only on GPE_OK and is released with gpe_plan_destroy.
  */

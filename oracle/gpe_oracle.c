@@ -143,9 +143,11 @@ static void fft_radix2(cplx_t *a, int n, int sign)
     }
 }
 
+/* Lengths that are not powers of two ("non-optimal grid sizes") take the
+ * plain definition of the transform, dft_direct: O(n^2), no factorisation to get wrong. */
 static void fft_1d(cplx_t *a, int n, int sign, int force_direct)
 {
-    if (n <= 16 || force_direct) dft_direct(a, n, sign);
+    if (n <= 16 || force_direct || (n & (n - 1)) != 0) dft_direct(a, n, sign);
     else fft_radix2(a, n, sign);
 }
 

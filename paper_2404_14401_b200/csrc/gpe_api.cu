@@ -13,12 +13,13 @@
 #include "../../include/gpe.h"
 #include "gpe_dispatch.h"
 #include "gpe_kernels.cuh"
+#include "gpe_mixed.cuh"
 
 using namespace gpe;
 
 namespace {
 
-constexpr int kMaxCpm = 1024;   // partial-sum slots per member
+constexpr int kMaxCpm = 2048;   // partial-sum slots per member (one per row in the mixed-radix family)
 constexpr int kReduceCtas = 1024;  // CTAs per member of the prologue reduction
 constexpr int kStepsPerGraph = 8;  // split-steps per CUDA graph launch
 constexpr double kPi = 3.14159265358979323846;
@@ -38,7 +39,11 @@ struct gpe_plan {
     int device = 0;            // the device the plan was created on; every call checks it is current
     // test hooks, read ONCE at gpe_plan_create from the environment (tests/test_gpu_parity.py):
     // GPE_NO_PAIR = one-number-per-element kernels for complex64 too, GPE_NO_MERGE = separate half-steps
-    bool no_pair = false, no_merge = false;
+    bool no_pair = false, no_merge = false, no_fuse = false;   // GPE_NO_FUSE: never the 2-pass form
+    bool no_chip = false;      // GPE_NO_CHIP: never the one-launch cluster kernel of gpe_chip.cuh
+    int chip_ok = -1;          // -1 not asked yet; 1 a cluster of that shape fits this device
+    bool mixed = false;        // nx or ny is not a power of two: the mixed-radix family (gpe_mixed.cuh)
+    MixPlan plx = {}, ply = {};
 
     // device tables (typed by dtype)
     void *tw_x = nullptr, *tw_y = nullptr;
@@ -84,6 +89,7 @@ struct gpe_plan {
     const void *g_psi = nullptr;
     double g_dt = 0.0;
     int g_mode = -1;
+    int g_fused = -1;          // the cached graph holds (B, CA) pairs of the 2-pass form
     long g_epoch = -1;
     long epoch = 0;  // bumped whenever device tables / flags may have changed
 
@@ -129,6 +135,19 @@ gpe_status check_device(gpe_plan *p) {
     } while (0)
 
 bool pow2_in_range(int n) { return n >= 64 && n <= 2048 && (n & (n - 1)) == 0; }
+// even, no prime factor above 5
+bool smooth_even_in_range(int n) {
+    if (n < 64 || n > 2048 || (n & 1)) return false;
+    for (int f : {2, 3, 5}) while (n % f == 0) n /= f;
+    return n == 1;
+}
+// radices of the Stockham stages: 8 while it divides, then 5, 4 (only when 8 no longer divides), 3, 2
+MixPlan make_mix_plan(int n) {
+    MixPlan pl = {};
+    for (int r : {8, 5, 4, 3, 2})
+        while (n % r == 0 && pl.nr < 12) { pl.radix[pl.nr++] = r; n /= r; }
+    return pl;
+}
 
 double coord(int i, int n, double L) { return -0.5 * L + (double)i * L / (double)n; }
 double wavenumber(int q, int n, double L) { return 2.0 * kPi * (double)(q < n / 2 ? q : q - n) / L; }
@@ -537,6 +556,31 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
                                                  (const T *)p->cavy, p->cavity_on, f);
         GPE_CUDA(p, cudaGetLastError());
     }
+    if (p->mixed) {
+        // sizes that are not powers of two: the mixed-radix passes of gpe_mixed.cuh, three
+        // launches per step, natural layout, separate half-steps
+        if (tvt || prof) return fail(p, GPE_EUNSUPPORTED, "ordering = 1 and per-pass profiling need power-of-two sizes");
+        a.fin.cpm = p->nx;   // one row per CTA in pass C
+        a.fin.normalise = imag ? 1 : 0;
+        a.fin.advance = 1;
+        a.fin.prepared = p->d_u0 ? 0 : 1;
+        a.fin.merged = 0;
+        a.fin.record_every = 0; a.fin.rec_first = 0; a.fin.records = nullptr;
+        for (long n = 0; n < n_steps; ++n) {
+            GPE_CUDA(p, LaunchMix<T>::row_fwd(a, p->ply, imag, p->stream));
+            GPE_CUDA(p, LaunchMix<T>::col(a, p->plx, imag, 0, p->stream));
+            GPE_CUDA(p, LaunchMix<T>::row_inv(a, p->ply, imag, p->stream));
+        }
+        if (imag) {
+            dim3 grid(256, p->batch);
+            k_rescale<T><<<grid, 256, 0, p->stream>>>((cx<T> *)psi, (size_t)p->nx * p->ny, p->st);
+            GPE_CUDA(p, cudaGetLastError());
+            k_reset_scale<<<(p->batch + 127) / 128, 128, 0, p->stream>>>(p->st, p->batch);
+            GPE_CUDA(p, cudaGetLastError());
+        }
+        p->step += n_steps;
+        return GPE_OK;
+    }
     // complex64 hot path: paired passes (gpe_pair.cuh) when built for both axis lengths
     const bool paired = oy->p_row_fwd && ox->p_col && !p->no_pair;
     a.fin.cpm = p->nx / (paired ? oy->p_rows_per_cta : oy->rows_per_cta);
@@ -646,12 +690,72 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
         p->step += n_steps;
         return GPE_OK;
     }
-    long n = 0;
-    if (!prof && n_steps >= 2 * kStepsPerGraph) {
+    // Small square grids (64^2 .. 256^2): every step of the call inside ONE cluster kernel (gpe_chip.cuh).
+    bool chip_done = false;
+    if (!prof && !p->no_chip && !p->no_pair && p->nx == p->ny && oy->chip) {
+        if (p->chip_ok < 0) p->chip_ok = oy->chip_available() ? 1 : 0;
+        if (p->chip_ok == 1) {
+            a.src = (const cx<T> *)psi; a.dst = (cx<T> *)psi;
+            GPE_CUDA(p, oy->chip(a, imag, n_steps, p->stream));
+            chip_done = true;
+        }
+    }
+    // 2-pass form ("fused pass structure"): A B (CA B)^(n-1) C, with CA = pass C of one step and
+    // pass A of the next in one kernel (k_row_ca_p / k_row_ca).  Allowed when the potential factor between two
+    // kinetic steps needs no global scalar of the array it multiplies: real time without the cavity term
+    // (merged half-steps), or imaginary time with g = 0 and no cavity term (a linear step: the per-step
+    // renormalisation commutes with it; the plain pass C that ends every call makes the final norm exact).
+    const bool fused = !chip_done && !prof && !p->no_fuse && n_steps >= 2 && !(p->flags & F_CAVITY) &&
+                       (imag ? !(p->flags & F_HAS_G) : a.fin.merged == 1) && a.fin.prepared == 1 &&
+                       (paired ? oy->p_row_ca != nullptr : oy->row_ca != nullptr);
+    if (fused) {
+        auto pass_ca = [&](const StepArgs<T, cx<T>> &u, cudaStream_t st) -> cudaError_t {
+            return paired ? oy->p_row_ca(u, imag, st) : oy->row_ca(u, imag, st);
+        };
+        cx<T> *mid = oop ? (cx<T> *)p->scratch : (cx<T> *)psi;
+        a.src = (const cx<T> *)psi; a.dst = mid;
+        GPE_CUDA(p, pass_a(a, p->stream));
+        a.src = mid;
+        auto pairs = [&](cudaStream_t st, int count) -> gpe_status {
+            for (int u = 0; u < count; ++u) {
+                GPE_CUDA(p, pass_b(a, st));
+                GPE_CUDA(p, pass_ca(a, st));
+            }
+            return GPE_OK;
+        };
+        long done = 0;
+        const long npairs = n_steps - 1;
+        if (npairs >= 2 * kStepsPerGraph + 1) {
+            if (!(p->g_exec && p->g_psi == psi && p->g_dt == dt && p->g_mode == (int)mode && p->g_epoch == p->epoch && p->g_fused == 1)) {
+                if (p->g_exec) { cudaGraphExecDestroy(p->g_exec); p->g_exec = nullptr; }
+                if (!p->cap_stream) GPE_CUDA(p, cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
+                if ((s = pairs(p->stream, 1)) != GPE_OK) return s;   // one-time function attributes outside the capture
+                done = 1;
+                GPE_CUDA(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
+                const gpe_status cs = pairs(p->cap_stream, kStepsPerGraph);
+                cudaGraph_t graph = nullptr;
+                cudaError_t ce = cudaStreamEndCapture(p->cap_stream, &graph);
+                if (cs != GPE_OK) { if (graph) cudaGraphDestroy(graph); return cs; }
+                if (ce != cudaSuccess) return cuda_fail(p, ce, "cudaStreamEndCapture");
+                ce = cudaGraphInstantiate(&p->g_exec, graph, 0);
+                cudaGraphDestroy(graph);
+                if (ce != cudaSuccess) { p->g_exec = nullptr; return cuda_fail(p, ce, "cudaGraphInstantiate"); }
+                p->g_psi = psi; p->g_dt = dt; p->g_mode = (int)mode; p->g_epoch = p->epoch; p->g_fused = 1;
+            }
+            for (; done + kStepsPerGraph <= npairs; done += kStepsPerGraph) GPE_CUDA(p, cudaGraphLaunch(p->g_exec, p->stream));
+        }
+        if ((s = pairs(p->stream, (int)(npairs - done))) != GPE_OK) return s;
+        GPE_CUDA(p, pass_b(a, p->stream));
+        a.dst = (cx<T> *)psi;
+        GPE_CUDA(p, pass_c(a, p->stream));
+        a.src = (const cx<T> *)psi;
+    }
+    long n = (fused || chip_done) ? n_steps : 0;
+    if (n == 0 && !prof && n_steps >= 2 * kStepsPerGraph) {
         // The arguments of the three passes do not depend on the step (all per-step state is on the
         // device), so kStepsPerGraph steps are captured once into a CUDA graph and replayed: one
         // host call per 3 * kStepsPerGraph kernels instead of one per kernel.
-        if (!(p->g_exec && p->g_psi == psi && p->g_dt == dt && p->g_mode == (int)mode && p->g_epoch == p->epoch)) {
+        if (!(p->g_exec && p->g_psi == psi && p->g_dt == dt && p->g_mode == (int)mode && p->g_epoch == p->epoch && p->g_fused == 0)) {
             if (p->g_exec) { cudaGraphExecDestroy(p->g_exec); p->g_exec = nullptr; }
             if (!p->cap_stream) GPE_CUDA(p, cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
             // first launches outside the capture: one-time function attributes are not stream work
@@ -667,7 +771,7 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
             ce = cudaGraphInstantiate(&p->g_exec, graph, 0);
             cudaGraphDestroy(graph);
             if (ce != cudaSuccess) { p->g_exec = nullptr; return cuda_fail(p, ce, "cudaGraphInstantiate"); }
-            p->g_psi = psi; p->g_dt = dt; p->g_mode = (int)mode; p->g_epoch = p->epoch;
+            p->g_psi = psi; p->g_dt = dt; p->g_mode = (int)mode; p->g_epoch = p->epoch; p->g_fused = 0;
         }
         for (; n + kStepsPerGraph <= n_steps; n += kStepsPerGraph) GPE_CUDA(p, cudaGraphLaunch(p->g_exec, p->stream));
     }
@@ -714,6 +818,12 @@ template <typename T> gpe_status fft_to_scratch(gpe_plan *p, const void *psi) {
     const Ops<T> *oy = get_ops<T>(p->ny), *ox = get_ops<T>(p->nx);
     StepArgs<T, cx<T>> a = base_args<T>(p, psi, p->scratch);
     a.flags |= F_NO_POT;
+    if (p->mixed) {
+        GPE_CUDA(p, LaunchMix<T>::row_fwd(a, p->ply, false, p->stream));
+        a.src = (const cx<T> *)p->scratch;
+        GPE_CUDA(p, LaunchMix<T>::col(a, p->plx, false, 1, p->stream));
+        return GPE_OK;
+    }
     GPE_CUDA(p, oy->row_fwd(a, false, p->stream));
     a.src = (const cx<T> *)p->scratch;
     GPE_CUDA(p, ox->col(a, false, 1, p->stream));
@@ -899,11 +1009,14 @@ gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly,
     if (nx <= 0 || ny <= 0 || batch < 1 || !(Lx > 0) || !(Ly > 0) || !std::isfinite(Lx) || !std::isfinite(Ly))
         return fail(nullptr, GPE_EINVAL, "nx, ny, batch must be positive and Lx, Ly finite and > 0");
     if (dtype != GPE_C64 && dtype != GPE_C128) return fail(nullptr, GPE_EINVAL, "unknown dtype");
-    if (!pow2_in_range(nx) || !pow2_in_range(ny))
-        return fail(nullptr, GPE_EUNSUPPORTED, "nx and ny must be powers of two in [64, 2048]");
+    if (!smooth_even_in_range(nx) || !smooth_even_in_range(ny))
+        return fail(nullptr, GPE_EUNSUPPORTED, "nx and ny must be even numbers in [64, 2048] with no prime factor above 5 "
+                                                "(powers of two run the fast kernels)");
     gpe_plan *p = new (std::nothrow) gpe_plan();
     if (!p) return fail(nullptr, GPE_ENOMEM, "out of host memory");
     p->nx = nx; p->ny = ny; p->batch = batch; p->Lx = Lx; p->Ly = Ly; p->dtype = dtype;
+    p->mixed = !pow2_in_range(nx) || !pow2_in_range(ny);
+    p->plx = make_mix_plan(nx); p->ply = make_mix_plan(ny);
     gpe_status s = GPE_OK;
     auto body = [&]() -> gpe_status {
         int dev_count = 0;
@@ -912,6 +1025,8 @@ gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly,
         GPE_CUDA(p, cudaGetDevice(&p->device));
         p->no_pair = getenv("GPE_NO_PAIR") != nullptr;     // test hooks, read once (see struct gpe_plan)
         p->no_merge = getenv("GPE_NO_MERGE") != nullptr;
+        p->no_fuse = getenv("GPE_NO_FUSE") != nullptr;
+        p->no_chip = getenv("GPE_NO_CHIP") != nullptr;
         // kinetic tables at their largest (complex) size: gpe_evolve fills them with a kernel and never
         // allocates (an allocation may synchronise the device)
         const size_t rb = dtype == GPE_C64 ? 4 : 8;

@@ -17,6 +17,12 @@ template <typename T> struct Ops {
     cudaError_t (*p_row_inv)(const A &, bool imag, cudaStream_t);
     cudaError_t (*p_col)(const A &, bool imag, cudaStream_t);
     int p_rows_per_cta;
+    // pass C of step n fused with pass A of step n+1 (the 2-pass form): both kernel families
+    cudaError_t (*row_ca)(const A &, bool imag, cudaStream_t);
+    cudaError_t (*p_row_ca)(const A &, bool imag, cudaStream_t);
+    // small square grids: all steps of a call in one cluster kernel (gpe_chip.cuh); null above 256
+    cudaError_t (*chip)(const A &, bool imag, long n_steps, cudaStream_t);
+    bool (*chip_available)();
 };
 
 #define GPE_DECL_OPS(N)                    \

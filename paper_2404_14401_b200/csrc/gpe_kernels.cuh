@@ -551,6 +551,48 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
     }
 }
 
+// ---------------------------------------------------------------- pass C of step n fused with pass A of step n+1
+// The 2-pass form (see k_row_ca_p in gpe_pair.cuh for when it applies and why the imaginary-time scale may lag
+// one step): load -> IFFT_y -> sum |psi|^2 -> both potential half-steps in one multiply -> FFT_y -> store.
+// The member's coefficients are read before the sums are published (the last CTA advances the state).
+template <typename T, int NY, bool IMAG>
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1))) k_row_ca(const StepArgs<T, cx<T>> a) {
+    using C = cx<T>;
+    using F = Fft1D<NY, 1, cx<T>>;
+    using G = RowGeom<NY>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *smem = reinterpret_cast<C *>(smem_raw);
+    __shared__ double red[96];
+    const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
+    C *sm = smem + r * F::SLOTS;
+    const int gpm = a.nx / G::RPC;
+    pdl_launch_dependents();
+    pdl_wait();
+    const long grp = blockIdx.x;
+    const long row = grp * G::RPC + r;
+    const int b = (int)(row / a.nx), i = (int)(row % a.nx);
+    const MemberState &ms = a.fin.st[b];
+    const T Asum = (T)(ms.A + ms.nA), scale = (T)ms.scale;
+    C *dst = a.dst + row * NY;
+    const C *src = a.src + row * NY;
+    C v[16];
+#pragma unroll
+    for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+        for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = __ldcg(src + F::nat(j, ii, rr));
+    F::inv(v, sm, j, a.tw_y, a.tw1_y);
+    T sn = T(0), st = T(0);
+#pragma unroll
+    for (int k = 0; k < 16; ++k) sn += v[k].x * v[k].x + v[k].y * v[k].y;
+    block_reduce_and_finalize(a.fin, b, (int)(grp % gpm), (double)sn, 0.0, 0.0, red);
+    potential_step16<T, IMAG, false, F::M1>(v, a, b, i, j, scale, T(2), Asum, T(0), T(0), sn, st);
+    F::fwd(v, sm, j, a.tw_y, a.tw1_y);
+#pragma unroll
+    for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+        for (int rr = 0; rr < F::RL; ++rr) dst[F::nat(j, ii, rr)] = v[ii * F::RL + rr];
+}
+
 // ---------------------------------------------------------------- launchers (one per T, N)
 template <typename T, int N> struct Launch {
     using C = cx<T>;
@@ -603,6 +645,16 @@ template <typename T, int N> struct Launch {
         };
         if (imag) return go(k_row_inv<T, N, true, false>);
         return a.fin.merged ? go(k_row_inv<T, N, false, true>) : go(k_row_inv<T, N, false, false>);
+    }
+    static cudaError_t row_ca(const A &a, bool imag, cudaStream_t s) {
+        dim3 grid(row_grid(a)), block(RowGeom<N>::THREADS);
+        auto go = [&](auto kern) -> cudaError_t {
+            cudaError_t e = prep(kern, row_smem());
+            if (e != cudaSuccess) return e;
+            e = launch_pdl(kern, grid, block, row_smem(), s, use_pdl(a), a);
+            return e != cudaSuccess ? e : cudaGetLastError();
+        };
+        return imag ? go(k_row_ca<T, N, true>) : go(k_row_ca<T, N, false>);
     }
     // nx == N
     static cudaError_t col(const A &a, bool imag, int mode, cudaStream_t s) {

@@ -446,6 +446,141 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     }
 }
 
+// ---------------------------------------------------------------- pass C of step n fused with pass A of step n+1
+// The 2-pass form of SURVEY.md 8(a): when the potential factor between two kinetic steps needs no global
+// scalar of the array it acts on, the rows never leave the SM between the inverse transform along y of
+// step n and the forward transform along y of step n+1:
+//   load (intermediate layout) -> IFFT_y -> partial sums of |psi|^2 -> psi *= exp(-s (V_n + V_{n+1} + 2 g|psi|^2) dt/2)
+//   -> FFT_y -> store (intermediate layout, in place).
+//   real time, no cavity term (a phase leaves |psi|^2 alone, and without Eq. 14 nothing else
+//     couples the points): both half-steps in one multiply, exactly the merged multiply of pass A;
+//   imaginary time with g = 0 and no cavity term (the paper's own benchmark workload): the
+//     step is linear, so the renormalisation of PAPER.md:116 commutes with it.  The 1/||psi|| applied here is the
+//     one of the PREVIOUS step (it only keeps the magnitudes near one); the last step of every gpe_evolve is the
+//     plain pass C, whose norm and final rescale are exact.
+// A_n is the member's current coefficient, A_{n+1} the one prepare_member left in nA during pass B; both are
+// read BEFORE this CTA publishes its partial sums, because the last CTA to publish advances the member's state.
+template <int NY, bool IMAG, bool LATE>
+__global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) / RowGeomP<NY>::THREADS) k_row_ca_p(const StepArgs<float, float2> a) {
+    using G = RowGeomP<NY>;
+    using F = Fft1D<G::H, 1, cpair>;
+    constexpr int H = G::H, M1 = F::M1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[96];
+    const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw) + r * F::TILE;
+    const long row = (long)blockIdx.x * G::RPC + r;
+    const int b = (int)(row / a.nx), i = (int)(row % a.nx), il = il_of<NY>(a.nx, a.batch);
+    const int gpm = a.nx / G::RPC;
+    const cpair *src = reinterpret_cast<const cpair *>(a.src);
+    cpair *dst = reinterpret_cast<cpair *>(a.dst);
+    if constexpr (!LATE) pdl_launch_dependents();
+    pdl_wait();
+    const MemberState &ms = a.fin.st[b];
+    const float Asum = (float)(ms.A + ms.nA), scale = (float)ms.scale;
+    cpair v[16];
+    const int rp = r >> 1, u = j + (r & 1) * G::TPF;
+    float2 *sm0 = reinterpret_cast<float2 *>(smem_raw) + (2 * rp) * F::TILE, *sm1 = sm0 + F::TILE;
+    const long rowp = (long)blockIdx.x * G::RPC + 2 * rp;
+    auto sync_row = [r] { if constexpr (G::NAMED) bar_named(1 + r, G::TPF); else __syncthreads(); };
+    auto sync_pair = [rp] { if constexpr (G::PAIRNAMED) bar_named(9 + rp, 2 * G::TPF); else __syncthreads(); };
+    if constexpr (G::PAIRMAP) {
+#pragma unroll
+        for (int ii = 0; ii < F::GL / 2; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) {
+                const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H, il);
+                ldcg_pair2(src + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
+            }
+        F::inv_pairfirst(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, sync_row, sync_pair);
+    } else {
+#pragma unroll
+        for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) v[ii * F::RL + rr] = ldcg_pair(src + ipos(row, F::nat(j, ii, rr), H, il));
+        if constexpr (G::NAMED) F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
+        else F::inv(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+    }
+    float2 p0[16], p1[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const float2 w = ldtw(a.tw_y, j + M1 * k);
+        const float tx = fmaf(v[k].re.y, w.x, v[k].im.y * w.y), ty = fmaf(v[k].im.y, w.x, -(v[k].re.y * w.y));
+        p0[k] = make_float2(v[k].re.x + tx, v[k].im.x + ty);
+        p1[k] = make_float2(v[k].re.x - tx, v[k].im.x - ty);
+    }
+    // partial sums of the array as it stands (norm of psi_{n+1} in real time; records), published at once
+    float2 sn, st;
+    reduce_pair16<M1>(p0, p1, a, j, sn, st);
+    const FinalizeParams &f = a.fin;
+    const int cim = (int)(blockIdx.x % gpm);
+    double dn = warp_sum((double)sn.x + (double)sn.y);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    constexpr int NW = G::THREADS / 32;
+    __shared__ int is_last;
+    if (lane == 0) red[wid] = dn;
+    __syncthreads();
+    unsigned int old = 0;
+    if (threadIdx.x == 0) {
+        double s0 = 0.0;
+#pragma unroll
+        for (int q = 0; q < NW; ++q) s0 += red[q];
+        f.partials[(size_t)b * f.cpm + cim] = make_double2(s0, 0.0);
+        __threadfence();
+        old = atomicAdd(&f.counters[b], 1u);
+    }
+    // both potential half-steps in one multiply, then pass A's radix-2 layer and forward transform
+    {
+        float2 dn_, dt_;
+        potential_pair16<IMAG, false, M1, H>(p0, p1, a, b, i, j, scale, 2.f, Asum, 0.f, 0.f, dn_, dt_);
+    }
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const float2 w = ldtw(a.tw_y, j + M1 * k);
+        const float dx = p0[k].x - p1[k].x, dy = p0[k].y - p1[k].y;
+        v[k].re = make_float2(p0[k].x + p1[k].x, fmaf(dx, w.x, -(dy * w.y)));
+        v[k].im = make_float2(p0[k].y + p1[k].y, fmaf(dx, w.y, dy * w.x));
+    }
+    if constexpr (G::PAIRMAP) {
+        F::fwd_pairlast(v, sm, sm0, sm1, j, u, a.tw_hy, a.tw1_hy, sync_row, sync_pair);
+#pragma unroll
+        for (int ii = 0; ii < F::GL / 2; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) {
+                const size_t pos = ipos(rowp, F::nat_t(u + 2 * G::TPF * ii, rr), H, il);
+                st_pair2(dst + pos, v[(2 * ii) * F::RL + rr], v[(2 * ii + 1) * F::RL + rr]);
+            }
+    } else {
+        // in place: every row of the CTA was loaded before the first barrier of the inverse transform
+        if constexpr (G::NAMED) F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [r] { bar_named(1 + r, G::TPF); });
+        else F::fwd(v, sm, j, a.tw_hy, a.tw1_hy, [] { __syncthreads(); });
+#pragma unroll
+        for (int ii = 0; ii < F::GL; ++ii)
+#pragma unroll
+            for (int rr = 0; rr < F::RL; ++rr) st_pair(dst + ipos(row, F::nat(j, ii, rr), H, il), v[ii * F::RL + rr]);
+    }
+    if constexpr (LATE) pdl_launch_dependents();
+    if (threadIdx.x == 0) is_last = (old == (unsigned int)(f.cpm - 1));
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        const volatile double2 *pp = f.partials + (size_t)b * f.cpm;
+        double s0 = 0.0;
+        for (int q = threadIdx.x; q < f.cpm; q += G::THREADS) s0 += pp[q].x;
+        s0 = warp_sum(s0);
+        __syncthreads();
+        if (lane == 0) red[wid] = s0;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t0 = 0.0;
+#pragma unroll
+            for (int q = 0; q < NW; ++q) t0 += red[q];
+            finalize_member(f, b, t0, 0.0, 0.0);
+            f.counters[b] = 0u;
+        }
+    }
+}
+
 // ---------------------------------------------------------------- launchers
 template <int N> struct LaunchP {
     using A = StepArgs<float, float2>;
@@ -482,6 +617,11 @@ template <int N> struct LaunchP {
         }
         if (imag) return go(k_row_inv_p<N, true, false, false>, grid, block, row_smem(), s, a);
         return a.fin.merged ? go(k_row_inv_p<N, false, true, false>, grid, block, row_smem(), s, a) : go(k_row_inv_p<N, false, false, false>, grid, block, row_smem(), s, a);
+    }
+    static cudaError_t row_ca(const A &a, bool imag, cudaStream_t s) {   // ny == N
+        dim3 grid((unsigned)((long)a.batch * a.nx / RowGeomP<N>::RPC)), block(RowGeomP<N>::THREADS);
+        if (late(a)) return imag ? go(k_row_ca_p<N, true, true>, grid, block, row_smem(), s, a) : go(k_row_ca_p<N, false, true>, grid, block, row_smem(), s, a);
+        return imag ? go(k_row_ca_p<N, true, false>, grid, block, row_smem(), s, a) : go(k_row_ca_p<N, false, false>, grid, block, row_smem(), s, a);
     }
     static cudaError_t col(const A &a, bool imag, cudaStream_t s) {       // nx == N
         dim3 grid((unsigned)(a.ny / 2 / ColGeomP<N>::CPW), (unsigned)a.batch), block(ColGeomP<N>::THREADS);

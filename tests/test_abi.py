@@ -51,7 +51,7 @@ def test_sass_is_sm100(lib):
 def test_validation_without_device():
     import paper_2404_14401_b200 as G
     with pytest.raises(G.GpeError) as e:
-        G.gpe_plan_create(100, 64, 1.0, 1.0, G.GPE_C64, 1)
+        G.gpe_plan_create(98, 64, 1.0, 1.0, G.GPE_C64, 1)
     assert e.value.status == 2 and "power" in str(e.value)
     with pytest.raises(G.GpeError) as e:
         G.gpe_plan_create(64, 64, 0.0, 1.0, G.GPE_C64, 1)

@@ -311,3 +311,110 @@ def test_evolve_only_enqueues(ordering):
         o.evolve(ref, dt, n, mode == "imag")
     assert _rel(psi.cpu().numpy(), ref) <= 13 * PER_STEP["c64"]      # the tables built on the device are right
     plan.close()
+
+
+def _local_workload(nx, ny, batch=1, g=40.0, v2d=False):
+    """No cavity term: static trap (+ optional 2-D array), ramped lattice, contact interaction."""
+    p = _general_workload(nx, ny, batch=batch)
+    p["cavity_on"] = 0
+    p["g"] = np.linspace(g, 1.5 * g, batch)
+    if not v2d:
+        p["v_static"] = None
+    return p
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("nx,ny,batch", [(64, 64, 1), (256, 256, 1), (128, 512, 2), (1024, 128, 1), (2048, 2048, 1)])
+def test_two_pass_real_time(monkeypatch, nx, ny, batch, dtype):
+    """The 2-pass form (real time with a local potential runs IFFT_y -> full potential factor
+    -> FFT_y in one kernel): psi and the records against the oracle for step counts on both sides of the
+    CUDA-graph threshold, over two calls, and against the 3-pass form of the same library (GPE_NO_FUSE)."""
+    torch = _torch()
+    for k in ("GPE_NO_PAIR", "GPE_NO_MERGE", "GPE_NO_FUSE"):
+        monkeypatch.delenv(k, raising=False)
+    big = nx * ny >= 2048 * 2048
+    p = _local_workload(nx, ny, batch, v2d=(nx == 256))
+    counts = (2, 5) if big else (3, 40)
+    ref = _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    ro = np.concatenate([o.evolve(ref, 1e-3, n, False, record_every=1) for n in counts])
+    outs = []
+    for fuse in (True, False):
+        if not fuse:
+            monkeypatch.setenv("GPE_NO_FUSE", "1")
+        plan = _gpu_plan(p, dtype, use_separable=(nx != 256))
+        psi = _to_dev(p["psi0"], dtype)
+        rg = np.concatenate([plan.evolve(psi, 1e-3, n, "real", record_every=1).cpu().numpy()[:n] for n in counts])
+        torch.cuda.synchronize()
+        out = psi.cpu().numpy()
+        e = _rel(out, ref)
+        assert e <= sum(counts) * PER_STEP[dtype], f"fuse={fuse}: {e:.3e}"
+        assert np.array_equal(rg[:, :, 0], ro[:, :, 0])
+        tol = 1e-5 if dtype == "c64" else 1e-10
+        assert np.allclose(rg[:, :, 1], ro[:, :, 1], rtol=tol, atol=0)          # the computed norm, every step
+        assert np.allclose(rg[:, :, 5], ro[:, :, 5], rtol=1e-14, atol=1e-300)
+        assert plan.step == sum(counts)
+        outs.append(out)
+        plan.close()
+    assert _rel(outs[0], outs[1].astype(np.complex128)) <= (2e-6 if dtype == "c64" else 1e-13)
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("n", [64, 128, 512, 2048])
+def test_two_pass_imag_time_linear(monkeypatch, n, dtype):
+    """The 2-pass form in imaginary time with g = 0 and no cavity term (the paper's Sec. 4.1 workload,
+    PAPER.md:130-132): the lagging lazy scale must not change the result -- psi after a run that ends in the
+    plain pass C is the oracle's (renormalised every step), norm 1, same energies."""
+    monkeypatch.delenv("GPE_NO_FUSE", raising=False)
+    p = W.sweep_s(n, dtype)
+    steps = 6 if n == 2048 else 60
+    plan = _gpu_plan(p, dtype)
+    psi, ref = _to_dev(p["psi0"], dtype), _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    rec = plan.evolve(psi, 1e-3, steps, "imag", record_every=3).cpu().numpy()
+    o.evolve(ref, 1e-3, steps, True)
+    e = _rel(psi.cpu().numpy(), ref)
+    assert e <= min(steps, 20) * PER_STEP[dtype], f"{e:.3e}"
+    assert np.allclose(rec[:, :, 1], 1.0, atol=1e-12)
+    go, oo = plan.observables(psi)[0][0], o.observables(ref)[0][0]
+    tol = 1e-5 if dtype == "c64" else 1e-10
+    assert abs(go["norm"] - 1.0) <= (2e-6 if dtype == "c64" else 1e-13)
+    for k in ("e_kin", "e_pot"):
+        assert abs(go[k] - oo[k]) <= tol * abs(oo[k]), k
+    plan.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+@pytest.mark.parametrize("mode", ["real", "imag"])
+@pytest.mark.parametrize("n,batch", [(64, 1), (128, 3), (256, 1)])
+def test_cluster_kernel_and_multi_launch_path_agree(monkeypatch, n, batch, mode, dtype):
+    """Square grids up to 256^2 run all steps of a call in one cluster kernel (gpe_chip.cuh); GPE_NO_CHIP
+    forces the multi-launch passes for the same sizes.  Both against the oracle (everything switched on:
+    2-D array, lattice ramp, cavity, g; records every step, two calls), and against each other."""
+    torch = _torch()
+    for k in ("GPE_NO_PAIR", "GPE_NO_MERGE", "GPE_NO_FUSE", "GPE_NO_CHIP"):
+        monkeypatch.delenv(k, raising=False)
+    p = _general_workload(n, n, batch=batch)
+    ref = _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    counts = (1, 24)
+    ro = np.concatenate([o.evolve(ref, 1e-3, c, mode == "imag", record_every=1) for c in counts])
+    outs = []
+    for chip in (True, False):
+        if not chip:
+            monkeypatch.setenv("GPE_NO_CHIP", "1")
+        plan = _gpu_plan(p, dtype, use_separable=False)
+        psi = _to_dev(p["psi0"], dtype)
+        rg = np.concatenate([plan.evolve(psi, 1e-3, c, mode, record_every=1).cpu().numpy()[:c] for c in counts])
+        torch.cuda.synchronize()
+        out = psi.cpu().numpy()
+        e = _rel(out, ref)
+        assert e <= 25 * PER_STEP[dtype], f"chip={chip}: {e:.3e}"
+        tol = 1e-5 if dtype == "c64" else 1e-10
+        assert np.array_equal(rg[:, :, 0], ro[:, :, 0])
+        for c in (1, 2, 3, 4, 5):
+            assert np.all(np.abs(rg[:, :, c] - ro[:, :, c]) <= tol * np.maximum(np.abs(ro[:, :, c]), 1e-2)), (chip, c)
+        assert plan.step == 25
+        outs.append(out)
+        plan.close()
+    assert _rel(outs[0], outs[1].astype(np.complex128)) <= (5e-6 if dtype == "c64" else 1e-13)

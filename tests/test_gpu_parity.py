@@ -499,7 +499,7 @@ def test_runs_are_bitwise_reproducible(nx, ny, batch, mode):
 def test_error_behaviour():
     import paper_2404_14401_b200 as G
     torch = _torch()
-    for bad in ((100, 64), (64, 4096), (32, 64)):
+    for bad in ((98, 64), (64, 4096), (32, 64), (75, 64)):
         with pytest.raises(G.GpeError) as e:
             G.gpe_plan_create(bad[0], bad[1], 1.0, 1.0, G.GPE_C64, 1)
         assert e.value.status == 2

@@ -68,3 +68,24 @@ def test_axes_not_transposed():
     assert abs(f[3, 0] - nx * ny) <= 1e-9
     f[3, 0] = 0
     assert np.max(np.abs(f)) <= 1e-9
+
+
+@pytest.mark.parametrize("n", [96, 160, 240, 90, 250])
+def test_non_power_of_two_lengths_take_the_definition(n):
+    """SURVEY.md 8(f) f4 ("non-optimal grid sizes"): lengths that are not powers of two go
+    through dft_direct.  Pinned against the DFT matrix and numpy, both directions."""
+    a = _rand(n, n)
+    j = np.arange(n)
+    F = np.exp(-2j * np.pi * np.outer(j, j) / n)
+    got = O.fft1(a, -1)
+    assert np.max(np.abs(got - F @ a)) <= 1e-12 * n
+    assert np.max(np.abs(got - np.fft.fft(a))) <= 1e-12 * n
+    assert np.max(np.abs(O.fft1(a, +1) - np.conj(F) @ a)) <= 1e-12 * n
+
+
+@pytest.mark.parametrize("shape", [(96, 160), (240, 64), (128, 90)])
+def test_fft2_non_power_of_two(shape):
+    a = _rand(shape, 17)
+    f = O.fft2(a, -1)
+    assert np.max(np.abs(f - np.fft.fft2(a))) <= 1e-11 * np.sqrt(a.size)
+    assert np.max(np.abs(O.fft2(f, +1) - a)) <= 1e-13 * np.sqrt(a.size)

@@ -678,3 +678,25 @@ def test_tvt_cavity_scalars_come_from_the_psi_entering_the_potential_factor():
     o.kinetic_step(c, dt / 2, True)
     th_mid = o.observables(c)[0][0]["theta"]
     assert abs(th_mid - th0) > 1e-6 * abs(th0)
+
+
+def test_gaussian_recurrence_on_a_non_power_of_two_grid():
+    """the whole step on a 96 x 80 grid (dft_direct on both axes) obeys the same closed form
+    as test_gaussian_recurrence_closed_form, so the non-power-of-two branch of the oracle is pinned by more than
+    its transform alone."""
+    p = W.config1(g=0.0, noise=0.0)
+    nx, ny, L = 96, 80, 16.0
+    p["nx"], p["ny"] = nx, ny
+    v2d, vx, vy = W.harmonic_trap(nx, ny, L, L)
+    p["v_static"], p["vx"], p["vy"] = v2d, vx, vy
+    psi = W.noisy_gaussian(nx, ny, L, L, 1.5, 1234, 0.0)
+    dt, nsteps = 1e-3, 300
+    o = Oracle(p)
+    o.evolve(psi, dt, nsteps, True)
+    a = 1.0 / 1.5 ** 2
+    for _ in range(nsteps):
+        b = a + dt / 2
+        a = b / (1 + b * dt) + dt / 2
+    obs, _, _ = o.observables(psi)
+    assert obs[0]["norm"] == pytest.approx(1.0, abs=1e-13)
+    assert obs[0]["e_kin"] + obs[0]["e_pot"] == pytest.approx(2 * (a / 4 + 1 / (4 * a)), abs=1e-9)
