@@ -169,6 +169,22 @@ def flops_per_point(npts: int) -> float:
     return 10.0 * math.log2(npts) + 90.0
 
 
+def step_form(p, mode):
+    """Which form of the step the library runs for a workload (csrc/gpe_api.cu evolve_impl) and how many times
+    psi crosses L2 / HBM per step in it (reads + writes, in units of the array): square grids up to 256^2 run
+    every step inside one cluster kernel whose rows stay in registers from pass C to pass A (4 sweeps); without
+    the cavity term in real time, or with g = 0 and no cavity term in imaginary time, passes C and A fuse
+    (2 kernels, 4 sweeps); everything else is the three fused passes (6 sweeps)."""
+    import numpy as np
+    cavity = bool(p.get("cavity_on", 0))
+    g0 = not np.any(np.asarray(p.get("g", 0.0)) != 0.0)
+    if p["nx"] == p["ny"] and p["nx"] <= 256:
+        return "one cluster kernel per call, rows in registers from pass C to pass A", 4
+    if not cavity and (mode == "real" or g0):
+        return "2 kernels per step (pass B, fused C+A)", 4
+    return "3 fused passes per step", 6
+
+
 def other_workloads(G, torch, peak, roofs):
     """Short device-resident timings of the other BASELINE.json configs (parity-test workloads, not the
     bench line): us per split-step, updates/s and the fraction of the roof that bounds each -- the byte
@@ -191,8 +207,9 @@ def other_workloads(G, torch, peak, roofs):
         p = make()
         us = _time_evolve(G, torch, p, dtype, batch, mode, dt, steps) / steps * 1e3
         pts = batch * p["nx"] * p["ny"]
-        bpp = 48.0 if dtype == "c64" else 96.0
-        row = {"updates_per_s": pts / (us * 1e-6), "us_per_split_step": us, "passes_per_step": 3,
+        form, sweeps = step_form(p, mode)
+        bpp = sweeps * (8.0 if dtype == "c64" else 16.0)
+        row = {"updates_per_s": pts / (us * 1e-6), "us_per_split_step": us, "form": form,
                "algorithmic_bytes_per_point": bpp, "byte_roofline_frac": pts * bpp / (us * 1e-6) / 1e9 / peak}
         if dtype == "c128":
             fl = flops_per_point(p["nx"] * p["ny"])
@@ -218,7 +235,7 @@ def sweep_s(G, torch):
             ts = [_time_evolve(G, torch, p, dtype, 1, "imag", 1e-3, 1000, warm=50) for _ in range(5)]
             mean = sum(ts) / len(ts)
             rows.append({"n": n, "dtype": dtype, "ms_per_1000_steps_mean_of_5": mean, "min": min(ts), "max": max(ts),
-                         "updates_per_s": n * n * 1000 / (mean * 1e-3)})
+                         "updates_per_s": n * n * 1000 / (mean * 1e-3), "form": step_form(p, "imag")[0]})
     return rows
 
 

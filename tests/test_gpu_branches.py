@@ -313,14 +313,28 @@ def test_evolve_only_enqueues(ordering):
     plan.close()
 
 
+def _records_ok(rg, ro, tol):
+    """step and A exact; norm and Theta by reading Q17; alpha by Q17's bound on Theta carried through Eq. 14
+    (alpha = K Theta + probe: an error dTheta moves alpha by |K| dTheta, and |K| = N eta / |Delta + i kappa|
+    is about 7 in these workloads, so a flat 1e-5 max(|alpha|, 1e-2) would be tighter than the Theta bar)."""
+    assert rg.shape == ro.shape
+    assert np.array_equal(rg[:, :, 0], ro[:, :, 0])
+    assert np.allclose(rg[:, :, 5], ro[:, :, 5], rtol=1e-14, atol=1e-300)
+    assert np.all(np.abs(rg[:, :, 1] - ro[:, :, 1]) <= tol * np.abs(ro[:, :, 1]))
+    th = np.maximum(np.abs(ro[:, :, 2]), 1e-2)
+    assert np.all(np.abs(rg[:, :, 2] - ro[:, :, 2]) <= tol * th)
+    gain = np.maximum(np.hypot(ro[:, :, 3], ro[:, :, 4]) / np.maximum(np.abs(ro[:, :, 2]), 1e-300), 1.0)
+    gain = np.where(np.abs(ro[:, :, 2]) > 1e-12, gain, 1.0)
+    for c in (3, 4):
+        assert np.all(np.abs(rg[:, :, c] - ro[:, :, c]) <= tol * th * np.maximum(gain, 1.0)), c
+
+
 def _local_workload(nx, ny, batch=1, g=40.0, v2d=False):
     """No cavity term: static trap (+ optional 2-D array), ramped lattice, contact interaction."""
     p = _general_workload(nx, ny, batch=batch)
     p["cavity_on"] = 0
     p["g"] = np.linspace(g, 1.5 * g, batch)
-    if not v2d:
-        p["v_static"] = None
-    return p
+    return p   # v_static stays: the oracle knows the trap only as a 2-D array (the GPU may take vx + vy instead)
 
 
 @pytest.mark.parametrize("dtype", ["c64", "c128"])
@@ -410,10 +424,7 @@ def test_cluster_kernel_and_multi_launch_path_agree(monkeypatch, n, batch, mode,
         out = psi.cpu().numpy()
         e = _rel(out, ref)
         assert e <= 25 * PER_STEP[dtype], f"chip={chip}: {e:.3e}"
-        tol = 1e-5 if dtype == "c64" else 1e-10
-        assert np.array_equal(rg[:, :, 0], ro[:, :, 0])
-        for c in (1, 2, 3, 4, 5):
-            assert np.all(np.abs(rg[:, :, c] - ro[:, :, c]) <= tol * np.maximum(np.abs(ro[:, :, c]), 1e-2)), (chip, c)
+        _records_ok(rg, ro, 1e-5 if dtype == "c64" else 1e-10)
         assert plan.step == 25
         outs.append(out)
         plan.close()

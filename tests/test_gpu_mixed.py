@@ -7,6 +7,7 @@ import pytest
 import workloads as W
 from oracle import gpe_oracle
 from oracle.gpe_oracle import Oracle
+from tests.test_gpu_branches import _records_ok
 from tests.test_gpu_parity import PER_STEP, _general_workload, _gpu_plan, _oracle_input, _rel, _to_dev, _torch
 
 pytestmark = pytest.mark.gpu
@@ -64,9 +65,7 @@ def test_per_step_parity_mixed_radix(nx, ny, batch, mode, dtype):
     e = _rel(psi.cpu().numpy(), ref)
     assert e <= 12 * PER_STEP[dtype], f"12 steps: {e:.3e}"
     tol = 1e-5 if dtype == "c64" else 1e-10
-    assert np.array_equal(rg[:, :, 0], ro[:, :, 0])
-    for c in (1, 2, 3, 4, 5):
-        assert np.all(np.abs(rg[:, :, c] - ro[:, :, c]) <= tol * np.maximum(np.abs(ro[:, :, c]), 1e-2)), c
+    _records_ok(rg, ro, tol)
     og, oo = plan.observables(psi)[0], o.observables(ref)[0]
     for b in range(batch):
         for k in ("norm", "e_kin", "e_pot", "e_int", "theta"):
@@ -80,8 +79,7 @@ def test_mixed_radix_large_and_unsupported():
     ordering = 1 is refused for these sizes; odd sizes and prime factors above 5 are GPE_EUNSUPPORTED."""
     import paper_2404_14401_b200 as G
     p = _general_workload(500, 960)
-    p["v_static"] = None
-    plan = _gpu_plan(p, "c64")
+    plan = _gpu_plan(p, "c64")          # the trap as vx + vy on the GPU, as a 2-D array in the oracle
     psi, ref = _to_dev(p["psi0"], "c64"), _oracle_input(p["psi0"], "c64")
     plan.evolve(psi, 1e-3, 1, "real")
     Oracle(p).evolve(ref, 1e-3, 1, False)

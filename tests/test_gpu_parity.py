@@ -212,9 +212,11 @@ def test_config4_ramp_reduced(dtype):
         floor = np.abs(rfl - rref)
     err = np.abs(rec - rref)
     print("theta err", err[:, 0, 2], "fp32 floor", floor[:, 0, 2])
-    assert np.all(err[:, :, 2] <= tol * np.maximum(np.abs(rref[:, :, 2]), 1e-2))
-    amax = np.abs(rref[:, :, 3:5]).max()
-    assert np.all(err[:, :, 3:5] <= tol * max(amax, 1e-2))
+    thb = tol * np.maximum(np.abs(rref[:, :, 2]), 1e-2)
+    assert np.all(err[:, :, 2] <= thb)
+    # alpha = K Theta (Eq. 14): Q17's bound on Theta carried through |K| = |alpha| / |Theta| (at least 1)
+    gain = np.maximum(np.hypot(rref[:, :, 3], rref[:, :, 4]) / np.maximum(np.abs(rref[:, :, 2]), 1e-300), 1.0)
+    assert np.all(err[:, :, 3:5] <= (thb * gain)[:, :, None])
     assert np.allclose(rec[:, :, 5], rref[:, :, 5], rtol=1e-14)
     plan.close()
 
@@ -234,7 +236,15 @@ def test_config5_batch_reduced_and_member_equivalence():
         assert _rel(out[b], ref[b]) <= FULL_RUN["c64"], b
     gth = np.array([ob["theta"] for ob in plan.observables(psi)[0]])
     rth = np.array([ob["theta"] for ob in o.observables(ref)[0]])
-    assert np.all(np.abs(gth - rth) <= 1e-5 * np.maximum(np.abs(rth), 1e-2))
+    # reading Q17, or the fp32 floor of the method where that is larger (tests/test_gpu_fullsize.py states the rule:
+    # four times the envelope of the RELATIVE error of Theta that the oracle's own statements show in complex64 --
+    # the members still in their exponential growth phase freeze an early round-off error as a relative error)
+    r64 = Oracle(p).evolve(_oracle_input(p["psi0"], "c64"), 5e-4, 200, True, record_every=20)
+    r32 = Oracle(p, "f32").evolve(np.ascontiguousarray(p["psi0"].astype(np.complex64)), 5e-4, 200, True, record_every=20)
+    env = np.max(np.abs(r32[:, :, 2] - r64[:, :, 2]) / np.maximum(np.abs(r64[:, :, 2]), 1e-300), axis=0)
+    bound = np.maximum(1e-5 * np.maximum(np.abs(rth), 1e-2), 4.0 * env * np.abs(rth))
+    print("theta err", np.abs(gth - rth), "Q17 bar", 1e-5 * np.maximum(np.abs(rth), 1e-2), "4 x fp32 floor", 4.0 * env * np.abs(rth))
+    assert np.all(np.abs(gth - rth) <= bound)
     for b in (0, 3):
         q = W.member(p, b)
         plan1 = _gpu_plan(q, "c64")
