@@ -691,8 +691,14 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
         return GPE_OK;
     }
     // Small square grids (64^2 .. 256^2): every step of the call inside ONE cluster kernel (gpe_chip.cuh).
+    // Measured on B200 (us per step, cluster kernel against the multi-launch passes): 64^2 7.3 / 11.6, 128^2 7.8 / 11.0,
+    // 256^2 complex64 10.3 / 11.5 (cavity: 10.7 / 15.1); 256^2 complex128 is fp64-bound on the cluster's 16 SMs
+    // (17.0 against 15.2 in the 2-pass form on all SMs, but 17.0 against 23.9 with the cavity term): there the
+    // cluster kernel runs only when the 2-pass form is not available.
+    const bool fusable = !p->no_fuse && !(p->flags & F_CAVITY) && (imag ? !(p->flags & F_HAS_G) : !p->no_merge) && !p->d_u0;
+    const bool chip_wins = p->nx < 256 || sizeof(T) == 4 || !fusable;
     bool chip_done = false;
-    if (!prof && !p->no_chip && !p->no_pair && p->nx == p->ny && oy->chip) {
+    if (!prof && !p->no_chip && !p->no_pair && p->nx == p->ny && oy->chip && chip_wins) {
         if (p->chip_ok < 0) p->chip_ok = oy->chip_available() ? 1 : 0;
         if (p->chip_ok == 1) {
             a.src = (const cx<T> *)psi; a.dst = (cx<T> *)psi;

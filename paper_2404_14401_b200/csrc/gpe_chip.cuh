@@ -22,11 +22,14 @@
 #include <cooperative_groups.h>
 #include "gpe_kernels.cuh"
 
+#ifndef GPE_CHIP_NC16_MIN
+#define GPE_CHIP_NC16_MIN 128   // from this size on 16 CTAs per cluster
+#endif
 namespace gpe {
 namespace cg = cooperative_groups;
 
 template <typename T, int N> struct ChipGeom {
-    static constexpr int NC = (sizeof(T) == 8 && N >= 256) ? 16 : 8;   // CTAs per cluster (16 needs the non-portable opt-in)
+    static constexpr int NC = N >= GPE_CHIP_NC16_MIN ? 16 : 8;   // CTAs per cluster (16 needs the non-portable opt-in)
     static constexpr int RB = N / NC;                                  // rows (and columns) per CTA
     static constexpr int TPF = N / 16;                                 // threads per transform
     static constexpr int THREADS = RB * TPF;                           // 64^2: 32, 128^2: 128, 256^2: 512 (c64) / 256 (c128)
