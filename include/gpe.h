@@ -246,6 +246,22 @@ GPE_API gpe_status gpe_set_step(gpe_plan *p, long step);
  * gpe_plan_create failure on this thread.  The pointer stays valid until the next call. */
 GPE_API const char *gpe_last_error(const gpe_plan *p);
 
+/*
+ * gpe_norm_theta_noalloc -- the fused norm / cavity-overlap reduction of one step (PAPER.md:116 and PAPER.md:183,
+ * Eq. 14) as an entry point that ALLOCATES NOTHING: no plan, no cudaMalloc / cudaFree inside.  For callers that
+ * cannot allocate (CUDA graph capture, tight serving loops).  For every member b of
+ * psi_dev: DEVICE [batch][nx][ny] complex (dtype; aligned to one complex number), grid as in gpe_plan_create,
+ *   out_dev[b][0] = sum |psi|^2 dx dy,   out_dev[b][1] = sum cos(k x_i) cos(k y_j) |psi|^2 dx dy   (k = cavity_k)
+ * out_dev: DEVICE [batch][2] doubles, 16-byte aligned, caller-owned.  Enqueued on cuda_stream, no synchronisation.
+ * Scratch (per-CTA partial sums and counters) is a fixed 65 792-byte device array inside the library, held by every
+ * GPU that loads it; hence the limits batch <= 64 and nx, ny <= 4096 (GPE_EUNSUPPORTED beyond, GPE_EINVAL on bad
+ * arguments; text from gpe_noalloc_last_error).  Every call shares that array: calls that overlap on the GPU
+ * (different streams or threads) race and must be serialised by the caller.
+ */
+GPE_API gpe_status gpe_norm_theta_noalloc(const void *psi_dev, int nx, int ny, double Lx, double Ly, gpe_dtype dtype,
+                                          int batch, double cavity_k, double *out_dev, void *cuda_stream);
+GPE_API const char *gpe_noalloc_last_error(void);
+
 /* Library build information: "libgpe <version> sm_100a". */
 GPE_API const char *gpe_version(void);
 

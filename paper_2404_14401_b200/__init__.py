@@ -9,7 +9,7 @@ call fails loudly with GPE_ECUDA when no device is present, and a missing librar
 from .binding import (  # noqa: F401
     GPE_C64, GPE_C128, GPE_REAL_TIME, GPE_IMAG_TIME, GPE_NREC, GpeError, Plan,
     gpe_plan_create, gpe_plan_set_stream, gpe_plan_destroy, gpe_set_potential, gpe_evolve,
-    gpe_observables, gpe_populations, gpe_profile_passes, gpe_measure_roofs, gpe_fft2_forward, gpe_get_step, gpe_set_step,
+    gpe_observables, gpe_populations, gpe_profile_passes, gpe_measure_roofs, gpe_norm_theta_noalloc, gpe_fft2_forward, gpe_get_step, gpe_set_step,
     gpe_last_error, gpe_version,
     gpe_potential_desc, gpe_obs, library_path, load_library,
 )

@@ -88,6 +88,10 @@ def load_library() -> C.CDLL:
     lib.gpe_profile_passes.argtypes = [vp, vp, d, l, i, C.POINTER(C.c_double)]
     lib.gpe_measure_roofs.restype = i
     lib.gpe_measure_roofs.argtypes = [vp, C.POINTER(C.c_double)]
+    lib.gpe_norm_theta_noalloc.restype = i
+    lib.gpe_norm_theta_noalloc.argtypes = [vp, i, i, d, d, i, i, d, vp, vp]
+    lib.gpe_noalloc_last_error.restype = C.c_char_p
+    lib.gpe_noalloc_last_error.argtypes = []
     lib.gpe_get_step.restype = i
     lib.gpe_get_step.argtypes = [vp, C.POINTER(l)]
     lib.gpe_set_step.restype = i
@@ -180,6 +184,16 @@ def gpe_measure_roofs(cuda_stream: int = 0) -> dict:
     _check(load_library().gpe_measure_roofs(C.c_void_p(cuda_stream), out), None)
     return {"l2_rw_32MiB_gbs": out[0], "l2_rw_64MiB_gbs": out[1], "hbm_rw_1GiB_gbs": out[2],
             "fp32_fma_tflops": out[3], "fp64_fma_tflops": out[4]}
+
+
+def gpe_norm_theta_noalloc(psi_ptr: int, nx: int, ny: int, Lx: float, Ly: float, dtype: int, batch: int,
+                           cavity_k: float, out_ptr: int, cuda_stream: int = 0) -> None:
+    """out[b] = {norm, theta} of member b, written on the device; allocates nothing (include/gpe.h)."""
+    lib = load_library()
+    st = lib.gpe_norm_theta_noalloc(C.c_void_p(psi_ptr), int(nx), int(ny), float(Lx), float(Ly), int(dtype), int(batch),
+                                    float(cavity_k), C.c_void_p(out_ptr), C.c_void_p(cuda_stream))
+    if st != 0:
+        raise GpeError(st, lib.gpe_noalloc_last_error().decode())
 
 
 def gpe_get_step(plan) -> int:

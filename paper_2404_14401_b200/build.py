@@ -59,6 +59,9 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     o = os.path.join(OBJ, "api.o")
     objs.append(o)
     jobs.append([nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, "gpe_api.cu"), "-o", o])
+    o = os.path.join(OBJ, "noalloc.o")
+    objs.append(o)
+    jobs.append([nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, "gpe_noalloc.cu"), "-o", o])
     with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
         logs = list(ex.map(_run, jobs))
     if verbose or ptxas_v:
