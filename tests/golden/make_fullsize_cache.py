@@ -10,7 +10,10 @@ Items (one .npz each under tests/golden/fullsize/, keyed by config, input dtype 
   c3        config 3: 1024^2, complex64 input, imaginary time dt=5e-4 x 5000, seed 7
   c4_c64    config 4: 2048^2, complex64 input (the fp32-rounded psi0, up-cast), real time dt=1e-4 x 10000
   c4_c128   config 4: 2048^2, complex128 input, same run
-  c5        config 5: 64 x 512^2, complex64 input, imaginary time dt=5e-4 x 3000
+  c5        config 5: 64 x 512^2, complex64 input, imaginary time dt=5e-4 x 3000 -- the oracle runs EIGHT of the 64
+            members (C5_MEMBERS: the four corners of the (V_p, Delta) sweep and four points of its diagonal; members
+            never interact, so member b of the batch is the single-grid run with its parameters); the GPU test runs
+            all 64 and compares these eight
   <item>_floor   the same run with the oracle's statements compiled in complex64 (-DREAL=float): the
             fp32 round-off floor OF THE METHOD, never used as a reference.
             Needs <item>.npz (it stores its distance to it).
@@ -44,12 +47,14 @@ from oracle.gpe_oracle import Oracle, OBS_NAMES        # noqa: E402
 HERE = os.path.dirname(os.path.abspath(__file__))
 CACHE = os.path.join(HERE, "fullsize")
 
+C5_MEMBERS = (0, 7, 18, 27, 36, 45, 56, 63)   # member index 8 b + a: V_p = 20 a / 7, Delta = -3 + 2.8 b / 7
+
 ITEMS = {
     # name: (workload factory, input dtype, mode, dt, checkpoints, record_every, sample stride)
     "c3": (lambda: W.config3(), "c64", "imag", 5e-4, (1, 10, 100, 1000, 5000), 100, 4),
     "c4_c64": (lambda: W.config4(), "c64", "real", 1e-4, (1, 10, 100, 1000, 5000, 10000), 100, 8),
     "c4_c128": (lambda: W.config4(dtype="c128"), "c128", "real", 1e-4, (1, 100, 1000, 10000), 100, 8),
-    "c5": (lambda: W.config5(), "c64", "imag", 5e-4, (1, 100, 3000), 500, 8),
+    "c5": (lambda: W.select_members(W.config5(), C5_MEMBERS), "c64", "imag", 5e-4, (1, 100, 1000, 3000), 500, 8),
 }
 
 
@@ -88,7 +93,8 @@ def run_item(name: str, out_dir: str, scale: int = 1) -> str:
     p = make()
     imag = mode == "imag"
     ref_file = os.path.join(out_dir, base + ".npz")
-    out = {"stride": np.int64(stride), "steps": np.array(checkpoints, dtype=np.int64), "dt": np.float64(dt),
+    out = {"members": np.array(C5_MEMBERS if base == "c5" else range(p.get("batch", 1)), dtype=np.int64),
+           "stride": np.int64(stride), "steps": np.array(checkpoints, dtype=np.int64), "dt": np.float64(dt),
            "imag": np.int64(imag), "record_every": np.int64(record_every),
            "oracle_sha16": np.array(oracle_sha()), "item": np.array(name)}
     if floor:

@@ -205,9 +205,17 @@ def shard_members(batch: int, rank: int, world: int) -> range:
     return range(lo, lo + base + (1 if rank < extra else 0))
 
 
+def select_members(p: dict, idx) -> dict:
+    """The sub-workload holding only the members `idx` of a batched workload `p` (same order)."""
+    return _select(p, [int(i) for i in idx])
+
+
 def shard(p: dict, rank: int, world: int) -> dict:
     """The sub-workload holding only this rank's members of a batched workload `p`."""
-    idx = list(shard_members(p["batch"], rank, world))
+    return _select(p, list(shard_members(p["batch"], rank, world)))
+
+
+def _select(p: dict, idx: list) -> dict:
     B = p["batch"]
     q = copy.deepcopy(p)
     q["batch"] = len(idx)
