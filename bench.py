@@ -324,8 +324,8 @@ def run_reference(args):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture:
 # pass index -> bytes.  ncu flushes the caches before every replay, so each pass reads psi once from DRAM
 # and writes (almost) nothing back; in the timed run the 32 MiB array never leaves L2 at all.
-TRAFFIC_BYTES_PER_LAUNCH = {0: 33.67e6 + 1.02e6, 1: 33.68e6 + 0.008e6, 2: 33.67e6 + 0.66e6}
-TRAFFIC_SOURCE = "profiles/r01_final.md section 3 (ncu --set full, cache-flushed replay; not measured by this run)"
+TRAFFIC_BYTES_PER_LAUNCH = {0: 33.67e6 + 1.14e6, 1: 33.68e6 + 0.003e6, 2: 33.67e6 + 0.78e6}
+TRAFFIC_SOURCE = "profiles/r02_final.md section 3 (ncu --set full, cache-flushed replay; not measured by this run)"
 
 
 def run_ours(args):

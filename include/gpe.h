@@ -168,7 +168,12 @@ GPE_API gpe_status gpe_set_potential(gpe_plan *p, const gpe_potential_desc *d);
  * new (dt, mode) pair are written by a kernel on the same stream, nothing is allocated), no host
  * round trip of the per-step scalars (norm, Theta, alpha live in device memory; north_star (3)).
  * The plan's device must be current (GPE_EINVAL otherwise; this holds for every call on a plan).
- * GPE_ESTATE before gpe_set_potential; GPE_EINVAL on bad arguments; GPE_ECUDA on launch errors.
+ * How the steps are run is chosen per call and does not change what is computed: three
+ * fused passes per step; two where no global scalar sits between pass C and the next pass A (real time without the
+ * cavity term; imaginary time with g = 0 and no cavity term); every step inside ONE thread-block-cluster kernel for
+ * square grids up to 256^2; mixed-radix passes for sizes that are not powers of two.
+ * GPE_ESTATE before gpe_set_potential; GPE_EINVAL on bad arguments; GPE_ECUDA on launch errors;
+ * GPE_EUNSUPPORTED for ordering = 1 on a size that is not a power of two.
  */
 GPE_API gpe_status gpe_evolve(gpe_plan *p, void *psi_dev, double dt, long n_steps, gpe_mode mode,
                       long record_every, double *records_dev);

@@ -429,3 +429,17 @@ def test_cluster_kernel_and_multi_launch_path_agree(monkeypatch, n, batch, mode,
         outs.append(out)
         plan.close()
     assert _rel(outs[0], outs[1].astype(np.complex128)) <= (5e-6 if dtype == "c64" else 1e-13)
+
+
+def test_measure_roofs_is_sane():
+    """gpe_measure_roofs (the denominators bench.py reports against): positive, ordered as the memory hierarchy
+    is (L2-resident >= 0.8 x HBM-resident), fp32 FMA rate above fp64's, and the call leaves no error behind."""
+    import paper_2404_14401_b200 as G
+    r = G.gpe_measure_roofs(_torch().cuda.current_stream().cuda_stream)
+    assert 1000.0 < r["hbm_rw_1GiB_gbs"] < 20000.0
+    assert r["l2_rw_32MiB_gbs"] >= 0.8 * r["hbm_rw_1GiB_gbs"] and r["l2_rw_64MiB_gbs"] >= 0.8 * r["hbm_rw_1GiB_gbs"]
+    assert 10.0 < r["fp64_fma_tflops"] < r["fp32_fma_tflops"] < 400.0
+    p = _general_workload(64, 64)
+    plan = _gpu_plan(p, "c64")
+    plan.evolve(_to_dev(p["psi0"], "c64"), 1e-3, 2, "real")
+    plan.close()
