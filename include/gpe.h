@@ -136,10 +136,10 @@ typedef struct {
      * spells out.  1: T/2 V T/2, the form the paper prints (Eqs. 3-4): half a kinetic
      * step, then A_n, Theta_n, alpha_n and |psi|^2 taken from the psi that ENTERS the potential factor,
      * one full factor exp(-sigma (V_n + g|psi|^2) dt), half a kinetic step, and in imaginary time the
-     * renormalisation.  Real time runs the same three fused passes per step (adjacent kinetic halves
-     * merge; one extra kinetic-only unit per call and per record boundary); imaginary time runs the
-     * unmerged form, two units of three passes per step.  With ordering = 1 gpe_evolve uploads a
-     * second set of kinetic tables the first time a (dt, mode) pair is seen. */
+     * renormalisation.  Both time modes run three fused passes per step (adjacent kinetic halves merge --
+     * in imaginary time around the renormalisation, whose norm is then taken in k space; one extra
+     * kinetic-only unit per call and per record boundary).  With ordering = 1 gpe_evolve fills a second
+     * set of kinetic tables (dt/2) on the device the first time a (dt, mode) pair is seen.  Powers of two only. */
     int ordering;
 } gpe_potential_desc;
 

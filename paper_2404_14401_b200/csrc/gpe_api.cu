@@ -64,6 +64,7 @@ struct gpe_plan {
     MemberState *st = nullptr;
     double2 *partials = nullptr;
     double *partials_b = nullptr;   // third sum (full cavity model)
+    double *partials_k = nullptr;   // k-space partial sums of pass B (T/2 V T/2 in imaginary time, merged kinetic halves)
     double *d_u0 = nullptr;         // [batch] U0 of Eqs. 12, 15; nullptr = three-term model
     std::vector<double> h_u0;
     unsigned int *counters = nullptr;
@@ -509,6 +510,7 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     a.inv_p = (T)(1.0 / ((double)p->nx * (double)p->ny));
     FinalizeParams &f = a.fin;
     f.partials_b = p->partials_b; f.cav_u0 = p->d_u0;
+    f.partials_k = p->partials_k; f.knorm = 0; f.cpmk = 0; f.kscale = (double)p->nx * (double)p->ny;
     f.st = p->st; f.partials = p->partials; f.counters = p->counters; f.nonfinite = p->nonfinite;
     f.sched_len = p->sched_len; f.sched_step = p->d_sched_step; f.sched_amp = p->d_sched_amp;
     f.sched_batched = p->sched_batched;
@@ -673,13 +675,28 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
                 done += chunk;
             }
         } else {
-            // unmerged: the norm is taken after the second kinetic half, so the halves of
-            // consecutive steps cannot merge without a k-space sum in pass B (not built)
-            for (long i = 0; i < n_steps; ++i) {
-                if ((s = half_kinetic(p->step + i, 0)) != GPE_OK) return s;
-                StepArgs<T, cx<T>> u = ah;
-                u.fin = a.fin; u.fin.merged = 0; u.fin.tvt = 0; u.fin.prepared = 0;
-                if ((s = unit(u, (T)dt, (T)0)) != GPE_OK) return s;
+            // T/2 (V T N')^(c-1) V T/2 N per chunk of c steps.  The renormalisation N' between the kinetic halves of
+            // consecutive steps is a scalar, so the halves merge into ONE pass B on the dt/2 tables applied twice,
+            // which takes the norm of the wavefunction at the step boundary as a k-space sum in between (Parseval;
+            // k_col_p KNORM); the last block of pass C turns it into the lazy scale and divides Theta by it.  The
+            // first half of a chunk is the kinetic-only unit, its last step ends with T/2 and the real-space norm;
+            // a chunk ends where a record is due (the record is taken from psi_{n+1} itself).
+            const int cpmk = paired ? p->ny / 2 / ox->p_colpairs_per_cta : p->ny / ox->cols_per_cta;
+            for (long done = 0; done < n_steps;) {
+                const long stepnow = p->step + done;
+                long chunk = n_steps - done;
+                if (records && record_every > 0) {
+                    const long to_rec = record_every - (stepnow % record_every);
+                    if (to_rec < chunk) chunk = to_rec;
+                }
+                if ((s = half_kinetic(stepnow, 0)) != GPE_OK) return s;
+                for (long i = 0; i < chunk; ++i) {
+                    StepArgs<T, cx<T>> u = ah;
+                    u.fin = a.fin; u.fin.merged = 0; u.fin.tvt = 0; u.fin.prepared = 0;
+                    if (i < chunk - 1) { u.fin.knorm = 1; u.fin.cpmk = cpmk; }
+                    if ((s = unit(u, (T)dt, (T)0)) != GPE_OK) return s;
+                }
+                done += chunk;
             }
             dim3 grid(256, p->batch);
             k_rescale<T><<<grid, 256, 0, p->stream>>>((cx<T> *)psi, (size_t)p->nx * p->ny, p->st);
@@ -1046,6 +1063,7 @@ gpe_status gpe_plan_create(gpe_plan **out, int nx, int ny, double Lx, double Ly,
         GPE_CUDA(p, cudaMemset(p->st, 0, sizeof(MemberState) * batch));
         GPE_CUDA(p, cudaMalloc((void **)&p->partials, sizeof(double2) * (size_t)batch * kMaxCpm));
         GPE_CUDA(p, cudaMalloc((void **)&p->partials_b, sizeof(double) * (size_t)batch * kMaxCpm));
+        GPE_CUDA(p, cudaMalloc((void **)&p->partials_k, sizeof(double) * (size_t)batch * kMaxCpm));
         GPE_CUDA(p, cudaMalloc((void **)&p->counters, sizeof(unsigned int) * batch));
         GPE_CUDA(p, cudaMemset(p->counters, 0, sizeof(unsigned int) * batch));
         GPE_CUDA(p, cudaMalloc((void **)&p->d_call, sizeof(CallParams)));
@@ -1076,7 +1094,7 @@ gpe_status gpe_plan_destroy(gpe_plan *p) {
     if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->kin_y2, p->kinh_x, p->kinh_y, p->kinh_y2, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
-                    p->ytab, p->g, p->v2d, p->st, p->partials, p->partials_b, p->d_u0, p->counters, p->nonfinite, p->d_sched_step,
+                    p->ytab, p->g, p->v2d, p->st, p->partials, p->partials_b, p->partials_k, p->d_u0, p->counters, p->nonfinite, p->d_sched_step,
                     p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->d_probe_omega, p->d_probe_delta,
                     p->d_probe_phi, p->scratch, p->obs_dev,
                     p->pop_dev, p->obsA_dev};

@@ -23,6 +23,7 @@ template <typename T> struct Ops {
     // small square grids: all steps of a call in one cluster kernel (gpe_chip.cuh); null above 256
     cudaError_t (*chip)(const A &, bool imag, long n_steps, cudaStream_t);
     bool (*chip_available)();
+    int cols_per_cta, p_colpairs_per_cta;   // columns (column pairs) per CTA of pass B: number of its partial sums
 };
 
 #define GPE_DECL_OPS(N)                    \

@@ -14,6 +14,7 @@ template <typename T, int N, bool ON = (sizeof(T) == 4 && N >= 128)> struct Pair
     static constexpr decltype(Ops<T>::p_col) col = nullptr;
     static constexpr decltype(Ops<T>::p_row_ca) row_ca = nullptr;
     static constexpr int rpc = 0;
+    static constexpr int cpw = 0;
 };
 template <int N> struct PairOps<float, N, true> {
     static constexpr auto row_fwd = &LaunchP<N>::row_fwd;
@@ -21,6 +22,7 @@ template <int N> struct PairOps<float, N, true> {
     static constexpr auto col = &LaunchP<N>::col;
     static constexpr auto row_ca = &LaunchP<N>::row_ca;
     static constexpr int rpc = RowGeomP<N>::RPC;
+    static constexpr int cpw = ColGeomP<N>::CPW;
 };
 template <typename T, int N, bool ON = (N <= 256)> struct ChipOps {
     static constexpr decltype(Ops<T>::chip) run = nullptr;
@@ -43,5 +45,7 @@ extern const Ops<GPE_T> GPE_CAT3(ops_, GPE_TAG, GPE_N) = {
     PairOps<GPE_T, GPE_N>::row_ca,
     ChipOps<GPE_T, GPE_N>::run,
     ChipOps<GPE_T, GPE_N>::available,
+    ColGeom<GPE_T, GPE_N>::W,
+    PairOps<GPE_T, GPE_N>::cpw,
 };
 }  // namespace gpe

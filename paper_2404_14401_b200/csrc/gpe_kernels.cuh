@@ -201,9 +201,24 @@ __device__ inline void block_reduce_and_finalize(const FinalizeParams &f, int b,
         __syncthreads();
         if (lane == 0) { red[w] = a; red[32 + w] = c; red[64 + w] = e; }
         __syncthreads();
-        if (threadIdx.x == 0) {
-            double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+        double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+        if (threadIdx.x == 0)
             for (int i = 0; i < nw; ++i) { t0 += red[i]; t1 += red[32 + i]; t2 += red[64 + i]; }
+        if (f.knorm) {   // the norm from pass B's k-space partial sums (merged kinetic halves, see k_col)
+            double k = 0.0;
+            const double *pk = f.partials_k + (size_t)b * f.cpmk;
+            for (int q = threadIdx.x; q < f.cpmk; q += blockDim.x) k += __ldcg(pk + q);
+            k = warp_sum(k);
+            __syncthreads();
+            if (lane == 0) red[w] = k;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                double tk = 0.0;
+                for (int i = 0; i < nw; ++i) tk += red[i];
+                t0 = tk * f.kscale;
+            }
+        }
+        if (threadIdx.x == 0) {
             finalize_member(f, b, t0, t1, t2);
             f.counters[b] = 0u;
         }
@@ -458,7 +473,7 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS, 1) k_col(const StepAr
     C v[16];
     pdl_launch_dependents();
     pdl_wait();
-    if (MODE == 0 && blockIdx.x == 0 && threadIdx.x == 0 && a.fin.prepared) prepare_member(a.fin, b);
+    if (MODE != 1 && blockIdx.x == 0 && threadIdx.x == 0 && a.fin.prepared) prepare_member(a.fin, b);
 #pragma unroll
     for (int k = 0; k < 16; ++k) v[k] = __ldcg(src + (size_t)(j + F::M1 * k) * ny);
     F::fwd(v, sm, j, a.tw_x, a.tw1_x);
@@ -471,6 +486,8 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS, 1) k_col(const StepAr
     } else {
         if constexpr (IMAG) {
             const T ey = a.kin_yr[col];
+            T acc = T(0);
+            const T bigp = T(1) / a.inv_p;   // nx ny: a power of two, exact
 #pragma unroll
             for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
@@ -478,7 +495,24 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS, 1) k_col(const StepAr
                     T f = a.kin_xr[F::nat(j, ii, rr)] * ey;
                     v[ii * F::RL + rr].x *= f;
                     v[ii * F::RL + rr].y *= f;
+                    if constexpr (MODE == 2) {   // merged kinetic halves: see k_col_p (gpe_pair.cuh)
+                        acc = fma(v[ii * F::RL + rr].x, v[ii * F::RL + rr].x, fma(v[ii * F::RL + rr].y, v[ii * F::RL + rr].y, acc));
+                        const T f2 = f * bigp;
+                        v[ii * F::RL + rr].x *= f2;
+                        v[ii * F::RL + rr].y *= f2;
+                    }
                 }
+            if constexpr (MODE == 2) {
+                __shared__ double redk[32];
+                const double sk = warp_sum((double)acc);
+                if ((threadIdx.x & 31) == 0) redk[threadIdx.x >> 5] = sk;
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    double t = 0.0;
+                    for (int q = 0; q < G::THREADS / 32; ++q) t += redk[q];
+                    a.fin.partials_k[(size_t)b * a.fin.cpmk + blockIdx.x] = t;
+                }
+            }
         } else {
             // kinetic factor (1+a)(1+b)/P with a, b = exp(-i k^2 dt/2) - 1 of the two axes, applied
             // as v/P + v*g, g = a' + b' + a'b (a' = a/P from the x table, b' = b/P): see
@@ -660,7 +694,10 @@ template <typename T, int N> struct Launch {
     static cudaError_t col(const A &a, bool imag, int mode, cudaStream_t s) {
         dim3 grid((unsigned)(a.ny / ColGeom<T, N>::W), (unsigned)a.batch), block(ColGeom<T, N>::THREADS);
         cudaError_t e;
-        if (mode == 1) {
+        if (mode == 0 && imag && a.fin.knorm) {
+            if ((e = prep(k_col<T, N, true, 2>, col_smem())) != cudaSuccess) return e;
+            { cudaError_t le = launch_pdl(k_col<T, N, true, 2>, grid, block, col_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
+        } else if (mode == 1) {
             if ((e = prep(k_col<T, N, false, 1>, col_smem())) != cudaSuccess) return e;
             { cudaError_t le = launch_pdl(k_col<T, N, false, 1>, grid, block, col_smem(), s, use_pdl(a), a); if (le != cudaSuccess) return le; }
         } else if (imag) {
@@ -673,6 +710,7 @@ template <typename T, int N> struct Launch {
         return cudaGetLastError();
     }
     static int rows_per_cta() { return RowGeom<N>::RPC; }
+    static int cols_per_cta() { return ColGeom<T, N>::W; }
 };
 
 }  // namespace gpe

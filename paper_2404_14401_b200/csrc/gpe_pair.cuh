@@ -273,7 +273,10 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
 }
 
 // ---------------------------------------------------------------- pass B (columns)
-template <int NX, bool IMAG, bool LATE>
+// KNORM (imaginary time, T/2 V T/2 with merged kinetic halves): the tables hold HALF a kinetic step h; the factor is
+// applied twice and the k-space sum of |psi^ h / P|^2 taken in between (Parseval: the norm of the wavefunction at the
+// step boundary, FinalizeParams::partials_k)
+template <int NX, bool IMAG, bool LATE, bool KNORM = false>
 __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / ColGeomP<NX>::THREADS) k_col_p(const StepArgs<float, float2> a) {
     using G = ColGeomP<NX>;
     using F = Fft1D<NX, G::CPW, cpair>;
@@ -298,6 +301,8 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / Col
     F::fwd(v, sm, j, a.tw_x, a.tw1_x);
     if constexpr (IMAG) {
         const float2 ey = *reinterpret_cast<const float2 *>(a.kin_yr + 2 * cp);
+        float2 acc = make_float2(0.f, 0.f);
+        const float bigp = 1.0f / a.inv_p;   // nx ny: a power of two, exact
 #pragma unroll
         for (int ii = 0; ii < F::GL; ++ii)
 #pragma unroll
@@ -305,7 +310,23 @@ __global__ void __launch_bounds__(ColGeomP<NX>::THREADS, GPE_COLP_RESIDENT / Col
                 const float2 f = rmuls(ey, a.kin_xr[F::nat(j, ii, rr)]);
                 cpair &z = v[ii * F::RL + rr];
                 z.re = rmul(z.re, f); z.im = rmul(z.im, f);
+                if constexpr (KNORM) {
+                    acc = rfma(z.re, z.re, rfma(z.im, z.im, acc));
+                    const float2 f2 = rmuls(f, bigp);
+                    z.re = rmul(z.re, f2); z.im = rmul(z.im, f2);
+                }
             }
+        if constexpr (KNORM) {
+            __shared__ double redk[32];
+            const double s = warp_sum((double)acc.x + (double)acc.y);
+            if ((threadIdx.x & 31) == 0) redk[threadIdx.x >> 5] = s;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                double t = 0.0;
+                for (int q = 0; q < G::THREADS / 32; ++q) t += redk[q];
+                a.fin.partials_k[(size_t)b * a.fin.cpmk + blockIdx.x] = t;
+            }
+        }
     } else {
         // kinetic factor (1+a)(1+b)/P applied as v/P + v*g, g = a' + b' + a'b (k_col of
         // gpe_kernels.cuh); b differs between the two columns (lanes), a is common to both
@@ -341,7 +362,7 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
     using F = Fft1D<G::H, 1, cpair>;
     constexpr int H = G::H, M1 = F::M1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double red[96];
+    __shared__ double red[128];
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     float2 *sm = reinterpret_cast<float2 *>(smem_raw) + r * F::TILE;
     const long row = (long)blockIdx.x * G::RPC + r;
@@ -433,14 +454,20 @@ __global__ void __launch_bounds__(RowGeomP<NY>::THREADS, (GPE_ROWP_MINB * 128) /
             s2 = warp_sum(s2);
         }
         s0 = warp_sum(s0); s1 = warp_sum(s1);
+        double s3 = 0.0;
+        if (f.knorm) {   // the norm from pass B's k-space partial sums (merged kinetic halves, see k_col_p)
+            const double *pk = f.partials_k + (size_t)b * f.cpmk;
+            for (int q = threadIdx.x; q < f.cpmk; q += G::THREADS) s3 += __ldcg(pk + q);
+            s3 = warp_sum(s3);
+        }
         __syncthreads();
-        if (lane == 0) { red[wid] = s0; red[32 + wid] = s1; red[64 + wid] = s2; }
+        if (lane == 0) { red[wid] = s0; red[32 + wid] = s1; red[64 + wid] = s2; red[96 + wid] = s3; }
         __syncthreads();
         if (threadIdx.x == 0) {
-            double t0 = 0.0, t1 = 0.0, t2 = 0.0;
+            double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
 #pragma unroll
-            for (int q = 0; q < NW; ++q) { t0 += red[q]; t1 += red[32 + q]; t2 += red[64 + q]; }
-            finalize_member(f, b, t0, t1, t2);
+            for (int q = 0; q < NW; ++q) { t0 += red[q]; t1 += red[32 + q]; t2 += red[64 + q]; t3 += red[96 + q]; }
+            finalize_member(f, b, f.knorm ? t3 * f.kscale : t0, t1, t2);
             f.counters[b] = 0u;
         }
     }
@@ -625,6 +652,7 @@ template <int N> struct LaunchP {
     }
     static cudaError_t col(const A &a, bool imag, cudaStream_t s) {       // nx == N
         dim3 grid((unsigned)(a.ny / 2 / ColGeomP<N>::CPW), (unsigned)a.batch), block(ColGeomP<N>::THREADS);
+        if (imag && a.fin.knorm) return late(a) ? go(k_col_p<N, true, true, true>, grid, block, col_smem(), s, a) : go(k_col_p<N, true, false, true>, grid, block, col_smem(), s, a);
         if (late(a)) return imag ? go(k_col_p<N, true, true>, grid, block, col_smem(), s, a) : go(k_col_p<N, false, true>, grid, block, col_smem(), s, a);
         return imag ? go(k_col_p<N, true, false>, grid, block, col_smem(), s, a) : go(k_col_p<N, false, false>, grid, block, col_smem(), s, a);
     }

@@ -71,6 +71,12 @@ struct FinalizeParams {
     int merged;               // 1: pass C left the second half-step pending (real time, paired passes)
     int tvt;                  // 1: T/2 V T/2 ordering in real time: the pending factor takes the coefficients of THIS psi
     long long step0;          // used when advance == 0: sets the step counter
+    // T/2 V T/2 in imaginary time with merged kinetic halves (gpe_api.cu): pass B leaves per-CTA partial sums of
+    // |psi^ h / P|^2 (h = half a kinetic step) in partials_k; the last block of pass C takes the norm from them,
+    // norm = kscale * sum * dxdy (kscale = nx ny), instead of from its own real-space sum
+    int knorm, cpmk;
+    double kscale;
+    double *partials_k;       // [batch][cpmk]
 };
 
 enum : int {

@@ -21,8 +21,11 @@ Bars (north_star), all written here:
              near zero by accident.  For Theta and alpha the envelope is carried as a RELATIVE error: while
              the self-organising mode grows exponentially (config 3: from 1e-4 to 0.66 in 1500 steps) an
              error made in its amplitude early on is frozen as a relative error of Theta -- measured on B200:
-             8e-5 relative after 100 steps, unchanged at step 1000, gone once the mode saturates.  Every
-             comparison is printed with both numbers, so no row is outside silently.
+             4e-5 relative after 100 steps, unchanged at step 1000, gone once the mode saturates.  In a batch,
+             the members whose |Theta| is below Q17's clamp of 1e-2 (seed level or near threshold: SURVEY.md
+             8(c) R2 expects 1e-3 .. 2e-2 relative differences between ANY two fp32 runs there) form one
+             statistical class: each may show the relative error the worst of them has shown so far, times
+             CLASS_K.  Every comparison is printed with error, bar, floor and bound: no row is outside silently.
 """
 import os
 
@@ -46,6 +49,7 @@ REL = {"c64": 1e-5, "c128": 1e-10}
 # Measured on B200, CUDA path against the complex64 oracle, both relative to the complex128 oracle: config 3
 # Theta in the growth phase 1.8x, config 4 every quantity 0.03x - 0.3x, reduced config 5 member 3 4.7x.
 FLOOR_K = 8.0
+CLASS_K = 2.0   # factor on the envelope over the members of the near-threshold class (see the top of the file)
 E_COLS = (1, 2, 3, 4)   # e_kin, e_pot, e_int, e_cav in the observables row
 
 
@@ -124,9 +128,16 @@ def _run_cached(name, make, dtype):
         og, oo = _obs_array(plan, psi)[members], ref[f"obs_{c}"]
         of = fl[f"floor_obs_{c}"] if fl is not None else oo
         k = int(np.argmax(np.abs(og[:, 5] - oo[:, 5]) / np.maximum(np.abs(oo[:, 5]), 1e-2)))
-        env["theta"] = np.maximum(env["theta"], np.abs(of[:, 5] - oo[:, 5]) / np.maximum(np.abs(oo[:, 5]), 1e-300))
+        relf = np.abs(of[:, 5] - oo[:, 5]) / np.maximum(np.abs(oo[:, 5]), 1e-300)
+        env["theta"] = np.maximum(env["theta"], relf)
+        small = np.abs(oo[:, 5]) < 1e-2
+        if small.any():
+            env["class"] = max(env.get("class", 0.0), float(relf[small].max()))
+        fl_k = env["theta"][k]
+        if small[k]:
+            fl_k = max(fl_k, CLASS_K / FLOOR_K * env.get("class", 0.0))
         _check(f"step {c}: Theta (member {k}, {oo[k, 5]:+.4e})", abs(og[k, 5] - oo[k, 5]),
-               REL[dtype] * max(abs(oo[k, 5]), 1e-2), float(env["theta"][k] * abs(oo[k, 5])), failures)
+               REL[dtype] * max(abs(oo[k, 5]), 1e-2), float(fl_k * abs(oo[k, 5])), failures)
         Eg, Eo, Ef = og[:, E_COLS].sum(1), oo[:, E_COLS].sum(1), of[:, E_COLS].sum(1)
         k = int(np.argmax(np.abs(Eg - Eo) / np.abs(Eo)))
         env["energy"] = np.maximum(env["energy"], np.abs(Ef - Eo))
@@ -148,7 +159,11 @@ def _run_cached(name, make, dtype):
             err = np.abs(rg[:, :, col] - ro[:, :, col])
             # envelope over the run, carried as a relative error of the recorded quantity (see the top of the file)
             mag = np.maximum(np.abs(ro[:, :, col]), 1e-300)
-            floor = np.maximum.accumulate(np.abs(rf[:, :, col] - ro[:, :, col]) / mag, axis=0) * mag
+            relf = np.abs(rf[:, :, col] - ro[:, :, col]) / mag
+            own = np.maximum.accumulate(relf, axis=0)
+            small = np.abs(ro[:, :, 2]) < 1e-2                                   # the near-threshold class, by Theta
+            cls = np.maximum.accumulate(np.where(small, relf, 0.0).max(axis=1))  # its envelope over members and time
+            floor = np.where(small, np.maximum(own, CLASS_K / FLOOR_K * cls[:, None]), own) * mag
             bound = np.maximum(REL[dtype] * scale, FLOOR_K * floor)
             i, b = np.unravel_index(int(np.argmax(err / bound)), err.shape)
             _check(f"records: {nm} (worst: step {int(ro[i, b, 0])}, member {b})", float(err[i, b]),
