@@ -2,7 +2,7 @@
 //
 // At these sizes a pass is a few hundred nanoseconds of work and a step was three dependent launches of
 // about 5 us each (profiles/r01_final.md: 256^2 15.2 us per step, 0.03 of its byte roofline).  Here one
-// thread-block cluster per batch member (8 CTAs, 16 for 256^2 complex128) stays resident for the whole call:
+// thread-block cluster per batch member (8 CTAs at 64^2, 16 from 128^2 on) stays resident for the whole call:
 //   * CTA `rank` owns N / NC rows in the row phases and N / NC columns in the column phase;
 //   * the kernel boundaries between the passes become hardware cluster barriers
 //     (barrier.cluster.arrive.release / wait.acquire, about 0.2 us), the data crosses between the row and the
@@ -32,7 +32,7 @@ template <typename T, int N> struct ChipGeom {
     static constexpr int NC = N >= GPE_CHIP_NC16_MIN ? 16 : 8;   // CTAs per cluster (16 needs the non-portable opt-in)
     static constexpr int RB = N / NC;                                  // rows (and columns) per CTA
     static constexpr int TPF = N / 16;                                 // threads per transform
-    static constexpr int THREADS = RB * TPF;                           // 64^2: 32, 128^2: 128, 256^2: 512 (c64) / 256 (c128)
+    static constexpr int THREADS = RB * TPF;                           // 64^2: 32, 128^2: 64, 256^2: 256
     using FR = Fft1D<N, 1, cx<T>>;                                     // a row in its own SLOTS-element tile
     using FC = Fft1D<N, RB, cx<T>>;                                    // RB columns interleaved in one tile
     static constexpr size_t SMEM = sizeof(cx<T>) * (size_t)RB * FR::SLOTS;
@@ -84,8 +84,7 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
     C *pcol = psi + col;
 
     FinalizeParams f = a.fin;
-    f.st = &lms - b;                                   // f.st[b] is the local copy
-    f.call = &lcall;
+    f.call = &lcall;                                   // the member's state is passed as `&lms` where it is needed
     if (tid == 0) {
         lms = a.fin.st[b];
         lcall = *a.fin.call;
@@ -113,7 +112,7 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
             for (int rr = 0; rr < FR::RL; ++rr) prow[FR::nat(j, ii, rr)] = v[ii * FR::RL + rr];
         cluster.sync();
         // ---- pass B: FFT along x, kinetic factor, inverse FFT along x on this CTA's columns
-        if (tid == 0 && f.prepared) prepare_member(f, b);
+        if (tid == 0 && f.prepared) prepare_member(f, b, &lms);
 #pragma unroll
         for (int k = 0; k < 16; ++k) v[k] = __ldcg(pcol + (size_t)(jc + FC::M1 * k) * N);
         FC::fwd(v, smc, jc, a.tw_x, a.tw1_x);
@@ -181,7 +180,7 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
         if (tid == 0) {
             double t0 = 0.0, t1 = 0.0, t2 = 0.0;
             for (int q = 0; q < NC; ++q) { t0 += part[q][0]; t1 += part[q][1]; t2 += part[q][2]; }
-            finalize_member(f, b, t0, t1, t2);
+            finalize_member(f, b, t0, t1, t2, &lms);
         }
         __syncthreads();
     }

@@ -93,14 +93,16 @@ __device__ inline void step_coefficients(const FinalizeParams &f, int b, long lo
     }
 }
 // Called by one thread of pass B per member while step n runs: coefficients of step n + 1.
-__device__ inline void prepare_member(const FinalizeParams &f, int b) {
-    MemberState &s = f.st[b];
+// `local`: the member's state when it does not live at f.st[b] (the cluster kernel keeps a copy per CTA)
+__device__ inline void prepare_member(const FinalizeParams &f, int b, MemberState *local = nullptr) {
+    MemberState &s = local ? *local : f.st[b];
     step_coefficients(f, b, s.step + 1, 0.0, s.nA, s.nKre, s.nKim, s.nKc, s.nPre, s.nPim, s.nPc);
 }
 
 // Called by one thread of the last block of member b with the raw sums over the stored psi.
-__device__ inline void finalize_member(const FinalizeParams &f, int b, double sum_n, double sum_t, double sum_b) {
-    MemberState &s = f.st[b];
+__device__ inline void finalize_member(const FinalizeParams &f, int b, double sum_n, double sum_t, double sum_b,
+                                       MemberState *local = nullptr) {
+    MemberState &s = local ? *local : f.st[b];
     double norm = sum_n * f.dxdy, theta = sum_t * f.dxdy, bunch = sum_b * f.dxdy;
     if (!(norm == norm) || norm > 1e300 || norm < 0.0 || (f.normalise && !(norm > 0.0))) *f.nonfinite = 1;
     long long n1;

@@ -443,3 +443,24 @@ def test_measure_roofs_is_sane():
     plan = _gpu_plan(p, "c64")
     plan.evolve(_to_dev(p["psi0"], "c64"), 1e-3, 2, "real")
     plan.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_two_pass_with_midpoint_schedule_and_batch(monkeypatch, dtype):
+    """The fused C+A kernel takes A_{n+1} from the coefficients pass B prepared: with mid-step sampling of a ramp
+    (sched_midpoint) and a different schedule per member, on a non-square grid (multi-launch 2-pass path)."""
+    monkeypatch.delenv("GPE_NO_FUSE", raising=False)
+    p = _local_workload(256, 128, batch=2)
+    p["sched_midpoint"] = 1
+    p["sched_step"] = np.array([0.0, 5.0, 5.0, 30.0])
+    p["sched_amp"] = np.array([[6.0, 6.0, 9.0, 12.0], [0.0, 10.0, 3.0, 0.0]])
+    plan = _gpu_plan(p, dtype)
+    psi, ref = _to_dev(p["psi0"], dtype), _oracle_input(p["psi0"], dtype)
+    o = Oracle(p)
+    rg = plan.evolve(psi, 1e-3, 33, "real", record_every=1).cpu().numpy()
+    ro = o.evolve(ref, 1e-3, 33, False, record_every=1)
+    e = _rel(psi.cpu().numpy(), ref)
+    assert e <= 33 * PER_STEP[dtype], f"{e:.3e}"
+    assert np.allclose(rg[:, :, 5], ro[:, :, 5], rtol=1e-14, atol=1e-300)
+    assert np.allclose(rg[:, :, 1], ro[:, :, 1], rtol=1e-5 if dtype == "c64" else 1e-10, atol=0)
+    plan.close()
