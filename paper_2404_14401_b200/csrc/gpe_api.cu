@@ -49,6 +49,7 @@ struct gpe_plan {
     void *tw_x = nullptr, *tw_y = nullptr;
     void *tw1_x = nullptr, *tw1_y = nullptr;
     void *tw_hy = nullptr, *tw1_hy = nullptr;  // length ny/2 (paired row passes)
+    void *tw1e_x = nullptr, *tw1e_y = nullptr; // first-stage twiddles for eight points per thread (cluster kernel)
     void *ytab2 = nullptr;
     void *kin_x = nullptr, *kin_y = nullptr, *kin_y2 = nullptr;
     double kin_dt = 0.0;
@@ -198,6 +199,14 @@ template <typename T> gpe_status make_twiddles(gpe_plan *p) {
                 re[k * m1 + j] = cos(a1); im[k * m1 + j] = sin(a1);
             }
         s = upload_cplx<T>(p, ax == 0 ? &p->tw1_x : &p->tw1_y, re, im);
+        if (s != GPE_OK) return s;
+        const int m8 = n / 8;   // the same table for eight points per thread (gpe_chip.cuh)
+        for (int k = 0; k < 8; ++k)
+            for (int j = 0; j < m8; ++j) {
+                double a1 = -2.0 * kPi * (double)((long)k * j % n) / (double)n;
+                re[k * m8 + j] = cos(a1); im[k * m8 + j] = sin(a1);
+            }
+        s = upload_cplx<T>(p, ax == 0 ? &p->tw1e_x : &p->tw1e_y, re, im);
         if (s != GPE_OK) return s;
     }
     {   // the same two tables for length ny/2 (gpe_pair.cuh, passes A and C)
@@ -502,6 +511,7 @@ template <typename T> StepArgs<T, cx<T>> base_args(gpe_plan *p, const void *src,
     a.g = (const T *)p->g;
     a.tw_x = (const cx<T> *)p->tw_x; a.tw_y = (const cx<T> *)p->tw_y;
     a.tw1_x = (const cx<T> *)p->tw1_x; a.tw1_y = (const cx<T> *)p->tw1_y;
+    a.tw1e_x = (const cx<T> *)p->tw1e_x; a.tw1e_y = (const cx<T> *)p->tw1e_y;
     a.tw_hy = (const cx<T> *)p->tw_hy; a.tw1_hy = (const cx<T> *)p->tw1_hy;
     a.ytab2 = (const T *)p->ytab2;
     a.kin_xc = (const cx<T> *)p->kin_x; a.kin_yc = (const cx<T> *)p->kin_y;
@@ -1093,7 +1103,7 @@ gpe_status gpe_plan_destroy(gpe_plan *p) {
     cudaStreamSynchronize(p->stream);
     if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
-    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->kin_y2, p->kinh_x, p->kinh_y, p->kinh_y2, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
+    void *bufs[] = {p->d_call, p->tw_x, p->tw_y, p->tw1_x, p->tw1_y, p->tw1e_x, p->tw1e_y, p->tw_hy, p->tw1_hy, p->ytab2, p->kin_x, p->kin_y, p->kin_y2, p->kinh_x, p->kinh_y, p->kinh_y2, p->vx, p->vy, p->latx, p->laty, p->cavx, p->cavy,
                     p->ytab, p->g, p->v2d, p->st, p->partials, p->partials_b, p->partials_k, p->d_u0, p->counters, p->nonfinite, p->d_sched_step,
                     p->d_sched_amp, p->d_eta, p->d_natoms, p->d_delta, p->d_kappa, p->d_probe_omega, p->d_probe_delta,
                     p->d_probe_phi, p->scratch, p->obs_dev,

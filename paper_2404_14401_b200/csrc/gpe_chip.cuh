@@ -25,18 +25,28 @@
 #ifndef GPE_CHIP_NC16_MIN
 #define GPE_CHIP_NC16_MIN 128   // from this size on 16 CTAs per cluster
 #endif
+// Points per thread (Fft1D's P).  Eight points per thread give twice the warps and half the dependent chain of
+// sixteen.  Measured on B200, us per step (sweep / pulse / cavity workloads, complex64), P = 8 against P = 16:
+// 64^2 4.7 / 4.7 / 5.6 against 7.3 / 7.1 / 8.0 (complex128 5.9 against 8.9); 128^2 6.6 / 6.6 / 7.6 against 7.8 / 7.5 / 8.4;
+// 256^2 12.0 / 11.2 / 12.2 against 10.3 / 9.7 / 10.7 (one more exchange per transform).  The fp32 norm drift of a
+// real-time step (a fixed bias of the few distinct rounded twiddles a small transform uses) is -6.2e-8 against
+// -5.6e-8 at 64^2 but -1.0e-7 against -2.6e-8 at 128^2: eight points per thread at 64^2 only.
+#ifndef GPE_CHIP_P8_MAX_N
+#define GPE_CHIP_P8_MAX_N 64
+#endif
 namespace gpe {
 namespace cg = cooperative_groups;
 
 template <typename T, int N> struct ChipGeom {
     static constexpr int NC = N >= GPE_CHIP_NC16_MIN ? 16 : 8;   // CTAs per cluster (16 needs the non-portable opt-in)
+    static constexpr int P = N <= GPE_CHIP_P8_MAX_N ? 8 : 16;          // points per thread
     static constexpr int RB = N / NC;                                  // rows (and columns) per CTA
-    static constexpr int TPF = N / 16;                                 // threads per transform
+    static constexpr int TPF = N / P;                                  // threads per transform
     static constexpr int THREADS = RB * TPF;                           // 64^2: 32, 128^2: 64, 256^2: 256
-    using FR = Fft1D<N, 1, cx<T>>;                                     // a row in its own SLOTS-element tile
-    using FC = Fft1D<N, RB, cx<T>>;                                    // RB columns interleaved in one tile
+    using FR = Fft1D<N, 1, cx<T>, P>;                                  // a row in its own SLOTS-element tile
+    using FC = Fft1D<N, RB, cx<T>, P>;                                 // RB columns interleaved in one tile
     static constexpr size_t SMEM = sizeof(cx<T>) * (size_t)RB * FR::SLOTS;
-    static_assert(N >= 64 && N <= 256 && RB >= 1 && THREADS >= 32 && THREADS <= 512, "small grids only");
+    static_assert(N >= 64 && N <= 256 && RB >= 1 && THREADS >= 32 && THREADS <= 512 && THREADS % 32 == 0, "small grids only");
 };
 
 // sum over the CTA of three doubles (fixed order), result valid in thread 0
@@ -60,7 +70,7 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
     using FR = typename G::FR;
     using FC = typename G::FC;
     using C = cx<T>;
-    constexpr int NC = G::NC, RB = G::RB, TPF = G::TPF, M1 = FR::M1;
+    constexpr int NC = G::NC, RB = G::RB, TPF = G::TPF, M1 = FR::M1, P = G::P;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
     __shared__ MemberState lms;          // this CTA's copy of the member's state (identical in all CTAs)
@@ -83,6 +93,8 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
     C *prow = psi + (size_t)i * N;
     C *pcol = psi + col;
 
+    // first-stage twiddles transposed for P points per thread: [P][N/P] (the plan keeps both layouts)
+    const C *tw1x = P == 16 ? a.tw1_x : a.tw1e_x, *tw1y = P == 16 ? a.tw1_y : a.tw1e_y;
     FinalizeParams f = a.fin;
     f.call = &lcall;                                   // the member's state is passed as `&lms` where it is needed
     if (tid == 0) {
@@ -92,9 +104,9 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
     }
     __syncthreads();
 
-    C v[16];
+    C v[P];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) v[k] = __ldcg(prow + j + M1 * k);
+    for (int k = 0; k < P; ++k) v[k] = __ldcg(prow + j + M1 * k);
 
     for (long step = 0; step < n_steps; ++step) {
         // ---- pass A: potential half-step (merged with the pending one in real time) and FFT along y
@@ -105,7 +117,7 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
             potential_step16<T, IMAG, false, M1>(v, a, b, i, j, (T)lms.scale, pend ? T(2) : T(1), (T)(pend ? lms.A + lms.A_pend : lms.A),
                                                  (T)(pend ? lms.C + lms.C_pend : lms.C), (T)(pend ? lms.D + lms.D_pend : lms.D) * cx2, sn, st);
         }
-        FR::fwd(v, smr, j, a.tw_y, a.tw1_y);
+        FR::fwd(v, smr, j, a.tw_y, tw1y);
 #pragma unroll
         for (int ii = 0; ii < FR::GL; ++ii)
 #pragma unroll
@@ -114,8 +126,8 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
         // ---- pass B: FFT along x, kinetic factor, inverse FFT along x on this CTA's columns
         if (tid == 0 && f.prepared) prepare_member(f, b, &lms);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = __ldcg(pcol + (size_t)(jc + FC::M1 * k) * N);
-        FC::fwd(v, smc, jc, a.tw_x, a.tw1_x);
+        for (int k = 0; k < P; ++k) v[k] = __ldcg(pcol + (size_t)(jc + FC::M1 * k) * N);
+        FC::fwd(v, smc, jc, a.tw_x, tw1x);
         if constexpr (IMAG) {
             const T ey = a.kin_yr[col];
 #pragma unroll
@@ -144,20 +156,20 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
                     z.x = ox; z.y = oy;
                 }
         }
-        FC::inv(v, smc, jc, a.tw_x, a.tw1_x);
+        FC::inv(v, smc, jc, a.tw_x, tw1x);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) pcol[(size_t)(jc + FC::M1 * k) * N] = v[k];
+        for (int k = 0; k < P; ++k) pcol[(size_t)(jc + FC::M1 * k) * N] = v[k];
         cluster.sync();
         // ---- pass C: inverse FFT along y, second half-step (left pending in real time), sums
 #pragma unroll
         for (int ii = 0; ii < FR::GL; ++ii)
 #pragma unroll
             for (int rr = 0; rr < FR::RL; ++rr) v[ii * FR::RL + rr] = __ldcg(prow + FR::nat(j, ii, rr));
-        FR::inv(v, smr, j, a.tw_y, a.tw1_y);
+        FR::inv(v, smr, j, a.tw_y, tw1y);
         T sn = T(0), st = T(0);
         if (!IMAG && f.merged) {
 #pragma unroll
-            for (int k = 0; k < 16; ++k) {
+            for (int k = 0; k < P; ++k) {
                 const T d = v[k].x * v[k].x + v[k].y * v[k].y;
                 sn += d;
                 if (a.flags & F_CAVITY) st = fma(d, a.ytab[4 * (j + M1 * k) + 2], st);
@@ -185,7 +197,7 @@ __global__ void __launch_bounds__(ChipGeom<T, N>::THREADS, 1) k_chip(const StepA
         __syncthreads();
     }
 #pragma unroll
-    for (int k = 0; k < 16; ++k) prow[j + M1 * k] = v[k];
+    for (int k = 0; k < P; ++k) prow[j + M1 * k] = v[k];
     if (rank == 0 && tid == 0) a.fin.st[b] = lms;
 }
 

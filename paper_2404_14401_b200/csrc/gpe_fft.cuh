@@ -166,43 +166,50 @@ template <int R, int SIGN, typename E> __device__ __forceinline__ void dft(E *v)
 // table fetch (plain cached load; the read-only path, __ldg, measured no faster on B200)
 template <typename C> __device__ __forceinline__ C ldtw(const C *__restrict__ t, int i) { return t[i]; }
 
-template <int N> struct Fact;
-template <> struct Fact<64> { static constexpr int R2 = 4, R3 = 1; };
-template <> struct Fact<128> { static constexpr int R2 = 8, R3 = 1; };
-template <> struct Fact<256> { static constexpr int R2 = 16, R3 = 1; };
-template <> struct Fact<512> { static constexpr int R2 = 8, R3 = 4; };
-template <> struct Fact<1024> { static constexpr int R2 = 8, R3 = 8; };
-template <> struct Fact<2048> { static constexpr int R2 = 16, R3 = 8; };
+// N = P * R2 * R3: the radices of the second and third stage for P points per thread
+template <int N, int P = 16> struct Fact;
+template <> struct Fact<64, 16> { static constexpr int R2 = 4, R3 = 1; };
+template <> struct Fact<128, 16> { static constexpr int R2 = 8, R3 = 1; };
+template <> struct Fact<256, 16> { static constexpr int R2 = 16, R3 = 1; };
+template <> struct Fact<512, 16> { static constexpr int R2 = 8, R3 = 4; };
+template <> struct Fact<1024, 16> { static constexpr int R2 = 8, R3 = 8; };
+template <> struct Fact<2048, 16> { static constexpr int R2 = 16, R3 = 8; };
+// eight points per thread: twice the threads, half the dependent chain (the cluster kernel of gpe_chip.cuh)
+template <> struct Fact<64, 8> { static constexpr int R2 = 8, R3 = 1; };
+template <> struct Fact<128, 8> { static constexpr int R2 = 4, R3 = 4; };
+template <> struct Fact<256, 8> { static constexpr int R2 = 8, R3 = 4; };
 
-// One 1-D FFT of length N worked on by N/16 threads (index j), S = element stride of the
-// shared-memory tile (1 for a row, W for a tile of W columns).  tw[m] = exp(-2 pi i m / N).
-// E = element type (see the top of this file); twiddles are always one cx<T> per element.
-template <int N, int S, typename E> struct Fft1D {
+// One 1-D FFT of length N worked on by N/P threads (index j), every thread owning P points (16, or 8) at every
+// stage; S = element stride of the shared-memory tile (1 for a row, W for a tile of W columns).
+// tw[m] = exp(-2 pi i m / N).  E = element type (see the top of this file); twiddles are always one cx<T> per element.
+template <int N, int S, typename E, int P = 16> struct Fft1D {
     using T = typename El<E>::T;
     using C = cx<T>;
     using SE = typename El<E>::SE;
-    static constexpr int TPF = N / 16;
-    static constexpr int M1 = N / 16;
-    static constexpr int R2 = Fact<N>::R2, R3 = Fact<N>::R3;
+    static constexpr int LOGP = P == 16 ? 4 : 3;
+    static_assert(P == 16 || P == 8, "16 or 8 points per thread");
+    static constexpr int TPF = N / P;
+    static constexpr int M1 = N / P;
+    static constexpr int R2 = Fact<N, P>::R2, R3 = Fact<N, P>::R3;
     static constexpr int NST = R3 > 1 ? 3 : 2;
-    static constexpr int SLOTS = N + 16;           // one padding slot per k1 block
+    static constexpr int SLOTS = N + P;            // one padding slot per k1 block
     static constexpr int PLANE = SLOTS * S;        // distance between the planes of a cpair tile
     static constexpr int TILE = SLOTS * S * El<E>::PLANES;  // SE elements of one tile (S transforms)
     static constexpr int RL = NST == 3 ? R3 : R2;  // radix of the last stage
-    static constexpr int GL = 16 / RL;             // butterflies per thread in the last stage
+    static constexpr int GL = P / RL;              // butterflies per thread in the last stage
 
     __device__ __forceinline__ static int phys(int s) { return (s + s / M1) * S; }
 
     // natural output index of register (i*RL + r) of thread j after the forward transform
     __device__ __forceinline__ static int nat(int j, int i, int r) {
         int t = j + i * TPF;
-        int k1 = t & 15, u = t >> 4;
-        return NST == 3 ? k1 + 16 * u + 16 * R2 * r : k1 + 16 * r;
+        int k1 = t & (P - 1), u = t >> LOGP;
+        return NST == 3 ? k1 + P * u + P * R2 * r : k1 + P * r;
     }
 
     template <int R, int Mp> __device__ __forceinline__ static int base_slot(int t, int &q) {
         constexpr int M = Mp / R;
-        int k1 = t & 15, u = t >> 4;
+        int k1 = t & (P - 1), u = t >> LOGP;
         int blk = u / M;
         q = u % M;
         return k1 * M1 + blk * Mp + q;
@@ -210,7 +217,7 @@ template <int N, int S, typename E> struct Fft1D {
 
     template <int R, int Mp, bool LAST>
     __device__ __forceinline__ static void stage_fwd(E *v, SE *sm, int j, const C *__restrict__ tw) {
-        constexpr int G = 16 / R, M = Mp / R;
+        constexpr int G = P / R, M = Mp / R;
 #pragma unroll
         for (int i = 0; i < G; ++i) {
             int q, b = base_slot<R, Mp>(j + i * TPF, q);
@@ -233,7 +240,7 @@ template <int N, int S, typename E> struct Fft1D {
 
     template <int R, int Mp, bool LAST>
     __device__ __forceinline__ static void stage_inv(E *v, SE *sm, int j, const C *__restrict__ tw) {
-        constexpr int G = 16 / R, M = Mp / R;
+        constexpr int G = P / R, M = Mp / R;
         if constexpr (!LAST) {
 #pragma unroll
             for (int i = 0; i < G; ++i) {
@@ -261,8 +268,8 @@ template <int N, int S, typename E> struct Fft1D {
     // indices of the two transforms: register (2 i + w) * RL + r = X_w[nat_t(t, r)].  Needs GL >= 2.
     static constexpr int RLM = NST == 3 ? M1 / R2 : M1;   // Mp of the last stage
     __device__ __forceinline__ static int nat_t(int t, int r) {
-        int k1 = t & 15, u = t >> 4;
-        return NST == 3 ? k1 + 16 * u + 16 * R2 * r : k1 + 16 * r;
+        int k1 = t & (P - 1), u = t >> LOGP;
+        return NST == 3 ? k1 + P * u + P * R2 * r : k1 + P * r;
     }
     __device__ __forceinline__ static void last_fwd_pair(E *v, const SE *sm0, const SE *sm1, int u) {
         constexpr int M = RLM / RL;
@@ -297,11 +304,11 @@ template <int N, int S, typename E> struct Fft1D {
     template <typename Sync, typename Sync2>
     __device__ __forceinline__ static void fwd_pairlast(E *v, SE *sm, const SE *sm0, const SE *sm1, int j, int u,
                                                         const C *__restrict__ tw, const C *__restrict__ tw1, Sync SYNC, Sync2 SYNC2) {
-        dft<16, -1, E>(v);
+        dft<P, -1, E>(v);
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], ldtw(tw1, k * M1 + j));
+        for (int k = 1; k < P; ++k) v[k] = cmul(v[k], ldtw(tw1, k * M1 + j));
 #pragma unroll
-        for (int k = 0; k < 16; ++k) sst<PLANE>(sm, phys(j + M1 * k), v[k]);
+        for (int k = 0; k < P; ++k) sst<PLANE>(sm, phys(j + M1 * k), v[k]);
         if constexpr (NST == 3) {
             SYNC();
             stage_fwd<R2, M1, false>(v, sm, j, tw);
@@ -320,10 +327,10 @@ template <int N, int S, typename E> struct Fft1D {
             SYNC();
         }
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = sld<PLANE, E>(sm, phys(j + M1 * k));
+        for (int k = 0; k < P; ++k) v[k] = sld<PLANE, E>(sm, phys(j + M1 * k));
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], ldtw(tw1, k * M1 + j));
-        dft<16, +1, E>(v);
+        for (int k = 1; k < P; ++k) v[k] = cmulc(v[k], ldtw(tw1, k * M1 + j));
+        dft<P, +1, E>(v);
     }
 
     // in: v[a] = x[j + (N/16) a].  out: v[i*RL + r] = X[nat(j,i,r)] (unnormalised, e^{-i}).
@@ -335,11 +342,11 @@ template <int N, int S, typename E> struct Fft1D {
     template <typename Sync>
     __device__ __forceinline__ static void fwd(E *v, SE *sm, int j, const C *__restrict__ tw,
                                                const C *__restrict__ tw1, Sync SYNC) {
-        dft<16, -1, E>(v);
+        dft<P, -1, E>(v);
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], ldtw(tw1, k * M1 + j));
+        for (int k = 1; k < P; ++k) v[k] = cmul(v[k], ldtw(tw1, k * M1 + j));
 #pragma unroll
-        for (int k = 0; k < 16; ++k) sst<PLANE>(sm, phys(j + M1 * k), v[k]);
+        for (int k = 0; k < P; ++k) sst<PLANE>(sm, phys(j + M1 * k), v[k]);
         SYNC();
         stage_fwd<R2, M1, NST == 2>(v, sm, j, tw);
         if constexpr (NST == 3) {
@@ -366,10 +373,10 @@ template <int N, int S, typename E> struct Fft1D {
         }
         SYNC();
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = sld<PLANE, E>(sm, phys(j + M1 * k));
+        for (int k = 0; k < P; ++k) v[k] = sld<PLANE, E>(sm, phys(j + M1 * k));
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], ldtw(tw1, k * M1 + j));
-        dft<16, +1, E>(v);
+        for (int k = 1; k < P; ++k) v[k] = cmulc(v[k], ldtw(tw1, k * M1 + j));
+        dft<P, +1, E>(v);
     }
     __device__ __forceinline__ static void inv(E *v, SE *sm, int j, const C *__restrict__ tw,
                                                const C *__restrict__ tw1) {

@@ -316,8 +316,8 @@ __device__ __forceinline__ void sincosm1_small(double w, double *s, double *cm1)
 // phase applied -- with ONE warp-uniform decision between the small-angle polynomial and the
 // general path, so the common case has no per-point branch at all.
 // REDUCE: also returns sum |psi_new|^2 and sum cos(k_c y) |psi_new|^2 over the 16 points.
-template <typename T, bool IMAG, bool REDUCE, int M1>
-__device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<T, cx<T>> &a, int b, int i, int j,
+template <typename T, bool IMAG, bool REDUCE, int M1, int P = 16>
+__device__ __forceinline__ void potential_step16(cx<T> (&v)[P], const StepArgs<T, cx<T>> &a, int b, int i, int j,
                                                  T scale, T fac, T A, T Cc, T vadd, T &sn, T &st) {
     using V4 = typename Vec4<T>::type;
     const int flags = a.flags;
@@ -331,9 +331,9 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
     const T g = (flags & F_HAS_G) ? fac * a.g[b] : T(0);
     const T hdt = a.half_dt;
     const V4 *__restrict__ yt = reinterpret_cast<const V4 *>(a.ytab);
-    T w[16];
+    T w[P];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
+    for (int k = 0; k < P; ++k) {
         const V4 t = yt[j + M1 * k];
         if constexpr (IMAG) { v[k].x *= scale; v[k].y *= scale; }  // the lazy scale is 1 in real time
         const T d = v[k].x * v[k].x + v[k].y * v[k].y;
@@ -343,11 +343,11 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
     if (flags & F_HAS_V2D) {
         const T *__restrict__ v2 = a.v2d + ((flags & F_V2D_BATCHED) ? (size_t)b * a.nx * a.ny : 0) + (size_t)i * a.ny;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) w[k] = fma(v2[j + M1 * k], fac * hdt, w[k]);
+        for (int k = 0; k < P; ++k) w[k] = fma(v2[j + M1 * k], fac * hdt, w[k]);
     }
     if constexpr (IMAG) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
+        for (int k = 0; k < P; ++k) {
             const T e = exp_t(-w[k]);
             v[k].x *= e; v[k].y *= e;
         }
@@ -357,10 +357,10 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
         //   |w| <= 0.5 : degree-9 / degree-8 polynomials;   else: library range reduction
         float wmax = 0.f;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) wmax = fmaxf(wmax, fabsf(w[k]));
+        for (int k = 0; k < P; ++k) wmax = fmaxf(wmax, fabsf(w[k]));
         if (__all_sync(0xffffffffu, wmax <= 0.03125f)) {
 #pragma unroll
-            for (int k = 0; k < 16; ++k) {
+            for (int k = 0; k < P; ++k) {
                 const float w2 = w[k] * w[k];
                 const float sn_ = -fmaf(w[k] * w2, -1.6666667e-1f, w[k]);   // sin(-w)
                 const float cm1 = w2 * fmaf(w2, 4.1666667e-2f, -0.5f);
@@ -370,7 +370,7 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
             }
         } else if (__all_sync(0xffffffffu, wmax <= 0.5f)) {
 #pragma unroll
-            for (int k = 0; k < 16; ++k) {
+            for (int k = 0; k < P; ++k) {
                 float sn_, cm1;
                 sincosm1_small(-w[k], &sn_, &cm1);
                 const float nx_ = fmaf(v[k].x, cm1, fmaf(-v[k].y, sn_, v[k].x));
@@ -379,7 +379,7 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
             }
         } else {
 #pragma unroll
-            for (int k = 0; k < 16; ++k) {
+            for (int k = 0; k < P; ++k) {
                 float sn_, cm1;
                 sincosm1_general(-w[k], &sn_, &cm1);
                 const float nx_ = fmaf(v[k].x, cm1, fmaf(-v[k].y, sn_, v[k].x));
@@ -392,10 +392,10 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
         // (next terms 4e-20 / 6e-22 relative), the library's range reduction otherwise
         T wmax = T(0);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) wmax = fmax(wmax, fabs(w[k]));
+        for (int k = 0; k < P; ++k) wmax = fmax(wmax, fabs(w[k]));
         const bool small = __all_sync(0xffffffffu, wmax <= T(0.5));
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
+        for (int k = 0; k < P; ++k) {
             T sn_, cm1;
             if (small) sincosm1_small(-w[k], &sn_, &cm1);
             else sincosm1_t(-w[k], &sn_, &cm1);
@@ -406,7 +406,7 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[16], const StepArgs<
     if constexpr (REDUCE) {
         sn = T(0); st = T(0);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
+        for (int k = 0; k < P; ++k) {
             const T d = v[k].x * v[k].x + v[k].y * v[k].y;
             sn += d;
             if (flags & F_CAVITY) st = fma(d, a.ytab[4 * (j + M1 * k) + 2], st);

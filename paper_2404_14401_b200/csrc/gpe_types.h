@@ -105,6 +105,7 @@ template <typename T, typename C> struct StepArgs {
     T half_dt;                     // dt/2
     const C *tw_x, *tw_y;          // exp(-2 pi i m / nx), exp(-2 pi i m / ny)
     const C *tw1_x, *tw1_y;        // first-stage twiddles transposed: [16][n/16], exp(-2 pi i k j / n)
+    const C *tw1e_x, *tw1e_y;      // the same for eight points per thread: [8][n/8] (cluster kernel, n <= 256)
     const C *tw_hy, *tw1_hy;       // the same two tables for length ny/2 (paired row passes, gpe_pair.cuh)
     const T *ytab2;                // [ny/2][8] = {vy[n], vy[n+ny/2], lat[n], lat[n+ny/2], cav[n], cav[n+ny/2], 0, 0}
     const C *kin_xc, *kin_yc;      // real time: (exp(-i kx^2 dt/2) - 1)/(nx ny), exp(-i ky^2 dt/2) - 1

@@ -363,12 +363,19 @@ def test_full_cavity_model_parity(nx, ny, mode, dtype):
     e = _rel(psi.cpu().numpy(), ref)
     assert e <= 20 * PER_STEP[dtype], f"{e:.3e}"
     tol = 1e-5 if dtype == "c64" else 1e-10
-    for c in (1, 2, 3, 4, 5):
+    for c in (1, 2, 5):
         assert np.all(np.abs(rg[:, :, c] - ro[:, :, c]) <= tol * np.maximum(np.abs(ro[:, :, c]), 1e-2)), c
+    # alpha = K Theta (+ the probe term, member 0 in real time): reading Q17's bound on Theta carried through
+    # |K| = N eta / |Delta~ + i kappa|, taken from the probe-free member (Q17)
+    K1 = np.hypot(ro[:, 1, 3], ro[:, 1, 4]) / np.maximum(np.abs(ro[:, 1, 2]), 1e-300)
+    gain = np.maximum(1.0, K1.max())
+    for c in (3, 4):
+        assert np.all(np.abs(rg[:, :, c] - ro[:, :, c]) <= tol * np.maximum(np.abs(ro[:, :, c]), 1e-2 * gain)), c
     og, oo = plan.observables(psi)[0], o.observables(ref)[0]
     for b in range(2):
         for k in ("norm", "theta", "re_alpha", "im_alpha", "e_cav"):
-            assert abs(og[b][k] - oo[b][k]) <= tol * max(abs(oo[b][k]), 1e-2), (b, k)
+            g = gain if k in ("re_alpha", "im_alpha") else 1.0
+            assert abs(og[b][k] - oo[b][k]) <= tol * max(abs(oo[b][k]), 1e-2 * g), (b, k)
     # U0 matters at the level the test resolves: the recorded field of member 0 moves by > 10 %
     # (dispersive shift), and in real time (probe-driven field) psi itself by > 10 tolerances
     pn = dict(p); pn["cav_u0"] = np.array([0.0, 0.0])
