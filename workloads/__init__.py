@@ -231,3 +231,49 @@ def _select(p: dict, idx: list) -> dict:
     if p.get("psi0") is not None and np.asarray(p["psi0"]).ndim == 3:
         q["psi0"] = np.ascontiguousarray(np.asarray(p["psi0"])[idx])
     return q
+
+
+# ---------------------------------------------------------------- three dimensions
+def noisy_gaussian3(nx: int, ny: int, nz: int, Lx: float, Ly: float, Lz: float, sigma=(1.5, 1.5, 1.5),
+                    seed: int = 1234, noise: float = 0.05) -> np.ndarray:
+    """psi0[z, x, y] = exp(-x^2/(2 sx^2) - y^2/(2 sy^2) - z^2/(2 sz^2)) * (1 + noise*xi), xi = (2u1-1) + i(2u2-1),
+    u1 then u2 drawn as rng.random((nz, nx, ny)) from numpy default_rng(seed); normalised to
+    sum |psi|^2 dx dy dz = 1.  complex128, layout [nz][nx][ny] (y fastest)."""
+    x = axis(nx, Lx)[None, :, None]
+    y = axis(ny, Ly)[None, None, :]
+    z = axis(nz, Lz)[:, None, None]
+    sx, sy, sz = sigma
+    psi = np.exp(-x * x / (2.0 * sx * sx) - y * y / (2.0 * sy * sy) - z * z / (2.0 * sz * sz)).astype(np.complex128)
+    if noise != 0.0:
+        rng = np.random.default_rng(seed)
+        u1 = rng.random((nz, nx, ny))
+        u2 = rng.random((nz, nx, ny))
+        psi = psi * (1.0 + noise * ((2.0 * u1 - 1.0) + 1j * (2.0 * u2 - 1.0)))
+    dV = (Lx / nx) * (Ly / ny) * (Lz / nz)
+    psi /= math.sqrt(float(np.sum(np.abs(psi) ** 2)) * dV)
+    return np.ascontiguousarray(psi)
+
+
+def config3d(nx: int = 128, ny: int | None = None, nz: int | None = None, L: float = 16.0, g: float = 50.0,
+             w2=(1.0, 1.44, 0.64), dtype: str = "c64", dimple: float = 2.0, separable: bool = True,
+             mode: str = "imag", dt: float = 1e-3, n_steps: int = 100, seed: int = 11):
+    """The 3-D stand-in workload (the paper has none: three dimensions is the first item of its outlook,
+    PAPER.md:231): an anisotropic harmonic trap w2 = (wx^2, wy^2, wz^2) given as the separable arrays vx, vy, vz,
+    plus a non-separable Gaussian dimple -dimple * exp(-(x^2+y^2+z^2)/2) as the 3-D array v_static (None when
+    dimple = 0), contact interaction g, the seeded noisy Gaussian as the initial state.  With separable=False the
+    whole potential goes into v_static."""
+    ny = nx if ny is None else ny
+    nz = nx if nz is None else nz
+    x, y, z = axis(nx, L), axis(ny, L), axis(nz, L)
+    vx, vy, vz = 0.5 * w2[0] * x * x, 0.5 * w2[1] * y * y, 0.5 * w2[2] * z * z
+    p = dict(nx=nx, ny=ny, nz=nz, Lx=L, Ly=L, Lz=L, g=float(g), dtype=dtype, vx=vx, vy=vy, vz=vz, v_static=None)
+    if dimple != 0.0:
+        r2 = x[None, :, None] ** 2 + y[None, None, :] ** 2 + z[:, None, None] ** 2
+        p["v_static"] = np.ascontiguousarray(-dimple * np.exp(-0.5 * r2))
+    if not separable:
+        full = vz[:, None, None] + vx[None, :, None] + vy[None, None, :]
+        p["v_static"] = np.ascontiguousarray(full + (p["v_static"] if p["v_static"] is not None else 0.0))
+        p["vx"] = p["vy"] = p["vz"] = None
+    p["psi0"] = noisy_gaussian3(nx, ny, nz, L, L, L, (1.5, 1.3, 1.7), seed)
+    p["phases"] = [dict(mode=mode, dt=dt, n_steps=n_steps, record_every=0)]
+    return p
