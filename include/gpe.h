@@ -68,7 +68,7 @@ typedef enum {
 
 /* Bumped whenever a struct layout or a signature below changes; the Python binding refuses to run
  * against a library whose gpe_abi_version() or gpe_sizeof_potential_desc() differ from its own. */
-#define GPE_ABI_VERSION 3
+#define GPE_ABI_VERSION 4
 
 /*
  * gpe_plan_create -- the discretised problem of Eq. 1: an nx x ny periodic grid
@@ -266,6 +266,64 @@ GPE_API const char *gpe_last_error(const gpe_plan *p);
 GPE_API gpe_status gpe_norm_theta_noalloc(const void *psi_dev, int nx, int ny, double Lx, double Ly, gpe_dtype dtype,
                                           int batch, double cavity_k, double *out_dev, void *cuda_stream);
 GPE_API const char *gpe_noalloc_last_error(void);
+
+/*
+ * ---- Three dimensions (second half; the first item of the paper's outlook) ----
+ * The same split-step (Eqs. 2-4; imaginary time PAPER.md:112-116) for ONE wavefunction on an
+ * nx x ny x nz periodic grid over [-Lx/2, Lx/2) x [-Ly/2, Ly/2) x [-Lz/2, Lz/2):
+ *   psi <- exp(-s (V + g|psi|^2) dt/2)  IFFT3[ exp(-s |k|^2 dt/2) FFT3[ exp(-s (V + g|psi|^2) dt/2) psi ] ],
+ * s = i (real time) or 1 (imaginary time, followed by psi <- psi / sqrt(sum |psi|^2 dx dy dz)); the second
+ * potential factor takes |psi|^2 of the psi that enters it.  V = v_static + vx[i] + vy[j] + vz[l].
+ * Layout: psi and v_static are [nz][nx][ny], y fastest, z slowest.  No cavity terms, schedule or batch here.
+ * A step is three passes over the array, one per axis (csrc/gpe3_kernels.cuh); nothing is transposed.
+ *
+ * gpe3_plan_create: nx, ny, nz each one of 64, 128, 256, 512 (else GPE_EUNSUPPORTED); Lx, Ly, Lz > 0 and finite,
+ * dtype as above (else GPE_EINVAL).  Allocates tables and a few KB of reduction scratch on the current device; the
+ * caller owns psi.  *out is set only on GPE_OK; release with gpe3_plan_destroy (NULL is accepted).
+ */
+typedef struct gpe3_plan gpe3_plan;
+GPE_API gpe_status gpe3_plan_create(gpe3_plan **out, int nx, int ny, int nz, double Lx, double Ly, double Lz,
+                                    gpe_dtype dtype);
+GPE_API gpe_status gpe3_plan_set_stream(gpe3_plan *p, void *cuda_stream);   /* all later work of the plan goes there */
+GPE_API gpe_status gpe3_plan_destroy(gpe3_plan *p);
+
+/*
+ * gpe3_set_potential -- v_static_dev: DEVICE real array [nz][nx][ny] of the plan's real type (float for GPE_C64,
+ * double for GPE_C128), or NULL; vx, vy, vz: HOST doubles [nx], [ny], [nz], each may be NULL (= 0); g: contact
+ * coupling in the norm-1 convention.  Everything is copied (v_static device-to-device on the plan's stream); the
+ * call synchronises the stream.  GPE_EINVAL on a non-finite g / vx / vy / vz or a misaligned v_static_dev.
+ */
+GPE_API gpe_status gpe3_set_potential(gpe3_plan *p, const void *v_static_dev, const double *vx, const double *vy,
+                                      const double *vz, double g);
+
+#define GPE3_NREC 3 /* doubles per record: {step, norm, norm_pre} */
+/*
+ * gpe3_evolve -- n_steps steps in place on psi_dev: DEVICE [nz][nx][ny] complex of the plan's dtype, 16-byte
+ * aligned, caller-owned.  dt finite and non-zero, > 0 in imaginary time.  The plan keeps a step counter
+ * (gpe3_get_step / gpe3_set_step) that only numbers the records.  records_dev: DEVICE doubles, NULL or
+ * [n_rec][GPE3_NREC] with n_rec = floor((step + n_steps) / record_every) - floor(step / record_every): after every
+ * step whose index is a multiple of record_every, {index, sum |psi|^2 dV, the same sum before that step's
+ * renormalisation} (the two are equal in real time; in imaginary time the second gives the chemical potential
+ * estimate -log(norm_pre) / (2 dt)).  The call only ENQUEUES work on the plan's stream and returns; errors of the
+ * device side (a non-finite or zero norm) are reported by the next gpe3_synchronize.
+ * GPE_ESTATE before gpe3_set_potential or on another device than the plan's; GPE_EINVAL on bad arguments.
+ */
+GPE_API gpe_status gpe3_evolve(gpe3_plan *p, void *psi_dev, double dt, long long n_steps, gpe_mode mode,
+                               long long record_every, double *records_dev);
+
+/*
+ * gpe3_observables -- out_host[8] = {norm, e_kin, e_pot, e_int, <x^2>, <y^2>, <z^2>, 0} of psi_dev (not modified):
+ * norm = sum |psi|^2 dV, e_kin = (1/2) sum |k|^2 |psi^|^2 / sum |psi^|^2 * norm, e_pot = sum V |psi|^2 dV,
+ * e_int = (g/2) sum |psi|^4 dV, <x^2> = sum x_i^2 |psi|^2 dV (not divided by the norm).  Synchronises the stream.
+ */
+GPE_API gpe_status gpe3_observables(gpe3_plan *p, const void *psi_dev, double *out_host);
+
+/* Waits for the plan's stream; GPE_ENONFINITE (once) if an earlier gpe3_evolve saw a non-finite or zero norm. */
+GPE_API gpe_status gpe3_synchronize(gpe3_plan *p);
+GPE_API gpe_status gpe3_get_step(const gpe3_plan *p, long long *step);
+GPE_API gpe_status gpe3_set_step(gpe3_plan *p, long long step);   /* GPE_EINVAL for step < 0 */
+/* Text of the last error of the plan, or of the last failed gpe3_plan_create of this thread when p is NULL. */
+GPE_API const char *gpe3_last_error(const gpe3_plan *p);
 
 /* Library build information: "libgpe <version> sm_100a". */
 GPE_API const char *gpe_version(void);

@@ -12,4 +12,6 @@ from .binding import (  # noqa: F401
     gpe_observables, gpe_populations, gpe_profile_passes, gpe_measure_roofs, gpe_norm_theta_noalloc, gpe_fft2_forward, gpe_get_step, gpe_set_step,
     gpe_last_error, gpe_version,
     gpe_potential_desc, gpe_obs, library_path, load_library,
+    GPE3_NREC, OBS3_NAMES, Plan3, gpe3_plan_create, gpe3_plan_set_stream, gpe3_plan_destroy, gpe3_set_potential,
+    gpe3_evolve, gpe3_observables, gpe3_synchronize, gpe3_get_step, gpe3_set_step,
 )

@@ -12,7 +12,8 @@ _LIB = None
 GPE_C64, GPE_C128 = 0, 1
 GPE_REAL_TIME, GPE_IMAG_TIME = 0, 1
 GPE_NREC = 6
-GPE_ABI_VERSION = 3   # include/gpe.h
+GPE_ABI_VERSION = 4   # include/gpe.h
+GPE3_NREC = 3
 _STATUS = {0: "GPE_OK", 1: "GPE_EINVAL", 2: "GPE_EUNSUPPORTED", 3: "GPE_ENOMEM", 4: "GPE_ECUDA",
            5: "GPE_ESTATE", 6: "GPE_ENONFINITE"}
 
@@ -92,6 +93,27 @@ def load_library() -> C.CDLL:
     lib.gpe_norm_theta_noalloc.argtypes = [vp, i, i, d, d, i, i, d, vp, vp]
     lib.gpe_noalloc_last_error.restype = C.c_char_p
     lib.gpe_noalloc_last_error.argtypes = []
+    ll = C.c_longlong
+    lib.gpe3_plan_create.restype = i
+    lib.gpe3_plan_create.argtypes = [C.POINTER(vp), i, i, i, d, d, d, i]
+    lib.gpe3_plan_set_stream.restype = i
+    lib.gpe3_plan_set_stream.argtypes = [vp, vp]
+    lib.gpe3_plan_destroy.restype = i
+    lib.gpe3_plan_destroy.argtypes = [vp]
+    lib.gpe3_set_potential.restype = i
+    lib.gpe3_set_potential.argtypes = [vp, vp, vp, vp, vp, d]
+    lib.gpe3_evolve.restype = i
+    lib.gpe3_evolve.argtypes = [vp, vp, d, ll, i, ll, vp]
+    lib.gpe3_observables.restype = i
+    lib.gpe3_observables.argtypes = [vp, vp, C.POINTER(C.c_double)]
+    lib.gpe3_synchronize.restype = i
+    lib.gpe3_synchronize.argtypes = [vp]
+    lib.gpe3_get_step.restype = i
+    lib.gpe3_get_step.argtypes = [vp, C.POINTER(ll)]
+    lib.gpe3_set_step.restype = i
+    lib.gpe3_set_step.argtypes = [vp, ll]
+    lib.gpe3_last_error.restype = C.c_char_p
+    lib.gpe3_last_error.argtypes = [vp]
     lib.gpe_get_step.restype = i
     lib.gpe_get_step.argtypes = [vp, C.POINTER(l)]
     lib.gpe_set_step.restype = i
@@ -328,3 +350,124 @@ class Plan:
     @step.setter
     def step(self, v):
         gpe_set_step(self.plan, v)
+
+
+# ---- three dimensions (include/gpe.h, gpe3_*) -----------------------------------------------
+OBS3_NAMES = ("norm", "e_kin", "e_pot", "e_int", "x2", "y2", "z2", "reserved")
+
+
+def _check3(status: int, plan) -> None:
+    if status != 0:
+        raise GpeError(status, load_library().gpe3_last_error(plan).decode())
+
+
+def gpe3_plan_create(nx: int, ny: int, nz: int, Lx: float, Ly: float, Lz: float, dtype: int):
+    out = C.c_void_p()
+    _check3(load_library().gpe3_plan_create(C.byref(out), int(nx), int(ny), int(nz), float(Lx), float(Ly), float(Lz),
+                                            int(dtype)), None)
+    return out
+
+
+def gpe3_plan_set_stream(plan, cuda_stream: int) -> None:
+    _check3(load_library().gpe3_plan_set_stream(plan, C.c_void_p(cuda_stream)), plan)
+
+
+def gpe3_plan_destroy(plan) -> None:
+    _check3(load_library().gpe3_plan_destroy(plan), None)
+
+
+def gpe3_set_potential(plan, v_static_ptr, vx, vy, vz, g: float) -> None:
+    """v_static_ptr: device pointer or None; vx, vy, vz: host float64 arrays or None."""
+    keep = [None if a is None else np.ascontiguousarray(np.asarray(a, dtype=np.float64)) for a in (vx, vy, vz)]
+    ptrs = [None if a is None else a.ctypes.data for a in keep]
+    _check3(load_library().gpe3_set_potential(plan, v_static_ptr, ptrs[0], ptrs[1], ptrs[2], float(g)), plan)
+
+
+def gpe3_evolve(plan, psi_ptr: int, dt: float, n_steps: int, mode: int, record_every: int = 0,
+                records_ptr: int | None = None) -> None:
+    _check3(load_library().gpe3_evolve(plan, psi_ptr, float(dt), int(n_steps), int(mode), int(record_every), records_ptr), plan)
+
+
+def gpe3_observables(plan, psi_ptr: int) -> dict:
+    out = (C.c_double * 8)()
+    _check3(load_library().gpe3_observables(plan, psi_ptr, out), plan)
+    return dict(zip(OBS3_NAMES, [float(v) for v in out]))
+
+
+def gpe3_synchronize(plan) -> None:
+    _check3(load_library().gpe3_synchronize(plan), plan)
+
+
+def gpe3_get_step(plan) -> int:
+    v = C.c_longlong()
+    _check3(load_library().gpe3_get_step(plan, C.byref(v)), plan)
+    return int(v.value)
+
+
+def gpe3_set_step(plan, step: int) -> None:
+    _check3(load_library().gpe3_set_step(plan, int(step)), plan)
+
+
+class Plan3:
+    """gpe3_plan with torch tensors for device memory.  `p` is a workload dict of workloads.config3d()."""
+
+    def __init__(self, nx, ny, nz, Lx, Ly, Lz, dtype="c64", stream=None):
+        import torch
+        self.torch = torch
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.dtype = dtype
+        self.cdtype = torch.complex64 if dtype == "c64" else torch.complex128
+        self.rdtype = torch.float32 if dtype == "c64" else torch.float64
+        self.plan = gpe3_plan_create(nx, ny, nz, Lx, Ly, Lz, GPE_C64 if dtype == "c64" else GPE_C128)
+        if stream is not None:
+            gpe3_plan_set_stream(self.plan, stream)
+
+    def close(self):
+        if self.plan is not None:
+            gpe3_plan_destroy(self.plan)
+            self.plan = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_potential(self, p: dict) -> None:
+        vs = p.get("v_static")
+        t = None
+        if vs is not None:
+            t = self.torch.as_tensor(np.asarray(vs), dtype=self.rdtype).contiguous().cuda()
+            assert t.numel() == self.nx * self.ny * self.nz
+        gpe3_set_potential(self.plan, None if t is None else t.data_ptr(), p.get("vx"), p.get("vy"), p.get("vz"),
+                           float(p.get("g", 0.0)))
+
+    def evolve(self, psi, dt, n_steps, mode, record_every=0):
+        """psi: CUDA tensor [nz, nx, ny] of the plan's complex dtype, evolved in place.
+        Returns the records tensor [n_rec, 3] (device, float64) or None."""
+        torch = self.torch
+        assert psi.is_cuda and psi.dtype == self.cdtype and psi.is_contiguous()
+        assert psi.numel() == self.nx * self.ny * self.nz
+        m = GPE_IMAG_TIME if mode in ("imag", GPE_IMAG_TIME) else GPE_REAL_TIME
+        rec = None
+        if record_every > 0:
+            s0 = gpe3_get_step(self.plan)
+            nrec = (s0 + n_steps) // record_every - s0 // record_every
+            rec = torch.zeros((max(nrec, 1), GPE3_NREC), dtype=torch.float64, device=psi.device)
+        gpe3_evolve(self.plan, psi.data_ptr(), dt, n_steps, m, record_every, rec.data_ptr() if rec is not None else None)
+        return rec
+
+    def observables(self, psi) -> dict:
+        assert psi.is_cuda and psi.dtype == self.cdtype and psi.is_contiguous()
+        return gpe3_observables(self.plan, psi.data_ptr())
+
+    def synchronize(self) -> None:
+        gpe3_synchronize(self.plan)
+
+    @property
+    def step(self):
+        return gpe3_get_step(self.plan)
+
+    @step.setter
+    def step(self, v):
+        gpe3_set_step(self.plan, v)

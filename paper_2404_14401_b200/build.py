@@ -15,6 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgpe.so")
 SIZES = (64, 128, 256, 512, 1024, 2048)
+SIZES3 = (64, 128, 256, 512)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
@@ -56,6 +57,15 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
             objs.append(o)
             jobs.append([nvcc, *NVCC_FLAGS, *extra, f"-DGPE_T={typ}", f"-DGPE_N={n}", f"-DGPE_TAG={tag}",
                          "-c", os.path.join(CSRC, "gpe_inst.cu"), "-o", o])
+    for tag, typ in (("f", "float"), ("d", "double")):   # the 3-D passes (gpe3_kernels.cuh)
+        for n in SIZES3:
+            o = os.path.join(OBJ, f"inst3_{tag}_{n}.o")
+            objs.append(o)
+            jobs.append([nvcc, *NVCC_FLAGS, *extra, f"-DGPE_T={typ}", f"-DGPE_N={n}", f"-DGPE_TAG={tag}",
+                         "-c", os.path.join(CSRC, "gpe3_inst.cu"), "-o", o])
+    o = os.path.join(OBJ, "api3.o")
+    objs.append(o)
+    jobs.append([nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, "gpe3_api.cu"), "-o", o])
     o = os.path.join(OBJ, "api.o")
     objs.append(o)
     jobs.append([nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, "gpe_api.cu"), "-o", o])
