@@ -228,6 +228,43 @@ def other_workloads(G, torch, peak, hbm_peak, roofs):
     return out
 
 
+def three_d(G, torch, hbm_peak, l2_peak):
+    """The 3-D path (csrc/gpe3_kernels.cuh) on the seeded 3-D workload
+    (workloads.config3d: anisotropic trap as separable arrays + a Gaussian dimple as a 3-D array, g = 50).
+    Three in-place passes per step: 6 P s bytes of psi plus the potential array (P s/2 bytes, read once per step in
+    real time and twice in imaginary time).  Roof: HBM where the wavefunction does not fit L2 (256^3: 128 MiB), the
+    L2 figure of this run below."""
+    import numpy as np
+    import workloads as W
+    rows = []
+    for n, dtype, mode, steps in ((128, "c64", "real", 200), (128, "c64", "imag", 200), (256, "c64", "real", 40),
+                                  (256, "c64", "imag", 40), (256, "c128", "real", 20), (256, "c128", "imag", 20)):
+        p = W.config3d(n, dtype=dtype)
+        cd = np.complex64 if dtype == "c64" else np.complex128
+        plan = G.Plan3(n, n, n, p["Lx"], p["Ly"], p["Lz"], dtype)
+        plan.set_potential(p)
+        psi = torch.from_numpy(np.ascontiguousarray(p["psi0"].astype(cd))).cuda()
+        plan.evolve(psi, 1e-3, 5, mode)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        plan.evolve(psi, 1e-3, steps, mode)
+        e1.record()
+        torch.cuda.synchronize()
+        plan.synchronize()
+        plan.close()
+        us = e0.elapsed_time(e1) / steps * 1e3
+        pts, s = n ** 3, (8 if dtype == "c64" else 16)
+        bpp = 6.0 * s + (s / 2) * (2 if mode == "imag" else 1)
+        in_l2 = pts * s <= 96e6
+        roof = l2_peak if in_l2 else hbm_peak
+        rows.append({"grid": f"{n}^3", "dtype": dtype, "mode": mode, "us_per_split_step": us,
+                     "updates_per_s": pts / (us * 1e-6), "algorithmic_bytes_per_point": bpp,
+                     "bound": "l2" if in_l2 else "hbm", "byte_roof_gbs": roof,
+                     "byte_roofline_frac": pts * bpp / (us * 1e-6) / 1e9 / roof, "gpu_launches_per_step": 3})
+    return rows
+
+
 def sweep_s(G, torch):
     """The paper's own benchmark (Sec. 4.1): non-interacting gas in a fixed harmonic trap,
     imaginary time, 10^3 steps, N_x = N_y = 2^n, single and double precision, mean of 5 runs (the paper's
@@ -477,6 +514,7 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         extra["other_workloads"] = other_workloads(G, torch, peak, hbm_peak, roofs)
         extra["sweep_s"] = sweep_s(G, torch)
+        extra["three_d"] = three_d(G, torch, hbm_peak, peak)
         extra["comparison"] = torch_fft_comparison(torch, nx)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

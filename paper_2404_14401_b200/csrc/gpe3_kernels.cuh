@@ -19,6 +19,15 @@
 #pragma once
 #include "gpe_kernels.cuh"
 
+// resident CTAs per SM asked of the compiler for complex64 (measured on B200, 256^3 real time: column passes 1 -> 2
+// CTAs and row pass 2 -> 3: 304 -> 249 us per step; 3 CTAs of the column pass spill and lose: 263 us)
+#ifndef GPE3_COL_MINB
+#define GPE3_COL_MINB 2
+#endif
+#ifndef GPE3_ROW_MINB
+#define GPE3_ROW_MINB 3
+#endif
+
 namespace gpe {
 
 struct State3 {
@@ -156,7 +165,7 @@ __device__ __forceinline__ void finalize3(State3 *st, double total, double dV, l
 // ---------------------------------------------------------------- pass Y: rows
 // MODE 0: the step.  MODE 1: measure: sum kin[q] |psi^_y|^2 over the grid (kin = k_y^2) -> *measure_out.
 template <typename T, int NY, bool IMAG, int MODE>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? 2 : 1)) k3_row(const Args3<T> a) {
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE3_ROW_MINB : 1)) k3_row(const Args3<T> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
@@ -212,7 +221,7 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? 2 : 1)
 // ---------------------------------------------------------------- passes X and Z: lines of stride line_stride
 // grid = (columns of a slab / W, slabs).  FINAL: the last pass of the step (lines along z).
 template <typename T, int N, bool IMAG, int MODE>
-__global__ void __launch_bounds__(ColGeom<T, N>::THREADS, 1) k3_col(const Args3<T> a) {
+__global__ void __launch_bounds__(ColGeom<T, N>::THREADS, (sizeof(T) == 4 ? GPE3_COL_MINB : 1)) k3_col(const Args3<T> a) {
     using C = cx<T>;
     using G = ColGeom<T, N>;
     using F = Fft1D<N, G::W, cx<T>>;
