@@ -228,7 +228,7 @@ def other_workloads(G, torch, peak, hbm_peak, roofs):
     return out
 
 
-def three_d(G, torch, hbm_peak, l2_peak):
+def three_d(G, torch, hbm_peak, l2_peak, only=None):
     """The 3-D path (csrc/gpe3_kernels.cuh) on the seeded 3-D workload
     (workloads.config3d: anisotropic trap as separable arrays + a Gaussian dimple as a 3-D array, g = 50).
     Three in-place passes per step: 6 P s bytes of psi plus the potential array (P s/2 bytes, read once per step in
@@ -237,8 +237,9 @@ def three_d(G, torch, hbm_peak, l2_peak):
     import numpy as np
     import workloads as W
     rows = []
-    for n, dtype, mode, steps in ((128, "c64", "real", 200), (128, "c64", "imag", 200), (256, "c64", "real", 40),
-                                  (256, "c64", "imag", 40), (256, "c128", "real", 20), (256, "c128", "imag", 20)):
+    cases = ((128, "c64", "real", 200), (128, "c64", "imag", 200), (256, "c64", "real", 40),
+             (256, "c64", "imag", 40), (256, "c128", "real", 20), (256, "c128", "imag", 20)) if only is None else (only,)
+    for n, dtype, mode, steps in cases:
         p = W.config3d(n, dtype=dtype)
         cd = np.complex64 if dtype == "c64" else np.complex128
         plan = G.Plan3(n, n, n, p["Lx"], p["Ly"], p["Lz"], dtype)
@@ -545,9 +546,18 @@ def main():
     ap.add_argument("--inner", type=int, default=200, help="split-step steps per bench step")
     ap.add_argument("--n", type=int, default=2048, help="grid side (the metric is quoted at 2048)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--three-d", default=None, metavar="N,DTYPE,MODE,STEPS",
+                    help="time only the 3-D path on an N^3 grid, e.g. 256,c64,real,20 (profiling aid)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = max(args.warmup, 3) if os.environ.get("GPE_BENCH_STRICT", "1") == "1" else args.warmup
+    if args.three_d:   # one 3-D workload alone (the command the ncu captures of profiles/r02_3d.md run)
+        import torch
+        import paper_2404_14401_b200 as G
+        n, dtype, mode, steps = args.three_d.split(",")
+        hbm = _measured_peaks()[0]
+        print(json.dumps({"three_d": three_d(G, torch, hbm, hbm, (int(n), dtype, mode, int(steps)))}))
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

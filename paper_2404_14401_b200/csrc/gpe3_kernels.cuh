@@ -59,8 +59,12 @@ template <typename T> struct Args3 {
     long long step_index;            // index of the step being taken
     double *record;                  // {step, norm, norm_pre} of this step, or nullptr
     double *measure_out;             // measure mode: where the last CTA writes the total
+    int rev;                         // 1: CTAs take their tiles in descending order (see evolve3 in gpe3_api.cu)
 };
 
+// tile index of this CTA: blocks are dispatched in ascending order, rev walks the array the other way
+__device__ __forceinline__ unsigned tile_x(int rev) { return rev ? gridDim.x - 1u - blockIdx.x : blockIdx.x; }
+__device__ __forceinline__ unsigned tile_y(int rev) { return rev ? gridDim.y - 1u - blockIdx.y : blockIdx.y; }
 __device__ __forceinline__ void sincosm1_any(float w, float *s, float *cm1) { sincosm1_general(w, s, cm1); }
 __device__ __forceinline__ void sincosm1_any(double w, double *s, double *cm1) { sincosm1_t(w, s, cm1); }
 
@@ -173,7 +177,7 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE3_R
     C *smem = reinterpret_cast<C *>(smem_raw);
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
     C *sm = smem + r * F::SLOTS;
-    const long row = (long)blockIdx.x * G::RPC + r;
+    const long row = (long)tile_x(a.rev) * G::RPC + r;
     const int l = (int)(row / a.nx), i = (int)(row % a.nx);
     C *p = a.psi + row * NY;
     C v[16];
@@ -228,8 +232,8 @@ __global__ void __launch_bounds__(ColGeom<T, N>::THREADS, (sizeof(T) == 4 ? GPE3
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
     const int c = threadIdx.x % G::W, j = threadIdx.x / G::W;
-    const long col = (long)blockIdx.x * G::W + c;
-    C *p = a.psi + (long)blockIdx.y * a.slab_stride + col;
+    const long col = (long)tile_x(a.rev) * G::W + c;
+    C *p = a.psi + (long)tile_y(a.rev) * a.slab_stride + col;
     C *sm = smem + c;
     const long ls = a.line_stride;
     C v[16];
