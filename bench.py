@@ -262,7 +262,8 @@ def three_d(G, torch, hbm_peak, l2_peak, only=None):
         rows.append({"grid": f"{n}^3", "dtype": dtype, "mode": mode, "us_per_split_step": us,
                      "updates_per_s": pts / (us * 1e-6), "algorithmic_bytes_per_point": bpp,
                      "bound": "l2" if in_l2 else "hbm", "byte_roof_gbs": roof,
-                     "byte_roofline_frac": pts * bpp / (us * 1e-6) / 1e9 / roof, "gpu_launches_per_step": 3})
+                     "byte_roofline_frac": pts * bpp / (us * 1e-6) / 1e9 / roof,
+                     "gpu_launches_per_step": 4 if mode == "imag" else 3})
     return rows
 
 

@@ -174,6 +174,12 @@ gpe_status evolve3(gpe3_plan *p, void *psi, double dt, long long n_steps, int mo
         a.sums = (imag || rec || q == n_steps - 1) ? 1 : 0;
         a.record = rec ? records + 3 * (nrec++) : nullptr;
         GPE3_CUDA(p, run_axis<T>(p, a, 2, imag, 0));
+        if (a.sums) {
+            const unsigned int nparts = (unsigned int)((long)p->nx * p->ny / get_ops3<T>(p->nz)->cols_per_cta);
+            if (imag) k3_finalize<true><<<1, 256, 0, p->stream>>>(p->st, p->partials, nparts, a.dV, n, a.record, p->nonfinite);
+            else k3_finalize<false><<<1, 256, 0, p->stream>>>(p->st, p->partials, nparts, a.dV, n, a.record, p->nonfinite);
+            GPE3_CUDA(p, cudaGetLastError());
+        }
     }
     if (n_steps > 0) {
         if (imag) {

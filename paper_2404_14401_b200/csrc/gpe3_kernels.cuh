@@ -9,9 +9,9 @@
 //                                   FFT_y -> K_y -> IFFT_y -> store
 //   pass X (lines of stride ny):    tiles of W neighbouring y per CTA: FFT_x -> K_x -> IFFT_x
 //   pass Z (lines of stride nx ny): tiles of W neighbouring (x, y) per CTA: FFT_z -> K_z -> IFFT_z
-//                                   [imaginary time: -> second potential half-step -> partial sums of |psi|^2; the
-//                                   last CTA adds them in a fixed order, sets the lazy scale 1/sqrt(norm) and writes the
-//                                   record: no host round trip]
+//                                   [imaginary time: -> second potential half-step -> one partial sum of |psi|^2 per
+//                                   CTA; the one-CTA kernel k3_finalize adds them in a fixed order, sets the lazy scale
+//                                   1/sqrt(norm) and writes the record: no host round trip]
 // Real time: the second half-step of step n and the first of step n+1 see the same |psi|^2 and are applied as ONE
 // factor by pass Y of step n+1 (fac = 2); the first step of a call takes fac = 1 and a point-wise kernel closes the
 // call (k3_point).  Three passes are the floor for three axes held one at a time in registers / shared memory:
@@ -272,13 +272,41 @@ __global__ void __launch_bounds__(ColGeom<T, N>::THREADS, (sizeof(T) == 4 ? GPE3
 #pragma unroll
         for (int k = 0; k < 16; ++k) p[(long)(j + F::M1 * k) * ls] = v[k];
         if (a.final_axis && a.sums) {
-            double acc = 0.0;
+            // One partial per CTA, added up by k3_finalize after the pass.  A fence + counter + broadcast at the end of
+            // every CTA (the last-CTA pattern of reduce_ctas) held each CTA slot ~3 us longer: 124 instead of 82 us for
+            // this pass at 256^3 complex64; publishing the partial before the stores, as pass C of the 2-D path does,
+            // recovered only part of it (step 261 against 247 us).
+            // The 16 terms of a thread in T (one conversion per thread), the rest in double.
+            __shared__ double red[32];
+            T part = T(0);
 #pragma unroll
-            for (int k = 0; k < 16; ++k) acc += (double)v[k].x * (double)v[k].x + (double)v[k].y * (double)v[k].y;
-            double total;
-            if (reduce_ctas(acc, a.partials, a.counter, blockIdx.y * gridDim.x + blockIdx.x, gridDim.x * gridDim.y, total))
-                finalize3<IMAG>(a.st, total, a.dV, a.step_index, a.record, a.nonfinite);
+            for (int k = 0; k < 16; ++k) part = fma(v[k].x, v[k].x, fma(v[k].y, v[k].y, part));
+            const double acc = warp_sum((double)part);
+            if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                double t = 0.0;
+                for (int q = 0; q < G::THREADS / 32; ++q) t += red[q];
+                a.partials[blockIdx.y * gridDim.x + blockIdx.x] = t;
+            }
         }
+    }
+}
+
+// one CTA: the partial sums of the last pass in a fixed order, then the end of the step (finalize3)
+template <bool IMAG>
+__global__ void __launch_bounds__(256) k3_finalize(State3 *st, const double *partials, unsigned int n, double dV,
+                                                   long long step_index, double *record, int *nonfinite) {
+    __shared__ double red[8];
+    double t = 0.0;
+    for (unsigned int q = threadIdx.x; q < n; q += 256) t += partials[q];
+    t = warp_sum(t);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double total = 0.0;
+        for (int q = 0; q < 8; ++q) total += red[q];
+        finalize3<IMAG>(st, total, dV, step_index, record, nonfinite);
     }
 }
 
