@@ -178,3 +178,40 @@ def test_full_size_256_cubed(dtype):
     _check_obs(og, oo, dtype)
     out, ref, _, _, _, _ = _run_both(p, dtype, "real", 1e-3, 3)
     assert _rel(out, ref) <= _tol(dtype, 3)
+
+
+def test_largest_grid_properties():
+    """512^3 complex64 (1 GiB of wavefunction, the largest grid the boundary takes): what holds at any size --
+    norm conservation in real time, time reversal (the symmetric splitting is its own inverse under dt -> -dt), and
+    sampled lines of the kinetic factor against the closed form for a plane wave"""
+    import torch
+    import paper_2404_14401_b200 as G
+    n, L = 512, 20.0
+    plan = G.Plan3(n, n, n, L, L, L, "c64")
+    x = torch.linspace(-L / 2, L / 2 - L / n, n, device="cuda", dtype=torch.float32)
+    g = torch.Generator(device="cuda").manual_seed(3)
+    psi = torch.exp(-(x[None, :, None] ** 2 / 8 + x[None, None, :] ** 2 / 6 + x[:, None, None] ** 2 / 10)).to(torch.complex64)
+    psi = psi * (1 + 0.05 * torch.randn((n, n, n), device="cuda", generator=g))
+    dV = (L / n) ** 3
+    psi /= torch.sqrt((psi.real ** 2 + psi.imag ** 2).sum(dtype=torch.float64) * dV).to(torch.float32)
+    start = psi.clone()
+    xs = np.asarray(W.axis(n, L))
+    G.gpe3_set_potential(plan.plan, None, 0.5 * xs ** 2, 0.7 * xs ** 2, 0.4 * xs ** 2, 80.0)
+    rec = plan.evolve(psi, 1e-3, 4, "real", record_every=2).cpu().numpy()
+    assert np.abs(rec[:, 1] - 1.0).max() <= 2e-6
+    assert float((psi - start).abs().max()) > 1e-4          # it moved
+    plan.evolve(psi, -1e-3, 4, "real")
+    plan.synchronize()
+    err = torch.sqrt(((psi - start).abs() ** 2).sum(dtype=torch.float64) / (start.abs() ** 2).sum(dtype=torch.float64))
+    assert float(err) <= 1e-5
+    # a plane wave with mode numbers (3, -7, 5) on (x, y, z), V = 0, g = 0: one step multiplies it by e^{-i |k|^2 dt/2}
+    G.gpe3_set_potential(plan.plan, None, None, None, None, 0.0)
+    k = 2 * np.pi / L * np.array([3.0, -7.0, 5.0])
+    ph = (k[0] * x.double()[None, :, None] + k[1] * x.double()[None, None, :] + k[2] * x.double()[:, None, None])
+    wave = torch.complex(torch.cos(ph), torch.sin(ph)).to(torch.complex64)
+    del ph, start
+    ref_line = wave[17, 33, :].cpu().numpy().astype(np.complex128) * np.exp(-0.5j * float(k @ k) * 1e-2)
+    plan.evolve(wave, 1e-2, 1, "real")
+    got = wave[17, 33, :].cpu().numpy().astype(np.complex128)
+    assert np.abs(got - ref_line).max() <= 5e-6
+    plan.close()
