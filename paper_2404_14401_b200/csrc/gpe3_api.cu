@@ -38,6 +38,12 @@ struct gpe3_plan {
     unsigned int *counter = nullptr;
     int *nonfinite = nullptr;
     long long step = 0;
+    // CUDA graph of kGraphSteps plain steps (small grids) and what its kernel arguments were captured for
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t g_exec = nullptr;
+    void *g_psi = nullptr;
+    double g_dt = 0.0;
+    int g_imag = -1;
 };
 
 namespace {
@@ -138,11 +144,64 @@ template <typename T> void set_axis(gpe3_plan *p, Args3<T> &a, int ax, bool meas
     if (ax == 2) { a.line_stride = (long)p->nx * p->ny; a.slab_stride = 0; }
 }
 // the pass along axis ax (1: rows; 0, 2: columns)
-template <typename T> cudaError_t run_axis(gpe3_plan *p, const Args3<T> &a, int ax, bool imag, int mode) {
+template <typename T> cudaError_t run_axis(gpe3_plan *p, const Args3<T> &a, int ax, bool imag, int mode, cudaStream_t st, unsigned *nctas = nullptr) {
     const Ops3<T> *o = get_ops3<T>(axis_len(p, ax));
-    if (ax == 1) return o->row(a, imag, mode, p->stream);
-    if (ax == 0) return o->col(a, imag, mode, (unsigned)(p->ny / o->cols_per_cta), (unsigned)p->nz, p->stream);
-    return o->col(a, imag, mode, (unsigned)((long)p->nx * p->ny / o->cols_per_cta), 1u, p->stream);
+    if (ax == 1) return o->row(a, imag, mode, st);
+    if (ax == 0) return o->col(a, imag, mode, p->ny, (unsigned)p->nz, nctas, st);
+    return o->col(a, imag, mode, (long)p->nx * p->ny, 1u, nctas, st);
+}
+
+// one step on stream st.  fac: 1 or 2 (merged real-time halves); sums: reduce the norm at the end; step_index < 0:
+// a step replayed from the graph (no record, the device step counter just advances)
+template <typename T>
+gpe_status step3(gpe3_plan *p, const Args3<T> &base, bool imag, T fac, int sums, long long step_index, double *record, cudaStream_t st) {
+    Args3<T> a = base;
+    a.step_index = step_index;
+    a.pot = 1;
+    a.fac = fac;
+    set_axis<T>(p, a, 1, false);
+    GPE3_CUDA(p, run_axis<T>(p, a, 1, imag, 0, st));
+    a.pot = 0;
+    // the x pass walks the array backwards: it starts on the slabs the row pass wrote last, which are still in L2
+    // (256^3 complex64 real time: 249 -> 246 us per step; reversing other passes, or alternate steps, measured the same)
+    a.rev = 1;
+    set_axis<T>(p, a, 0, false);
+    GPE3_CUDA(p, run_axis<T>(p, a, 0, imag, 0, st));
+    set_axis<T>(p, a, 2, false);
+    a.rev = 0;
+    a.pot = imag ? 1 : 0;
+    a.sums = sums;
+    a.record = record;
+    unsigned int nparts = 0;
+    GPE3_CUDA(p, run_axis<T>(p, a, 2, imag, 0, st, &nparts));
+    if (sums) {
+        const bool pdl = (long)p->nx * p->ny * p->nz <= GPE3_PDL_MAX;
+        GPE3_CUDA(p, imag ? launch_pdl(k3_finalize<true>, dim3(1), dim3(256), 0, st, pdl, p->st, (const double *)p->partials, nparts, a.dV, step_index, record, p->nonfinite)
+                          : launch_pdl(k3_finalize<false>, dim3(1), dim3(256), 0, st, pdl, p->st, (const double *)p->partials, nparts, a.dV, step_index, record, p->nonfinite));
+    }
+    return GPE_OK;
+}
+
+// Small grids are bound by the host's launch rate (64^3: three 3-us kernels per step against ~7 us of host time per
+// launch): kGraphSteps plain steps -- no record, not the first or last step of a real-time call -- are captured once
+// into a CUDA graph and replayed.  The graph is keyed by everything its kernel arguments hold.
+constexpr int kGraphSteps = 8;
+template <typename T> gpe_status graph3(gpe3_plan *p, const Args3<T> &base, bool imag, double dt) {
+    if (p->g_exec && p->g_psi == (void *)base.psi && p->g_dt == dt && p->g_imag == (int)imag) return GPE_OK;
+    if (p->g_exec) { cudaGraphExecDestroy(p->g_exec); p->g_exec = nullptr; }
+    if (!p->cap_stream) GPE3_CUDA(p, cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
+    GPE3_CUDA(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
+    gpe_status s = GPE_OK;
+    for (int q = 0; q < kGraphSteps && s == GPE_OK; ++q) s = step3<T>(p, base, imag, imag ? T(1) : T(2), imag ? 1 : 0, -1, nullptr, p->cap_stream);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(p->cap_stream, &g);
+    if (s != GPE_OK) { if (g) cudaGraphDestroy(g); return s; }
+    if (e != cudaSuccess) return cuda_fail3(p, e, "cudaStreamEndCapture");
+    e = cudaGraphInstantiate(&p->g_exec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { p->g_exec = nullptr; return cuda_fail3(p, e, "cudaGraphInstantiate"); }
+    p->g_psi = (void *)base.psi; p->g_dt = dt; p->g_imag = (int)imag;
+    return GPE_OK;
 }
 
 template <typename T>
@@ -152,34 +211,25 @@ gpe_status evolve3(gpe3_plan *p, void *psi, double dt, long long n_steps, int mo
     if (s != GPE_OK) return s;
     Args3<T> base = base_args<T>(p, psi);
     base.half_dt = (T)(0.5 * dt);
+    const bool use_graph = (long)p->nx * p->ny * p->nz <= GPE3_PDL_MAX && n_steps >= 2 * kGraphSteps;
+    const bool recording = records && record_every > 0;
     long long nrec = 0;
-    for (long long q = 0; q < n_steps; ++q) {
+    for (long long q = 0; q < n_steps;) {
         const long long n = p->step + q;
-        const bool rec = records && record_every > 0 && ((n + 1) % record_every) == 0;
-        Args3<T> a = base;
-        a.step_index = n;
-        a.pot = 1;
-        a.fac = (imag || q == 0) ? T(1) : T(2);
-        set_axis<T>(p, a, 1, false);
-        GPE3_CUDA(p, run_axis<T>(p, a, 1, imag, 0));
-        a.pot = 0;
-        // the x pass walks the array backwards: it starts on the slabs the row pass wrote last, which are still in L2
-        // (256^3 complex64 real time: 249 -> 246 us per step; reversing other passes, or alternate steps, measured the same)
-        a.rev = 1;
-        set_axis<T>(p, a, 0, false);
-        GPE3_CUDA(p, run_axis<T>(p, a, 0, imag, 0));
-        set_axis<T>(p, a, 2, false);
-        a.rev = 0;
-        a.pot = imag ? 1 : 0;
-        a.sums = (imag || rec || q == n_steps - 1) ? 1 : 0;
-        a.record = rec ? records + 3 * (nrec++) : nullptr;
-        GPE3_CUDA(p, run_axis<T>(p, a, 2, imag, 0));
-        if (a.sums) {
-            const unsigned int nparts = (unsigned int)((long)p->nx * p->ny / get_ops3<T>(p->nz)->cols_per_cta);
-            if (imag) k3_finalize<true><<<1, 256, 0, p->stream>>>(p->st, p->partials, nparts, a.dV, n, a.record, p->nonfinite);
-            else k3_finalize<false><<<1, 256, 0, p->stream>>>(p->st, p->partials, nparts, a.dV, n, a.record, p->nonfinite);
-            GPE3_CUDA(p, cudaGetLastError());
+        // a chunk of plain steps: no record falls on indices n+1 .. n+kGraphSteps, and in real time neither the first
+        // step of the call (fac = 1) nor the last (it reduces the norm) is inside
+        const bool no_rec = !recording || (n + kGraphSteps) / record_every == n / record_every;
+        if (use_graph && no_rec && (imag ? q + kGraphSteps <= n_steps : (q >= 1 && q + kGraphSteps <= n_steps - 1))) {
+            if ((s = graph3<T>(p, base, imag, dt)) != GPE_OK) return s;
+            GPE3_CUDA(p, cudaGraphLaunch(p->g_exec, p->stream));
+            q += kGraphSteps;
+            continue;
         }
+        const bool rec = recording && ((n + 1) % record_every) == 0;
+        s = step3<T>(p, base, imag, (imag || q == 0) ? T(1) : T(2), (imag || rec || q == n_steps - 1) ? 1 : 0, n,
+                     rec ? records + 3 * (nrec++) : nullptr, p->stream);
+        if (s != GPE_OK) return s;
+        ++q;
     }
     if (n_steps > 0) {
         if (imag) {
@@ -203,7 +253,7 @@ template <typename T> gpe_status observables3(gpe3_plan *p, const void *psi, dou
         Args3<T> m = a;
         set_axis<T>(p, m, ax, true);
         m.measure_out = p->measure + ax;
-        GPE3_CUDA(p, run_axis<T>(p, m, ax, false, 1));
+        GPE3_CUDA(p, run_axis<T>(p, m, ax, false, 1, p->stream));
     }
     std::vector<double> h6((size_t)kObsCtas * 6);
     double k2sum[3];
@@ -232,6 +282,8 @@ const char *gpe3_last_error(const gpe3_plan *p) { return p ? p->err.c_str() : g_
 gpe_status gpe3_plan_destroy(gpe3_plan *p) {
     if (!p) return GPE_OK;
     cudaStreamSynchronize(p->stream);
+    if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
+    if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     void *bufs[] = {p->tw[0], p->tw[1], p->tw[2], p->tw1[0], p->tw1[1], p->tw1[2], p->kin[0], p->kin[1], p->kin[2],
                     p->k2[0], p->k2[1], p->k2[2], p->v3d, p->vsep[0], p->vsep[1], p->vsep[2], p->st, p->partials,
                     p->part6, p->measure, p->counter, p->nonfinite};
@@ -295,6 +347,7 @@ gpe_status gpe3_set_potential(gpe3_plan *p, const void *v_static_dev, const doub
             for (int i = 0; i < axis_len(p, ax); ++i)
                 if (!std::isfinite(sep[ax][i])) return fail3(p, GPE_EINVAL, "vx / vy / vz holds a non-finite value");
     p->has_potential = false;
+    if (p->g_exec) { cudaGraphExecDestroy(p->g_exec); p->g_exec = nullptr; }   // g, v3d are kernel arguments
     for (int ax = 0; ax < 3; ++ax) {
         std::vector<double> v((size_t)axis_len(p, ax), 0.0);
         if (sep[ax]) v.assign(sep[ax], sep[ax] + axis_len(p, ax));

@@ -8,7 +8,5 @@ namespace gpe {
 extern const Ops3<GPE_T> GPE_CAT3(ops3_, GPE_TAG, GPE_N) = {
     &Launch3<GPE_T, GPE_N>::row,
     &Launch3<GPE_T, GPE_N>::col,
-    RowGeom<GPE_N>::RPC,
-    ColGeom<GPE_T, GPE_N>::W,
 };
 }  // namespace gpe

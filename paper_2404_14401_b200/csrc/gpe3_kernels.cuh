@@ -27,8 +27,37 @@
 #ifndef GPE3_ROW_MINB
 #define GPE3_ROW_MINB 3
 #endif
+#ifndef GPE3_PDL_MAX
+#define GPE3_PDL_MAX (128L * 128L * 128L)
+#endif
 
 namespace gpe {
+
+// launch geometry of the 3-D passes: 256 threads per CTA from 256 points per line up (as the 2-D passes), 128 at 128
+// and 64 at 64 points, so that a 64^3 or 128^3 grid still gives every SM several CTAs (64^3 with 256-thread CTAs: 64
+// CTAs per pass on 148 SMs)
+// Threads per CTA by line length.  Rows: 64 at 64 points, 128 above (measured on B200, 256^3 complex64 real time
+// with 256 -> 128 threads in both kinds of pass: 245 -> 208 us per step, complex128 574 -> 419: more, smaller CTAs
+// overlap their load / transform / store phases better).  Columns of 256 points come in two widths: NARROW (128
+// threads, 8 columns) and WIDE (256 threads, 16 columns); narrow wins while the plane nx ny is small (256^3: 208
+// against 236 us) and loses when the lines are 2 MB apart (512 x 512 x 256: 1060 against 1013 us), see col_wide().
+#ifndef GPE3_ROW_T
+#define GPE3_ROW_T 128
+#endif
+template <int N> struct RowTarget3 { static constexpr int THREADS = N <= 64 ? 64 : (N <= 128 ? 128 : GPE3_ROW_T); };
+template <int N, bool WIDE> struct ColTarget3 { static constexpr int THREADS = N <= 64 ? 64 : (N <= 128 ? 128 : (N <= 256 ? (WIDE ? 256 : 128) : 256)); };
+template <int N> struct RowGeom3 {
+    static constexpr int TPF = N / 16;
+    static constexpr int RPC = (RowTarget3<N>::THREADS / TPF) < 1 ? 1 : (RowTarget3<N>::THREADS / TPF);   // rows per CTA
+    static constexpr int THREADS = RPC * TPF;
+};
+template <typename T, int N, bool WIDE = false> struct ColGeom3 {
+    static constexpr int TPF = N / 16;
+    static constexpr int WMIN = sizeof(T) == 4 ? 4 : 2;            // >= 32-byte row segments
+    static constexpr int W0 = ColTarget3<N, WIDE>::THREADS / TPF;
+    static constexpr int W = W0 < WMIN ? WMIN : W0;                // columns per CTA
+    static constexpr int THREADS = W * TPF;
+};
 
 struct State3 {
     double scale;      // lazy renormalisation: the stored psi times `scale` is the wavefunction
@@ -162,17 +191,17 @@ __device__ __forceinline__ void finalize3(State3 *st, double total, double dV, l
     if (IMAG) { st->scale = 1.0 / sqrt(pre); st->norm = 1.0; }
     else st->norm = pre;
     st->norm_pre = pre;
-    st->step = step_index + 1;
+    st->step = step_index >= 0 ? step_index + 1 : st->step + 1;
     if (record) { record[0] = (double)(step_index + 1); record[1] = IMAG ? 1.0 : pre; record[2] = pre; }
 }
 
 // ---------------------------------------------------------------- pass Y: rows
 // MODE 0: the step.  MODE 1: measure: sum kin[q] |psi^_y|^2 over the grid (kin = k_y^2) -> *measure_out.
 template <typename T, int NY, bool IMAG, int MODE>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE3_ROW_MINB : 1)) k3_row(const Args3<T> a) {
+__global__ void __launch_bounds__(RowGeom3<NY>::THREADS, (sizeof(T) == 4 ? GPE3_ROW_MINB : 1) * (256 / RowGeom3<NY>::THREADS)) k3_row(const Args3<T> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
-    using G = RowGeom<NY>;
+    using G = RowGeom3<NY>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
     const int r = threadIdx.x / G::TPF, j = threadIdx.x % G::TPF;
@@ -181,6 +210,8 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE3_R
     const int l = (int)(row / a.nx), i = (int)(row % a.nx);
     C *p = a.psi + row * NY;
     C v[16];
+    pdl_launch_dependents();   // small grids are launched with programmatic stream serialisation (Launch3::go)
+    pdl_wait();
 #pragma unroll
     for (int k = 0; k < 16; ++k) v[k] = __ldcg(p + j + F::M1 * k);
     if constexpr (MODE == 0) {
@@ -224,10 +255,10 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE3_R
 
 // ---------------------------------------------------------------- passes X and Z: lines of stride line_stride
 // grid = (columns of a slab / W, slabs).  FINAL: the last pass of the step (lines along z).
-template <typename T, int N, bool IMAG, int MODE>
-__global__ void __launch_bounds__(ColGeom<T, N>::THREADS, (sizeof(T) == 4 ? GPE3_COL_MINB : 1)) k3_col(const Args3<T> a) {
+template <typename T, int N, bool IMAG, int MODE, bool WIDE>
+__global__ void __launch_bounds__(ColGeom3<T, N, WIDE>::THREADS, (sizeof(T) == 4 ? GPE3_COL_MINB : 1) * (256 / ColGeom3<T, N, WIDE>::THREADS)) k3_col(const Args3<T> a) {
     using C = cx<T>;
-    using G = ColGeom<T, N>;
+    using G = ColGeom3<T, N, WIDE>;
     using F = Fft1D<N, G::W, cx<T>>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
@@ -237,6 +268,8 @@ __global__ void __launch_bounds__(ColGeom<T, N>::THREADS, (sizeof(T) == 4 ? GPE3
     C *sm = smem + c;
     const long ls = a.line_stride;
     C v[16];
+    pdl_launch_dependents();
+    pdl_wait();
 #pragma unroll
     for (int k = 0; k < 16; ++k) v[k] = __ldcg(p + (long)(j + F::M1 * k) * ls);
     F::fwd(v, sm, j, a.tw, a.tw1);
@@ -298,8 +331,16 @@ template <bool IMAG>
 __global__ void __launch_bounds__(256) k3_finalize(State3 *st, const double *partials, unsigned int n, double dV,
                                                    long long step_index, double *record, int *nonfinite) {
     __shared__ double red[8];
+    pdl_launch_dependents();
+    pdl_wait();
     double t = 0.0;
-    for (unsigned int q = threadIdx.x; q < n; q += 256) t += partials[q];
+    for (unsigned int q0 = threadIdx.x; q0 < n; q0 += 4 * 256) {   // four loads in flight per thread, fixed order of the adds
+        double u[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { const unsigned int q = q0 + 256u * k; u[k] = q < n ? __ldcg(partials + q) : 0.0; }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) t += u[k];
+    }
     t = warp_sum(t);
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = t;
     __syncthreads();
@@ -385,31 +426,41 @@ __global__ void k3_make_tables(T *kin, T *k2, int n, double L, double dt, int im
 // ---------------------------------------------------------------- launchers of one (dtype, N)
 template <typename T> struct Ops3 {
     cudaError_t (*row)(const Args3<T> &, bool imag, int mode, cudaStream_t);                 // ny == N
-    cudaError_t (*col)(const Args3<T> &, bool imag, int mode, unsigned gx, unsigned gy, cudaStream_t);   // line length == N
-    int rows_per_cta, cols_per_cta;
+    // line length == N; cols columns per slab, slabs of them; returns the number of CTAs (= partial sums) in *nctas
+    cudaError_t (*col)(const Args3<T> &, bool imag, int mode, long cols, unsigned slabs, unsigned *nctas, cudaStream_t);
 };
 
 template <typename T, int N> struct Launch3 {
     using C = cx<T>;
-    static size_t row_smem() { return sizeof(C) * RowGeom<N>::RPC * Fft1D<N, 1, C>::SLOTS; }
-    static size_t col_smem() { return sizeof(C) * ColGeom<T, N>::W * Fft1D<N, 1, C>::SLOTS; }
+    static size_t row_smem() { return sizeof(C) * RowGeom3<N>::RPC * Fft1D<N, 1, C>::SLOTS; }
+    template <bool WIDE> static size_t col_smem() { return sizeof(C) * ColGeom3<T, N, WIDE>::W * Fft1D<N, 1, C>::SLOTS; }
     template <typename K> static cudaError_t go(K kern, dim3 grid, unsigned threads, size_t smem, cudaStream_t s, const Args3<T> &a) {
         cudaError_t e = Launch<T, N>::prep(kern, smem);
         if (e != cudaSuccess) return e;
-        kern<<<grid, threads, smem, s>>>(a);
-        return cudaGetLastError();
+        // grids up to GPE3_PDL_MAX points: the CTAs of a pass may be scheduled while the previous one drains
+        // (launch latency and prologue off the critical path); they block in pdl_wait() until it has completed
+        const bool pdl = (long)a.nx * a.ny * a.nz <= GPE3_PDL_MAX;
+        return launch_pdl(kern, grid, dim3(threads), smem, s, pdl, a);
     }
     static cudaError_t row(const Args3<T> &a, bool imag, int mode, cudaStream_t s) {
-        const dim3 grid((unsigned)((long)a.nz * a.nx / RowGeom<N>::RPC));
-        const unsigned th = RowGeom<N>::THREADS;
+        const dim3 grid((unsigned)((long)a.nz * a.nx / RowGeom3<N>::RPC));
+        const unsigned th = RowGeom3<N>::THREADS;
         if (mode == 1) return go(k3_row<T, N, false, 1>, grid, th, row_smem(), s, a);
         return imag ? go(k3_row<T, N, true, 0>, grid, th, row_smem(), s, a) : go(k3_row<T, N, false, 0>, grid, th, row_smem(), s, a);
     }
-    static cudaError_t col(const Args3<T> &a, bool imag, int mode, unsigned gx, unsigned gy, cudaStream_t s) {
-        const dim3 grid(gx, gy);
-        const unsigned th = ColGeom<T, N>::THREADS;
-        if (mode == 1) return go(k3_col<T, N, false, 1>, grid, th, col_smem(), s, a);
-        return imag ? go(k3_col<T, N, true, 0>, grid, th, col_smem(), s, a) : go(k3_col<T, N, false, 0>, grid, th, col_smem(), s, a);
+    // the wide tile where the lines of a 256-point column pass are at least 2 MB apart (see ColTarget3)
+    static bool col_wide(const Args3<T> &a) { return N == 256 && (size_t)a.line_stride * sizeof(C) >= (size_t)(2u << 20); }
+    template <bool WIDE> static cudaError_t col_w(const Args3<T> &a, bool imag, int mode, long cols, unsigned slabs, unsigned *nctas, cudaStream_t s) {
+        using G = ColGeom3<T, N, WIDE>;
+        const dim3 grid((unsigned)(cols / G::W), slabs);
+        if (nctas) *nctas = grid.x * grid.y;
+        if (mode == 1) return go(k3_col<T, N, false, 1, WIDE>, grid, G::THREADS, col_smem<WIDE>(), s, a);
+        return imag ? go(k3_col<T, N, true, 0, WIDE>, grid, G::THREADS, col_smem<WIDE>(), s, a)
+                    : go(k3_col<T, N, false, 0, WIDE>, grid, G::THREADS, col_smem<WIDE>(), s, a);
+    }
+    static cudaError_t col(const Args3<T> &a, bool imag, int mode, long cols, unsigned slabs, unsigned *nctas, cudaStream_t s) {
+        if constexpr (N == 256) { if (col_wide(a)) return col_w<true>(a, imag, mode, cols, slabs, nctas, s); }
+        return col_w<false>(a, imag, mode, cols, slabs, nctas, s);
     }
 };
 

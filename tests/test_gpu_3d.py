@@ -215,3 +215,15 @@ def test_largest_grid_properties():
     got = wave[17, 33, :].cpu().numpy().astype(np.complex128)
     assert np.abs(got - ref_line).max() <= 5e-6
     plan.close()
+
+
+@pytest.mark.parametrize("mode", ["real", "imag"])
+def test_graph_replay_with_records(mode):
+    """small grids replay eight plain steps from a CUDA graph; records, the first and the last step of a call stay
+    outside it: 45 steps with a record every 10, then a second call that continues the count"""
+    p = W.config3d(64, g=40.0, seed=8)
+    out, ref, rg, ro, og, oo = _run_both(p, "c128", mode, 1e-3, 45 + 27, record_every=10, chunks=2)
+    assert _rel(out, ref) <= 1e-11
+    assert rg.shape == ro.shape and np.array_equal(rg[:, 0], ro[:, 0]) and len(rg) == 7
+    assert np.abs(rg[:, 1:] / ro[:, 1:] - 1).max() <= 1e-11
+    _check_obs(og, oo, "c128")
