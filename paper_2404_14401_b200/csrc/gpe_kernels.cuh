@@ -37,15 +37,26 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
 }
 
 // ---------------------------------------------------------------- launch geometry
+// Threads per CTA of the one-number-per-element passes (complex128, and complex64 at 64 points): 128 for rows of
+// 256 points and more and for columns of 256 and 512 points, 256 otherwise.  Measured on B200 in complex128 (us per
+// step, 256 -> 128 threads): 512^2 27.6 -> 22.0, 1024^2 42.5 -> 41.7 (rows; narrower column tiles lose there: 19.1 ->
+// 20.4 us for pass B), 2048^2 135.5 -> 133.0 -- more, smaller CTAs overlap their load / transform / store phases.
+#ifndef GPE_ROWG_THREADS
+#define GPE_ROWG_THREADS 128
+#endif
+#ifndef GPE_COLG_THREADS
+#define GPE_COLG_THREADS 128
+#endif
 template <int N> struct RowGeom {
     static constexpr int TPF = N / 16;
-    static constexpr int RPC = (256 / TPF) < 1 ? 1 : (256 / TPF);  // rows per CTA
-    static constexpr int THREADS = RPC * TPF;                      // 256
+    static constexpr int TARGET = N >= 256 ? GPE_ROWG_THREADS : 256;
+    static constexpr int RPC = (TARGET / TPF) < 1 ? 1 : (TARGET / TPF);  // rows per CTA
+    static constexpr int THREADS = RPC * TPF;
 };
 template <typename T, int N> struct ColGeom {
     static constexpr int TPF = N / 16;
     static constexpr int WMIN = sizeof(T) == 4 ? 4 : 2;            // >= 32-byte row segments
-    static constexpr int W0 = 256 / TPF;
+    static constexpr int W0 = ((N >= 256 && N <= 512) ? GPE_COLG_THREADS : 256) / TPF;
     static constexpr int W = W0 < WMIN ? WMIN : W0;                // columns per CTA
     static constexpr int THREADS = W * TPF;
 };
@@ -418,7 +429,7 @@ __device__ __forceinline__ void potential_step16(cx<T> (&v)[P], const StepArgs<T
 // complex128 rows: two 256-thread CTAs per SM (128 registers) from 512 points up -- measured on B200:
 // 2048^2 real time 185 -> 157 us per step, 1024^2 53 -> 45; below 512 one CTA with all registers wins.
 template <typename T, int NY, bool IMAG>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1))) k_row_fwd(const StepArgs<T, cx<T>> a) {
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1)) * (256 / RowGeom<NY>::THREADS > 0 ? 256 / RowGeom<NY>::THREADS : 1)) k_row_fwd(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
@@ -459,7 +470,7 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
 // MODE 0: forward, kinetic factor, inverse (the step).  MODE 1: forward only, natural order
 // (observables).
 template <typename T, int NX, bool IMAG, int MODE>
-__global__ void __launch_bounds__(ColGeom<T, NX>::THREADS, 1) k_col(const StepArgs<T, cx<T>> a) {
+__global__ void __launch_bounds__(ColGeom<T, NX>::THREADS, (256 / ColGeom<T, NX>::THREADS > 0 ? 256 / ColGeom<T, NX>::THREADS : 1)) k_col(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using G = ColGeom<T, NX>;
     using F = Fft1D<NX, G::W, cx<T>>;
@@ -543,7 +554,7 @@ __global__ void __launch_bounds__(ColGeom<T, NX>::THREADS, 1) k_col(const StepAr
 
 // ---------------------------------------------------------------- pass C
 template <typename T, int NY, bool IMAG, bool MERGED>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1))) k_row_inv(const StepArgs<T, cx<T>> a) {
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1)) * (256 / RowGeom<NY>::THREADS > 0 ? 256 / RowGeom<NY>::THREADS : 1)) k_row_inv(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
@@ -592,7 +603,7 @@ __global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_RO
 // one step): load -> IFFT_y -> sum |psi|^2 -> both potential half-steps in one multiply -> FFT_y -> store.
 // The member's coefficients are read before the sums are published (the last CTA advances the state).
 template <typename T, int NY, bool IMAG>
-__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1))) k_row_ca(const StepArgs<T, cx<T>> a) {
+__global__ void __launch_bounds__(RowGeom<NY>::THREADS, (sizeof(T) == 4 ? GPE_ROW_MINB : (NY >= 512 ? 2 : 1)) * (256 / RowGeom<NY>::THREADS > 0 ? 256 / RowGeom<NY>::THREADS : 1)) k_row_ca(const StepArgs<T, cx<T>> a) {
     using C = cx<T>;
     using F = Fft1D<NY, 1, cx<T>>;
     using G = RowGeom<NY>;
