@@ -227,3 +227,35 @@ def test_graph_replay_with_records(mode):
     assert rg.shape == ro.shape and np.array_equal(rg[:, 0], ro[:, 0]) and len(rg) == 7
     assert np.abs(rg[:, 1:] / ro[:, 1:] - 1).max() <= 1e-11
     _check_obs(og, oo, "c128")
+
+
+def test_graph_survives_a_new_potential_a_new_dt_and_a_user_stream():
+    """the graph of plain steps holds g, dt/2 and the potential pointers as kernel arguments: a second
+    gpe3_set_potential, another dt and another wavefunction buffer must each rebuild it; all work on a user stream"""
+    import torch
+    import paper_2404_14401_b200 as G
+    from oracle.gpe3_oracle import Oracle3
+    p = W.config3d(64, g=30.0, seed=12)
+    q = W.config3d(64, g=75.0, seed=12, w2=(0.5, 2.0, 1.0), dimple=-1.0)
+    stream = torch.cuda.Stream()
+    plan = G.Plan3(64, 64, 64, p["Lx"], p["Ly"], p["Lz"], "c128", stream=stream.cuda_stream)
+    ref = p["psi0"].copy()
+    with torch.cuda.stream(stream):
+        psi = torch.from_numpy(p["psi0"].copy()).cuda()
+        plan.set_potential(p)
+        plan.evolve(psi, 1e-3, 20, "real")
+        plan.evolve(psi, 2e-3, 20, "real")          # another dt
+        plan.set_potential(q)                         # another potential and g
+        plan.evolve(psi, 2e-3, 20, "real")
+        psi2 = psi.clone()                            # another buffer
+        plan.evolve(psi2, 2e-3, 20, "imag")
+        plan.evolve(psi2, 2e-3, 20, "imag")
+    plan.synchronize()
+    o = Oracle3(p)
+    o.evolve(ref, 1e-3, 20, False); o.evolve(ref, 2e-3, 20, False)
+    o2 = Oracle3(q)
+    o2.evolve(ref, 2e-3, 20, False)
+    assert _rel(psi.cpu().numpy(), ref) <= 1e-11
+    o2.evolve(ref, 2e-3, 40, True)
+    assert _rel(psi2.cpu().numpy(), ref) <= 1e-11
+    plan.close()
