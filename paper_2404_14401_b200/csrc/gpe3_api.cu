@@ -219,7 +219,9 @@ gpe_status evolve3(gpe3_plan *p, void *psi, double dt, long long n_steps, int mo
         // a chunk of plain steps: no record falls on indices n+1 .. n+kGraphSteps, and in real time neither the first
         // step of the call (fac = 1) nor the last (it reduces the norm) is inside
         const bool no_rec = !recording || (n + kGraphSteps) / record_every == n / record_every;
-        if (use_graph && no_rec && (imag ? q + kGraphSteps <= n_steps : (q >= 1 && q + kGraphSteps <= n_steps - 1))) {
+        // (q >= 1 in both modes: the first step of a call is launched directly, so that one-time function attributes --
+        // not stream work -- are set outside the capture)
+        if (use_graph && no_rec && q >= 1 && q + kGraphSteps <= n_steps - (imag ? 0 : 1)) {
             if ((s = graph3<T>(p, base, imag, dt)) != GPE_OK) return s;
             GPE3_CUDA(p, cudaGraphLaunch(p->g_exec, p->stream));
             q += kGraphSteps;

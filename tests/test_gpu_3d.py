@@ -259,3 +259,14 @@ def test_graph_survives_a_new_potential_a_new_dt_and_a_user_stream():
     o2.evolve(ref, 2e-3, 40, True)
     assert _rel(psi2.cpu().numpy(), ref) <= 1e-11
     plan.close()
+
+
+def test_graph_with_large_tiles_first_in_a_fresh_plan():
+    """64 x 64 x 512 in complex128 is small enough for the step graph while its 512-point passes need more than 48 KB of
+    shared memory: the opt-in attribute must be set by a direct launch before the capture"""
+    p = W.config3d(64, 64, 512, g=20.0, seed=13)
+    out, ref, _, _, _, _ = _run_both(p, "c128", "imag", 1e-3, 20)
+    assert _rel(out, ref) <= 1e-11
+    p = W.config3d(512, 64, 64, g=20.0, seed=14)
+    out, ref, _, _, _, _ = _run_both(p, "c128", "real", 1e-3, 20)
+    assert _rel(out, ref) <= 1e-11
