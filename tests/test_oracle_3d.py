@@ -115,12 +115,12 @@ def test_ground_state_energy_limit():
     p.update(vx=0.5 * w[0] ** 2 * x * x, vy=0.5 * w[1] ** 2 * y * y, vz=0.5 * w[2] ** 2 * z * z)
     psi = _gauss(p, [0.6, 0.6, 0.6])
     o = Oracle3(p)
-    rec = o.evolve(psi, 0.02, 600, True, record_every=600)
+    rec = o.evolve(psi, 0.025, 300, True, record_every=300)
     ob = o.observables(psi)
     E = ob["e_kin"] + ob["e_pot"]
     assert E == pytest.approx(sum(w) / 2, abs=2e-4)
     # norm_pre of the last step: e^{-2 mu dt} up to O(dt^3)  ->  mu = E for g = 0
-    assert -math.log(rec[-1, 2]) / (2 * 0.02) == pytest.approx(sum(w) / 2, abs=2e-4)
+    assert -math.log(rec[-1, 2]) / (2 * 0.025) == pytest.approx(sum(w) / 2, abs=2e-4)
     assert rec[-1, 1] == pytest.approx(1.0, abs=1e-13)
 
 
