@@ -7,6 +7,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <functional>
 #include <string>
 #include <vector>
 
@@ -640,16 +641,49 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
         ah.kin_xc = (const cx<T> *)p->kinh_x; ah.kin_yc = (const cx<T> *)p->kinh_y;
         ah.kin_xr = (const T *)p->kinh_x; ah.kin_yr = (const T *)p->kinh_y;
         ah.kin_y2 = (const T *)p->kinh_y2;
-        auto unit = [&](StepArgs<T, cx<T>> u, T hdt_a, T hdt_c) -> gpe_status {
+        auto unit_on = [&](StepArgs<T, cx<T>> u, T hdt_a, T hdt_c, cudaStream_t st) -> gpe_status {
             u.src = (const cx<T> *)psi; u.dst = (cx<T> *)psi;
             u.half_dt = hdt_a;
             if (oop) u.dst = (cx<T> *)p->scratch;
-            GPE_CUDA(p, pass_a(u, p->stream));
+            GPE_CUDA(p, pass_a(u, st));
             if (oop) u.src = (const cx<T> *)p->scratch;
-            GPE_CUDA(p, pass_b(u, p->stream));
+            GPE_CUDA(p, pass_b(u, st));
             u.half_dt = hdt_c;
             if (oop) u.dst = (cx<T> *)psi;
-            GPE_CUDA(p, pass_c(u, p->stream));
+            GPE_CUDA(p, pass_c(u, st));
+            return GPE_OK;
+        };
+        auto unit = [&](StepArgs<T, cx<T>> u, T hdt_a, T hdt_c) -> gpe_status { return unit_on(u, hdt_a, hdt_c, p->stream); };
+        // The units of a chunk except its last are identical launches (all per-step state is on the device):
+        // kStepsPerGraph of them are captured once into a CUDA graph and replayed.  `plain` launches one on a stream;
+        // `kind` (2: real time, 3: imaginary time) keys the cached graph beside psi, dt, mode and the potential's epoch.
+        auto replay_plain = [&](long count, int kind, const std::function<gpe_status(cudaStream_t)> &plain) -> gpe_status {
+            long done_u = 0;
+            if (count >= 2 * kStepsPerGraph + 1) {
+                if (!(p->g_exec && p->g_psi == psi && p->g_dt == dt && p->g_mode == (int)mode && p->g_epoch == p->epoch && p->g_fused == kind)) {
+                    if (p->g_exec) { cudaGraphExecDestroy(p->g_exec); p->g_exec = nullptr; }
+                    if (!p->cap_stream) GPE_CUDA(p, cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
+                    gpe_status s1 = plain(p->stream);   // one-time function attributes outside the capture
+                    if (s1 != GPE_OK) return s1;
+                    done_u = 1;
+                    GPE_CUDA(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
+                    gpe_status cs = GPE_OK;
+                    for (int q = 0; q < kStepsPerGraph && cs == GPE_OK; ++q) cs = plain(p->cap_stream);
+                    cudaGraph_t graph = nullptr;
+                    cudaError_t ce = cudaStreamEndCapture(p->cap_stream, &graph);
+                    if (cs != GPE_OK) { if (graph) cudaGraphDestroy(graph); return cs; }
+                    if (ce != cudaSuccess) return cuda_fail(p, ce, "cudaStreamEndCapture");
+                    ce = cudaGraphInstantiate(&p->g_exec, graph, 0);
+                    cudaGraphDestroy(graph);
+                    if (ce != cudaSuccess) { p->g_exec = nullptr; return cuda_fail(p, ce, "cudaGraphInstantiate"); }
+                    p->g_psi = psi; p->g_dt = dt; p->g_mode = (int)mode; p->g_epoch = p->epoch; p->g_fused = kind;
+                }
+                for (; done_u + kStepsPerGraph <= count; done_u += kStepsPerGraph) GPE_CUDA(p, cudaGraphLaunch(p->g_exec, p->stream));
+            }
+            for (; done_u < count; ++done_u) {
+                gpe_status s1 = plain(p->stream);
+                if (s1 != GPE_OK) return s1;
+            }
             return GPE_OK;
         };
         // half a kinetic step, then the scalars of step `stepnow` from the psi it leaves (no advance)
@@ -675,8 +709,12 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
                     if (to_rec < chunk) chunk = to_rec;
                 }
                 if ((s = half_kinetic(stepnow, 1)) != GPE_OK) return s;
-                for (long i = 0; i < chunk; ++i) {
-                    StepArgs<T, cx<T>> u = (i == chunk - 1) ? ah : a;
+                {
+                    StepArgs<T, cx<T>> u = a;
+                    u.fin = a.fin; u.fin.merged = 1; u.fin.tvt = 1;
+                    s = replay_plain(chunk - 1, 2, [&](cudaStream_t st) { return unit_on(u, (T)(0.5 * dt), (T)(0.5 * dt), st); });
+                    if (s != GPE_OK) return s;
+                    u = ah;
                     u.fin = a.fin; u.fin.merged = 1; u.fin.tvt = 1;
                     if ((s = unit(u, (T)(0.5 * dt), (T)(0.5 * dt))) != GPE_OK) return s;
                 }
@@ -700,10 +738,13 @@ gpe_status evolve_impl(gpe_plan *p, void *psi, double dt, long n_steps, gpe_mode
                     if (to_rec < chunk) chunk = to_rec;
                 }
                 if ((s = half_kinetic(stepnow, 0)) != GPE_OK) return s;
-                for (long i = 0; i < chunk; ++i) {
+                {
                     StepArgs<T, cx<T>> u = ah;
                     u.fin = a.fin; u.fin.merged = 0; u.fin.tvt = 0; u.fin.prepared = 0;
-                    if (i < chunk - 1) { u.fin.knorm = 1; u.fin.cpmk = cpmk; }
+                    StepArgs<T, cx<T>> uk = u;
+                    uk.fin.knorm = 1; uk.fin.cpmk = cpmk;
+                    s = replay_plain(chunk - 1, 3, [&](cudaStream_t st) { return unit_on(uk, (T)dt, (T)0, st); });
+                    if (s != GPE_OK) return s;
                     if ((s = unit(u, (T)dt, (T)0)) != GPE_OK) return s;
                 }
                 done += chunk;
