@@ -277,7 +277,7 @@ GPE_API const char *gpe_noalloc_last_error(void);
  * Layout: psi and v_static are [nz][nx][ny], y fastest, z slowest.  No cavity terms, schedule or batch here.
  * A step is three passes over the array, one per axis (csrc/gpe3_kernels.cuh); nothing is transposed.
  *
- * gpe3_plan_create: nx, ny, nz each one of 64, 128, 256, 512 (else GPE_EUNSUPPORTED); Lx, Ly, Lz > 0 and finite,
+ * gpe3_plan_create: nx, ny, nz each one of 64, 128, 256, 512, 1024 (else GPE_EUNSUPPORTED); Lx, Ly, Lz > 0 and finite,
  * dtype as above (else GPE_EINVAL).  Allocates tables and a few KB of reduction scratch on the current device; the
  * caller owns psi.  *out is set only on GPE_OK; release with gpe3_plan_destroy (NULL is accepted).
  */

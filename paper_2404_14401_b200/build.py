@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libgpe.so")
 SIZES = (64, 128, 256, 512, 1024, 2048)
-SIZES3 = (64, 128, 256, 512)
+SIZES3 = (64, 128, 256, 512, 1024)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 

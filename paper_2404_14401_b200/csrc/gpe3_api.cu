@@ -70,7 +70,7 @@ gpe_status check_device3(gpe3_plan *p) {
 }
 
 size_t real_bytes3(const gpe3_plan *p) { return p->dtype == GPE_C64 ? 4 : 8; }
-bool size_ok3(int n) { return n == 64 || n == 128 || n == 256 || n == 512; }
+bool size_ok3(int n) { return n == 64 || n == 128 || n == 256 || n == 512 || n == 1024; }
 int axis_len(const gpe3_plan *p, int ax) { return ax == 0 ? p->nx : ax == 1 ? p->ny : p->nz; }
 double axis_box(const gpe3_plan *p, int ax) { return ax == 0 ? p->Lx : ax == 1 ? p->Ly : p->Lz; }
 
@@ -301,13 +301,17 @@ gpe_status gpe3_plan_create(gpe3_plan **out, int nx, int ny, int nz, double Lx, 
         return fail3(nullptr, GPE_EINVAL, "Lx, Ly, Lz must be finite and > 0");
     if (dtype != GPE_C64 && dtype != GPE_C128) return fail3(nullptr, GPE_EINVAL, "unknown dtype");
     if (!size_ok3(nx) || !size_ok3(ny) || !size_ok3(nz))
-        return fail3(nullptr, GPE_EUNSUPPORTED, "the 3-D path takes nx, ny, nz in {64, 128, 256, 512}");
+        return fail3(nullptr, GPE_EUNSUPPORTED, "the 3-D path takes nx, ny, nz in {64, 128, 256, 512, 1024}");
     gpe3_plan *p = new (std::nothrow) gpe3_plan;
     if (!p) return fail3(nullptr, GPE_ENOMEM, "host allocation failed");
     p->nx = nx; p->ny = ny; p->nz = nz; p->Lx = Lx; p->Ly = Ly; p->Lz = Lz; p->dtype = dtype;
     auto body = [&]() -> gpe_status {
         GPE3_CUDA(p, cudaGetDevice(&p->device));
-        const size_t nparts = 32768 + 64;
+        // one partial per CTA of any pass: at most one CTA per line of a face of the grid
+        size_t face = (size_t)nx * ny;
+        if ((size_t)ny * nz > face) face = (size_t)ny * nz;
+        if ((size_t)nz * nx > face) face = (size_t)nz * nx;
+        const size_t nparts = face + 64;
         GPE3_CUDA(p, cudaMalloc(&p->st, sizeof(State3)));
         GPE3_CUDA(p, cudaMalloc(&p->partials, sizeof(double) * nparts));
         GPE3_CUDA(p, cudaMalloc(&p->part6, sizeof(double) * 6 * kObsCtas));

@@ -471,15 +471,16 @@ GPE3_DECL_OPS(64)
 GPE3_DECL_OPS(128)
 GPE3_DECL_OPS(256)
 GPE3_DECL_OPS(512)
+GPE3_DECL_OPS(1024)
 #undef GPE3_DECL_OPS
 
 template <typename T> inline const Ops3<T> *get_ops3(int n);
 template <> inline const Ops3<float> *get_ops3<float>(int n) {
-    switch (n) { case 64: return &ops3_f_64; case 128: return &ops3_f_128; case 256: return &ops3_f_256; case 512: return &ops3_f_512; }
+    switch (n) { case 64: return &ops3_f_64; case 128: return &ops3_f_128; case 256: return &ops3_f_256; case 512: return &ops3_f_512; case 1024: return &ops3_f_1024; }
     return nullptr;
 }
 template <> inline const Ops3<double> *get_ops3<double>(int n) {
-    switch (n) { case 64: return &ops3_d_64; case 128: return &ops3_d_128; case 256: return &ops3_d_256; case 512: return &ops3_d_512; }
+    switch (n) { case 64: return &ops3_d_64; case 128: return &ops3_d_128; case 256: return &ops3_d_256; case 512: return &ops3_d_512; case 1024: return &ops3_d_1024; }
     return nullptr;
 }
 

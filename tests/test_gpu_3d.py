@@ -98,6 +98,17 @@ def test_lengths_256_and_512_on_x_and_rows(dtype):
 
 
 @pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_elongated_grids_1024(dtype):
+    """1024 points along each axis in turn (cigar-shaped traps): the longest line the 3-D passes take"""
+    for shape in ((1024, 64, 64), (64, 1024, 64), (64, 64, 1024)):
+        for mode in ("real", "imag"):
+            p = W.config3d(*shape, g=30.0, seed=6)
+            out, ref, _, _, og, oo = _run_both(p, dtype, mode, 1e-3, 4)
+            assert _rel(out, ref) <= _tol(dtype, 4), (shape, mode)
+            _check_obs(og, oo, dtype)
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
 def test_records_and_chunked_calls(dtype):
     """records of both time modes, and a run split over several calls equals one call (step counter, merged
     half-steps across the call boundary, lazy scale applied at the end of every imaginary-time call)"""
@@ -143,7 +154,7 @@ def test_no_potential_no_interaction_is_free_expansion():
 def test_boundary_errors():
     import torch
     import paper_2404_14401_b200 as G
-    for bad in ((96, 64, 64), (64, 32, 64), (64, 64, 1024)):
+    for bad in ((96, 64, 64), (64, 32, 64), (64, 64, 2048)):
         with pytest.raises(G.GpeError, match="GPE_EUNSUPPORTED"):
             G.Plan3(*bad, 1.0, 1.0, 1.0)
     with pytest.raises(G.GpeError, match="GPE_EINVAL"):
