@@ -33,9 +33,7 @@
 
 namespace gpe {
 
-// launch geometry of the 3-D passes: 256 threads per CTA from 256 points per line up (as the 2-D passes), 128 at 128
-// and 64 at 64 points, so that a 64^3 or 128^3 grid still gives every SM several CTAs (64^3 with 256-thread CTAs: 64
-// CTAs per pass on 148 SMs)
+// launch geometry of the 3-D passes (64^3 with 256-thread CTAs had 64 CTAs per pass on 148 SMs).
 // Threads per CTA by line length.  Rows: 64 at 64 points, 128 above (measured on B200, 256^3 complex64 real time
 // with 256 -> 128 threads in both kinds of pass: 245 -> 208 us per step, complex128 574 -> 419: more, smaller CTAs
 // overlap their load / transform / store phases better).  Columns of 256 points come in two widths: NARROW (128
@@ -353,25 +351,37 @@ __global__ void __launch_bounds__(256) k3_finalize(State3 *st, const double *par
 
 // ---------------------------------------------------------------- point-wise kernels
 // MODE 0: psi <- psi * exp(-i (V + g|psi|^2) dt/2) (the closing half-step of a real-time call)
-// MODE 1: psi <- psi * scale (end of an imaginary-time call); thread 0 of the grid... (scale is reset by k3_reset)
+// MODE 1: psi <- psi * scale (end of an imaginary-time call; the scale is reset by the next kernel on the stream)
+// Four independent points per thread and iteration, so that four loads are in flight per thread.
 template <typename T, int MODE>
 __global__ void __launch_bounds__(256) k3_point(const Args3<T> a) {
-    const long slab = (long)a.nx * a.ny, npts = slab * a.nz;
+    const long slab = (long)a.nx * a.ny, npts = slab * a.nz, stride = (long)gridDim.x * blockDim.x;
     const T s = MODE == 1 ? (T)a.st->scale : T(1);
-    for (long q = (long)blockIdx.x * blockDim.x + threadIdx.x; q < npts; q += (long)gridDim.x * blockDim.x) {
-        cx<T> z = a.psi[q];
-        if constexpr (MODE == 1) { z.x *= s; z.y *= s; }
-        else {
-            const int l = (int)(q / slab), rem = (int)(q % slab), i = rem / a.ny, y = rem % a.ny;
-            T V = a.vz[l] + a.vx[i] + a.vy[y];
-            if (a.v3d) V += a.v3d[q];
-            const T w = fma(a.g, z.x * z.x + z.y * z.y, V) * a.half_dt;
-            T sn, cm1;
-            sincosm1_t(-w, &sn, &cm1);
-            const T ox = fma(z.x, cm1, fma(-z.y, sn, z.x)), oy = fma(z.x, sn, fma(z.y, cm1, z.y));
-            z.x = ox; z.y = oy;
+    for (long q0 = (long)blockIdx.x * blockDim.x + threadIdx.x; q0 < npts; q0 += 4 * stride) {
+        cx<T> z[4];
+        T V[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const long q = q0 + k * stride;
+            z[k] = q < npts ? a.psi[q] : mk<T>(T(0), T(0));
+            if constexpr (MODE == 0) V[k] = (q < npts && a.v3d) ? a.v3d[q] : T(0);
         }
-        a.psi[q] = z;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const long q = q0 + k * stride;
+            if (q >= npts) break;
+            if constexpr (MODE == 1) { z[k].x *= s; z[k].y *= s; }
+            else {
+                const int l = (int)(q / slab), rem = (int)(q % slab), i = rem / a.ny, y = rem % a.ny;
+                const T Vt = V[k] + a.vz[l] + a.vx[i] + a.vy[y];
+                const T w = fma(a.g, z[k].x * z[k].x + z[k].y * z[k].y, Vt) * a.half_dt;
+                T sn, cm1;
+                sincosm1_t(-w, &sn, &cm1);
+                const T ox = fma(z[k].x, cm1, fma(-z[k].y, sn, z[k].x)), oy = fma(z[k].x, sn, fma(z[k].y, cm1, z[k].y));
+                z[k].x = ox; z[k].y = oy;
+            }
+            a.psi[q] = z[k];
+        }
     }
 }
 
