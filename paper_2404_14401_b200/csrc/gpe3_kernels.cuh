@@ -34,14 +34,15 @@
 namespace gpe {
 
 // launch geometry of the 3-D passes (64^3 with 256-thread CTAs had 64 CTAs per pass on 148 SMs).
-// Threads per CTA by line length.  Rows: 64 at 64 points, 128 above (measured on B200, 256^3 complex64 real time
-// with 256 -> 128 threads in both kinds of pass: 245 -> 208 us per step, complex128 574 -> 419: more, smaller CTAs
+// Threads per CTA by line length.  Rows: 64 at 64 points, 128 at 128, 64 again from 256 points up (measured on
+// B200, 256^3 complex64 real time, with 256 -> 128 threads in both kinds of pass: 245 -> 208 us per step, complex128 574 -> 419: more, smaller CTAs
 // overlap their load / transform / store phases better).  Columns of 256 points come in two widths: NARROW (128
 // threads, 8 columns) and WIDE (256 threads, 16 columns); narrow wins while the plane nx ny is small (256^3: 208
 // against 236 us) and loses when the lines are 2 MB apart (512 x 512 x 256: 1060 against 1013 us), see col_wide().
 #ifndef GPE3_ROW_T
-#define GPE3_ROW_T 128
-#endif
+#define GPE3_ROW_T 64     // rows of 256 points and more: 64 threads (4 rows of 256 points); against 128: 256^3 complex64
+#endif                    // 209.4 -> 206.1 us per step, 512 x 512 x 256 1013 -> 1000, complex128 imaginary time 488 -> 473
+
 template <int N> struct RowTarget3 { static constexpr int THREADS = N <= 64 ? 64 : (N <= 128 ? 128 : GPE3_ROW_T); };
 template <int N, bool WIDE> struct ColTarget3 { static constexpr int THREADS = N <= 64 ? 64 : (N <= 128 ? 128 : (N <= 256 ? (WIDE ? 256 : 128) : 256)); };
 template <int N> struct RowGeom3 {
