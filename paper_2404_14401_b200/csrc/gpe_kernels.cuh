@@ -37,12 +37,12 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
 }
 
 // ---------------------------------------------------------------- launch geometry
-// Threads per CTA of the one-number-per-element passes (complex128, and complex64 at 64 points): 128 for rows of
-// 256 points and more and for columns of 256 and 512 points, 256 otherwise.  Measured on B200 in complex128 (us per
+// Threads per CTA of the one-number-per-element passes (complex128, and complex64 at 64 points): 64 (or one row) for
+// rows of 256 points and more, 128 for columns of 256 and 512 points, 256 otherwise.  Measured on B200 in complex128 (us per
 // step, 256 -> 128 threads): 512^2 27.6 -> 22.0, 1024^2 42.5 -> 41.7 (rows; narrower column tiles lose there: 19.1 ->
 // 20.4 us for pass B), 2048^2 135.5 -> 133.0 -- more, smaller CTAs overlap their load / transform / store phases.
 #ifndef GPE_ROWG_THREADS
-#define GPE_ROWG_THREADS 128
+#define GPE_ROWG_THREADS 64    // 64 against 128: 1024^2 complex128 41.7 -> 40.2 us per step, 512^2 22.0 -> 21.7, 2048^2 unchanged
 #endif
 #ifndef GPE_COLG_THREADS
 #define GPE_COLG_THREADS 128
