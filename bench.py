@@ -237,8 +237,9 @@ def three_d(G, torch, hbm_peak, l2_peak, only=None):
     import numpy as np
     import workloads as W
     rows = []
-    cases = ((128, "c64", "real", 200), (128, "c64", "imag", 200), (256, "c64", "real", 40),
-             (256, "c64", "imag", 40), (256, "c128", "real", 20), (256, "c128", "imag", 20)) if only is None else (only,)
+    cases = ((64, "c64", "real", 400), (128, "c64", "real", 200), (128, "c64", "imag", 200), (256, "c64", "real", 40),
+             (256, "c64", "imag", 40), (256, "c128", "real", 20), (256, "c128", "imag", 20),
+             (512, "c64", "real", 6)) if only is None else (only,)
     for n, dtype, mode, steps in cases:
         p = W.config3d(n, dtype=dtype)
         cd = np.complex64 if dtype == "c64" else np.complex128
@@ -263,7 +264,8 @@ def three_d(G, torch, hbm_peak, l2_peak, only=None):
                      "updates_per_s": pts / (us * 1e-6), "algorithmic_bytes_per_point": bpp,
                      "bound": "l2" if in_l2 else "hbm", "byte_roof_gbs": roof,
                      "byte_roofline_frac": pts * bpp / (us * 1e-6) / 1e9 / roof,
-                     "gpu_launches_per_step": 4 if mode == "imag" else 3})
+                     "gpu_launches_per_step": 4 if mode == "imag" else 3,
+                     "replayed_from_graph": bool(pts <= 128 ** 3 and steps >= 16)})
     return rows
 
 
