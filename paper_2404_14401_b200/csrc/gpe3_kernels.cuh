@@ -252,10 +252,18 @@ __global__ void __launch_bounds__(RowGeom3<NY>::THREADS, (sizeof(T) == 4 ? GPE3_
     }
 }
 
+#ifndef GPE3_COL_D128
+#define GPE3_COL_D128 3   // resident 128-thread CTAs per SM asked of the compiler for the complex128 column passes (168 registers, no
+                          // spills; against 2: 256^3 414 -> 401 us per step real time, 471 -> 441 imaginary time)
+#endif
+template <typename T, int N, bool WIDE> constexpr int col_minb3() {
+    constexpr int th = ColGeom3<T, N, WIDE>::THREADS;
+    return sizeof(T) == 4 ? GPE3_COL_MINB * (256 / th) : (th == 128 ? GPE3_COL_D128 : 256 / th);
+}
 // ---------------------------------------------------------------- passes X and Z: lines of stride line_stride
 // grid = (columns of a slab / W, slabs).  FINAL: the last pass of the step (lines along z).
 template <typename T, int N, bool IMAG, int MODE, bool WIDE>
-__global__ void __launch_bounds__(ColGeom3<T, N, WIDE>::THREADS, (sizeof(T) == 4 ? GPE3_COL_MINB : 1) * (256 / ColGeom3<T, N, WIDE>::THREADS)) k3_col(const Args3<T> a) {
+__global__ void __launch_bounds__(ColGeom3<T, N, WIDE>::THREADS, col_minb3<T, N, WIDE>()) k3_col(const Args3<T> a) {
     using C = cx<T>;
     using G = ColGeom3<T, N, WIDE>;
     using F = Fft1D<N, G::W, cx<T>>;
