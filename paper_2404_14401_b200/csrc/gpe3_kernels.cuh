@@ -27,6 +27,11 @@
 #ifndef GPE3_ROW_MINB
 #define GPE3_ROW_MINB 3
 #endif
+// complex128 lines of 512 points and more in 128-thread column CTAs of four columns (64-byte row segments), two per SM,
+// instead of eight columns in 256 threads (measured: 512 x 512 x 256 2458 -> 2287 us per step, 256 x 256 x 512 1007 -> 931)
+#ifndef GPE3_COL_D512_NARROW
+#define GPE3_COL_D512_NARROW 1
+#endif
 #ifndef GPE3_PDL_MAX
 #define GPE3_PDL_MAX (128L * 128L * 128L)
 #endif
@@ -53,7 +58,8 @@ template <int N> struct RowGeom3 {
 template <typename T, int N, bool WIDE = false> struct ColGeom3 {
     static constexpr int TPF = N / 16;
     static constexpr int WMIN = sizeof(T) == 4 ? 4 : 2;            // >= 32-byte row segments
-    static constexpr int W0 = ColTarget3<N, WIDE>::THREADS / TPF;
+    // complex128 lines of 512 points and more: 128 threads (4 columns = 64-byte row segments)
+    static constexpr int W0 = ((sizeof(T) == 8 && N >= 512 && GPE3_COL_D512_NARROW) ? 128 : ColTarget3<N, WIDE>::THREADS) / TPF;
     static constexpr int W = W0 < WMIN ? WMIN : W0;                // columns per CTA
     static constexpr int THREADS = W * TPF;
 };
@@ -258,7 +264,7 @@ __global__ void __launch_bounds__(RowGeom3<NY>::THREADS, (sizeof(T) == 4 ? GPE3_
 #endif
 template <typename T, int N, bool WIDE> constexpr int col_minb3() {
     constexpr int th = ColGeom3<T, N, WIDE>::THREADS;
-    return sizeof(T) == 4 ? GPE3_COL_MINB * (256 / th) : (th == 128 ? GPE3_COL_D128 : 256 / th);
+    return sizeof(T) == 4 ? GPE3_COL_MINB * (256 / th) : (th == 128 ? (N <= 256 ? GPE3_COL_D128 : 2) : 256 / th);
 }
 // ---------------------------------------------------------------- passes X and Z: lines of stride line_stride
 // grid = (columns of a slab / W, slabs).  FINAL: the last pass of the step (lines along z).
